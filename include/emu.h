@@ -1,0 +1,138 @@
+/* emu.h - C ABI of libemu4pi: 4pi track finding over the 3D grain cloud of emulsion views
+ * (Ariga & Ariga, arXiv 1311.5334, section 2), hand-written CUDA for sm_100a (B200).
+ *
+ * Citations: P:NN = /root/reference/PAPER.md line NN; "reading Qn" = DESIGN.md section 3.
+ *
+ * Conventions for every call
+ *  - Pointers prefixed d_ are DEVICE pointers owned by the CALLER (e.g. torch.empty(..., device="cuda")).
+ *    `stream` is a cudaStream_t passed as void* (NULL = default stream).  The library keeps no global
+ *    state, allocates no persistent memory and is re-entrant per stream.
+ *  - Every call only ENQUEUES work on `stream` and returns without synchronising:
+ *      EMU_OK            0
+ *      EMU_ERR_INVALID  -1  null / misaligned pointer, bad params, a documented range violated
+ *      EMU_ERR_CAPACITY -2  workspace (or an output array) too small, detected on the host
+ *      EMU_ERR_CUDA     -3  a CUDA runtime call failed (cudaGetLastError != cudaSuccess)
+ *    Conditions only the device can see (too many candidates / tracks / members, coordinates out of
+ *    range) are reported in d_counts[EMU_CNT_STATUS]; outputs are then unspecified and the caller
+ *    retries with larger buffers.  No exceptions, no aborts, no printing.
+ *  - Units: q = 1/64 um; all coordinates int32.  |coordinate| < 2^17 (box <= 2^16 plus slack for
+ *    out-of-box grains) so that every product of the tube test fits in 64 bits.
+ *  - A "row" is a row index of the caller's d_grains array (the "original index" of a grain).
+ */
+#ifndef EMU_H_
+#define EMU_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define EMU_OK 0
+#define EMU_ERR_INVALID (-1)
+#define EMU_ERR_CAPACITY (-2)
+#define EMU_ERR_CUDA (-3)
+
+typedef struct emu_params {
+  int32_t struct_size;         /* = sizeof(emu_params): ABI check                                          */
+  int32_t view_size_q[3];      /* box [0,size) per axis; 1 <= size <= 65536 (1024 um)                      */
+  int32_t cell_size_q[3];      /* > 0.  Paper: 32 px x 32 px x 1 frame.  Has NO effect on the      */
+                               /* track list (reading Q10); it only steers the speed of the search.        */
+  int32_t sep_min_q;           /* seed <=> sep_min_q^2 <= D2 < sep_max_q^2 (reading Q1; "smaller      */
+  int32_t sep_max_q;           /*  than 25 um" = 1600).  1 <= sep_min_q < sep_max_q <= 2048                */
+  int32_t tube_r2_q;           /* tube radius squared, q^2; 0.8 um -> floor(0.64*4096) = 2621 (reading Q3) */
+  int32_t tube_ext_q;          /* -1 = count along the whole line (reading Q4).  >= 0: EMU_ERR_INVALID     */
+  int32_t min_grains;          /* threshold, >= 2: n >= min_grains (reading Q6; "e.g. 5")             */
+  int32_t max_tracks_per_view; /* capacity of the track list per view, 1..65536                            */
+  int32_t reserved[4];         /* [0] = expected candidates per grain used to size internal chunks         */
+                               /* (0 = default 48); the rest must be 0                                     */
+} emu_params;
+
+typedef struct emu_track {     /* 32 B */
+  int32_t view;
+  int32_t seed_a, seed_b;      /* rows of the two seed grains, seed_a < seed_b                             */
+  int32_t n_tube;              /* grains inside the tube of the seed line, seed grains included     */
+  int32_t n_members;           /* grains kept after the exclusive association                       */
+  int32_t member_off;          /* first member in d_members                                                */
+  int32_t seed_d2;             /* |B-A|^2 in q^2                                                           */
+  int32_t pad;                 /* 0                                                                        */
+} emu_track;
+
+typedef struct emu_fit {       /* 48 B */
+  int32_t axis;                /* dominant axis u: 0=x 1=y 2=z; |0x100 if all members share u (den = 0)    */
+  int32_t n;                   /* members                                                                  */
+  int32_t u_min, u_max;        /* extent of the members along u (segment start / end, Fig. 5), q      */
+  double slope[2], icpt[2];    /* minor coords (x,y | y,z | x,z for u = z | x | y) = slope*u + icpt, q     */
+} emu_fit;
+
+/* d_counts[8] (int64), written by emu_find_tracks / emu_count_seeds */
+#define EMU_CNT_SEEDS 0        /* grain pairs inside the separation window                          */
+#define EMU_CNT_TESTS 1        /* point-line tests executed (implementation figure, not compared)          */
+#define EMU_CNT_CANDIDATES 2   /* seeds with n_tube >= min_grains                                          */
+#define EMU_CNT_TRACKS 3
+#define EMU_CNT_MEMBERS 4
+#define EMU_CNT_STATUS 5       /* 0 = fine, else OR of the EMU_ST_* bits                                   */
+#define EMU_CNT_PAIR_TESTS 6   /* pair-distance tests executed (implementation figure)                     */
+#define EMU_CNT_NEED 7         /* largest candidate count one internal chunk needed                        */
+#define EMU_ST_CAND_OVERFLOW 1    /* candidate workspace too small: give more workspace / raise reserved[0] */
+#define EMU_ST_TRACK_OVERFLOW 2   /* a view has more than max_tracks_per_view tracks                       */
+#define EMU_ST_MEMBER_OVERFLOW 4  /* members_capacity too small                                            */
+#define EMU_ST_RANGE 8            /* a count does not fit its field (n_tube >= 8192)                       */
+#define EMU_ST_COORD 16           /* emu_bin_grains saw |coordinate| >= 2^17                               */
+
+/* Host-only (no CUDA call).  Workspace each call needs for this batch shape; both outputs optional.
+ * find_bytes is a recommendation (internal view chunks adapt to whatever >= the minimum is given). */
+int emu_workspace_bytes(const emu_params* params, int64_t n_grains, int32_t n_views,
+                        size_t* bin_bytes, size_t* find_bytes);
+
+/* Number of cells per view and grid dimensions, ceil(view_size/cell_size) per axis (the paper's
+ * geometry 1280x1024x40 with cells 32x32x1 gives 40x32x40 = 51 200).  Host-only. */
+int64_t emu_grid_cells(const emu_params* params, int32_t dims_out[3]);
+
+/* A1 "3D hash table" ("All recognized grains are then attributed to these cells").
+ *  in : d_grains  int32[n_grains][4] = x,y,z,w (w = caller payload, ignored), 16-byte aligned;
+ *       d_view_off int32[n_views+1], non-decreasing, [0] = 0, [n_views] = n_grains < 2^31.
+ *  out: d_sorted  int32[n_grains][4] = x,y,z,row ordered by (view, cell, row), where
+ *       cell = cx + nx*(cy + ny*cz), c = clamp(floor(coord/cell_size), 0, n-1) (out-of-box grains are
+ *       legal and land in the boundary cells, reading Q13);
+ *       d_cell_start int32[n_views*n_cells+1]: first position in d_sorted of every (view, cell).
+ *  d_status: int64[1], OR-ed with EMU_ST_COORD if a coordinate is out of range (may be d_counts+5).
+ *  d_ws / ws_bytes: scratch of at least the size emu_workspace_bytes reports. */
+int emu_bin_grains(const emu_params* params, const int32_t* d_grains, const int32_t* d_view_off,
+                   int64_t n_grains, int32_t n_views, int32_t* d_sorted, int32_t* d_cell_start,
+                   int64_t* d_status, void* d_ws, size_t ws_bytes, void* stream);
+
+/* A2..A5 + A7: seeds -> tube count -> threshold -> exclusive association -> threshold -> order
+ * (Fig. 4).
+ *  in : d_sorted, d_cell_start as written by emu_bin_grains with the SAME params; d_view_off.
+ *  out: d_tracks emu_track[<= n_views*max_tracks_per_view], written compactly: view v owns entries
+ *       d_track_off[v] .. d_track_off[v+1]-1, best first (reading Q7 order); d_track_off int32[n_views+1];
+ *       d_members int32[members_capacity]: rows, each track's members contiguous at member_off, ascending;
+ *       d_counts int64[8] (see EMU_CNT_*), zeroed by the call. */
+int emu_find_tracks(const emu_params* params, const int32_t* d_sorted, const int32_t* d_cell_start,
+                    const int32_t* d_view_off, int64_t n_grains, int32_t n_views,
+                    emu_track* d_tracks, int32_t* d_track_off, int32_t* d_members, int64_t members_capacity,
+                    int64_t* d_counts, void* d_ws, size_t ws_bytes, void* stream);
+
+/* A2 + A3 only, for per-seed parity checks: writes (view, row_a, row_b, n_tube), row_a < row_b, for
+ * every seed, in no particular order, to d_seed_dump int32[dump_capacity][4].  d_counts[EMU_CNT_SEEDS]
+ * receives the number of seeds (which may exceed dump_capacity; the excess is not written).
+ * d_ws: scratch of at least 32*n_views + 512 bytes. */
+int emu_count_seeds(const emu_params* params, const int32_t* d_sorted, const int32_t* d_cell_start,
+                    const int32_t* d_view_off, int64_t n_grains, int32_t n_views,
+                    int32_t* d_seed_dump, int64_t dump_capacity, int64_t* d_counts,
+                    void* d_ws, size_t ws_bytes, void* stream);
+
+/* A6 least-squares line per track (BASELINE.json north_star; reading Q9; not in the paper).
+ *  in : d_grains in ORIGINAL order (members are rows of it); tracks / offsets / members from
+ *       emu_find_tracks.  n_tracks is read on the device from d_track_off[n_views].
+ *  out: d_fits emu_fit[same capacity as d_tracks], entry t for track t. */
+int emu_fit_tracks(const emu_params* params, const int32_t* d_grains, const emu_track* d_tracks,
+                   const int32_t* d_track_off, const int32_t* d_members, int32_t n_views,
+                   emu_fit* d_fits, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* EMU_H_ */

@@ -1,0 +1,223 @@
+"""ctypes binding of include/emu.h.  Marshalling only: every step of the path runs in the CUDA kernels.
+
+Compute calls take torch CUDA tensors (caller-owned device memory) and enqueue on the current torch
+stream.  `run_path` is a convenience that allocates the outputs and calls the three entry points in
+order; it adds no arithmetic.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libemu4pi.so")
+
+EMU_CNT = dict(seeds=0, tests=1, candidates=2, tracks=3, members=4, status=5, pair_tests=6, need=7)
+EMU_ST = dict(cand_overflow=1, track_overflow=2, member_overflow=4, range=8, coord=16)
+_ERR = {-1: "EMU_ERR_INVALID", -2: "EMU_ERR_CAPACITY", -3: "EMU_ERR_CUDA"}
+
+TRACK_DTYPE = np.dtype([("view", "<i4"), ("seed_a", "<i4"), ("seed_b", "<i4"), ("n_tube", "<i4"),
+                        ("n_members", "<i4"), ("member_off", "<i4"), ("seed_d2", "<i4"), ("pad", "<i4")])
+FIT_DTYPE = np.dtype([("axis", "<i4"), ("n", "<i4"), ("u_min", "<i4"), ("u_max", "<i4"),
+                      ("slope", "<f8", (2,)), ("icpt", "<f8", (2,))])
+
+
+class EmuError(RuntimeError):
+    pass
+
+
+class emu_params(C.Structure):
+    _fields_ = [("struct_size", C.c_int32), ("view_size_q", C.c_int32 * 3), ("cell_size_q", C.c_int32 * 3),
+                ("sep_min_q", C.c_int32), ("sep_max_q", C.c_int32), ("tube_r2_q", C.c_int32),
+                ("tube_ext_q", C.c_int32), ("min_grains", C.c_int32), ("max_tracks_per_view", C.c_int32),
+                ("reserved", C.c_int32 * 4)]
+
+
+_SYMBOLS = ["emu_workspace_bytes", "emu_grid_cells", "emu_bin_grains", "emu_find_tracks", "emu_count_seeds",
+            "emu_fit_tracks"]
+_lib = None
+
+
+def library_path() -> str:
+    return _LIB_PATH
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_LIB_PATH):
+            raise EmuError(f"{_LIB_PATH} is missing: build it with `python -m paper_1311_5334_b200.build` "
+                           "(or __graft_entry__.build()).  There is no CPU fallback.")
+        L = C.CDLL(_LIB_PATH)
+        vp, i64, i32, sz = C.c_void_p, C.c_int64, C.c_int32, C.c_size_t
+        L.emu_workspace_bytes.restype = C.c_int
+        L.emu_workspace_bytes.argtypes = [vp, i64, i32, C.POINTER(sz), C.POINTER(sz)]
+        L.emu_grid_cells.restype = i64
+        L.emu_grid_cells.argtypes = [vp, C.POINTER(i32 * 3)]
+        L.emu_bin_grains.restype = C.c_int
+        L.emu_bin_grains.argtypes = [vp, vp, vp, i64, i32, vp, vp, vp, vp, sz, vp]
+        L.emu_find_tracks.restype = C.c_int
+        L.emu_find_tracks.argtypes = [vp, vp, vp, vp, i64, i32, vp, vp, vp, i64, vp, vp, sz, vp]
+        L.emu_count_seeds.restype = C.c_int
+        L.emu_count_seeds.argtypes = [vp, vp, vp, vp, i64, i32, vp, i64, vp, vp, sz, vp]
+        L.emu_fit_tracks.restype = C.c_int
+        L.emu_fit_tracks.argtypes = [vp, vp, vp, vp, vp, i32, vp, vp]
+        _lib = L
+    return _lib
+
+
+def exported_symbols() -> list:
+    """Names include/emu.h declares, each resolved in the loaded library (raises if one is missing)."""
+    L = _load()
+    for s in _SYMBOLS:
+        getattr(L, s)
+    return list(_SYMBOLS)
+
+
+def make_params(view_size_q, cell_size_q, sep_min_q, sep_max_q, tube_r2_q, min_grains,
+                max_tracks_per_view=4096, tube_ext_q=-1, cand_per_grain=0) -> emu_params:
+    p = emu_params()
+    p.struct_size = C.sizeof(emu_params)
+    p.view_size_q[:] = [int(x) for x in view_size_q]
+    p.cell_size_q[:] = [int(x) for x in cell_size_q]
+    p.sep_min_q, p.sep_max_q, p.tube_r2_q = int(sep_min_q), int(sep_max_q), int(tube_r2_q)
+    p.tube_ext_q, p.min_grains, p.max_tracks_per_view = int(tube_ext_q), int(min_grains), int(max_tracks_per_view)
+    p.reserved[0] = int(cand_per_grain)
+    return p
+
+
+def _check(rc: int, what: str):
+    if rc != 0:
+        raise EmuError(f"{what} returned {_ERR.get(rc, rc)}")
+
+
+def _ptr(t):
+    return C.c_void_p(t.data_ptr()) if t is not None else C.c_void_p(0)
+
+
+def _stream():
+    import torch
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def _dev(t, dtype=None):
+    if not t.is_cuda or not t.is_contiguous() or (dtype is not None and t.dtype != dtype):
+        raise EmuError("expected a contiguous CUDA tensor of the documented dtype")
+    return t
+
+
+def _nbytes(t) -> int:
+    return t.numel() * t.element_size()
+
+
+def emu_workspace_bytes(params: emu_params, n_grains: int, n_views: int):
+    b, f = C.c_size_t(0), C.c_size_t(0)
+    _check(_load().emu_workspace_bytes(C.byref(params), n_grains, n_views, C.byref(b), C.byref(f)),
+           "emu_workspace_bytes")
+    return int(b.value), int(f.value)
+
+
+def emu_grid_cells(params: emu_params):
+    dims = (C.c_int32 * 3)()
+    n = _load().emu_grid_cells(C.byref(params), C.byref(dims))
+    if n < 0:
+        raise EmuError("emu_grid_cells: bad params")
+    return int(n), tuple(int(x) for x in dims)
+
+
+def emu_bin_grains(params, d_grains, d_view_off, n_grains, n_views, d_sorted, d_cell_start, d_status, d_ws):
+    import torch
+    _dev(d_grains, torch.int32); _dev(d_view_off, torch.int32); _dev(d_sorted, torch.int32)
+    _dev(d_cell_start, torch.int32); _dev(d_status, torch.int64); _dev(d_ws)
+    _check(_load().emu_bin_grains(C.byref(params), _ptr(d_grains), _ptr(d_view_off), n_grains, n_views,
+                                  _ptr(d_sorted), _ptr(d_cell_start), _ptr(d_status), _ptr(d_ws), _nbytes(d_ws),
+                                  _stream()), "emu_bin_grains")
+
+
+def emu_find_tracks(params, d_sorted, d_cell_start, d_view_off, n_grains, n_views, d_tracks, d_track_off, d_members,
+                    d_counts, d_ws):
+    import torch
+    _dev(d_sorted, torch.int32); _dev(d_cell_start, torch.int32); _dev(d_view_off, torch.int32)
+    _dev(d_tracks, torch.int32); _dev(d_track_off, torch.int32); _dev(d_members, torch.int32)
+    _dev(d_counts, torch.int64); _dev(d_ws)
+    _check(_load().emu_find_tracks(C.byref(params), _ptr(d_sorted), _ptr(d_cell_start), _ptr(d_view_off), n_grains,
+                                   n_views, _ptr(d_tracks), _ptr(d_track_off), _ptr(d_members), d_members.numel(),
+                                   _ptr(d_counts), _ptr(d_ws), _nbytes(d_ws), _stream()), "emu_find_tracks")
+
+
+def emu_count_seeds(params, d_sorted, d_cell_start, d_view_off, n_grains, n_views, d_seed_dump, d_counts, d_ws):
+    import torch
+    _dev(d_sorted, torch.int32); _dev(d_cell_start, torch.int32); _dev(d_view_off, torch.int32)
+    _dev(d_seed_dump, torch.int32); _dev(d_counts, torch.int64); _dev(d_ws)
+    _check(_load().emu_count_seeds(C.byref(params), _ptr(d_sorted), _ptr(d_cell_start), _ptr(d_view_off), n_grains,
+                                   n_views, _ptr(d_seed_dump), d_seed_dump.numel() // 4, _ptr(d_counts), _ptr(d_ws),
+                                   _nbytes(d_ws), _stream()), "emu_count_seeds")
+
+
+def emu_fit_tracks(params, d_grains, d_tracks, d_track_off, d_members, n_views, d_fits):
+    import torch
+    _dev(d_grains, torch.int32); _dev(d_tracks, torch.int32); _dev(d_track_off, torch.int32)
+    _dev(d_members, torch.int32); _dev(d_fits)
+    _check(_load().emu_fit_tracks(C.byref(params), _ptr(d_grains), _ptr(d_tracks), _ptr(d_track_off),
+                                  _ptr(d_members), n_views, _ptr(d_fits), _stream()), "emu_fit_tracks")
+
+
+class PathBuffers:
+    """Caller-owned device memory for a batch shape, allocated once with torch and reused per step."""
+
+    def __init__(self, params: emu_params, n_grains: int, n_views: int, members_capacity: int | None = None,
+                 find_ws_bytes: int | None = None, device="cuda"):
+        import torch
+        self.params, self.n_grains, self.n_views = params, n_grains, n_views
+        ncell, _ = emu_grid_cells(params)
+        bin_b, find_b = emu_workspace_bytes(params, n_grains, n_views)
+        if find_ws_bytes is not None:
+            find_b = find_ws_bytes
+        cap = max(n_views * params.max_tracks_per_view, 1)
+
+        def e(n, dt):
+            return torch.empty(n, dtype=dt, device=device)
+        self.sorted = torch.empty((max(n_grains, 1), 4), dtype=torch.int32, device=device)
+        self.cell_start = e(n_views * ncell + 1, torch.int32)
+        self.tracks = torch.empty((cap, 8), dtype=torch.int32, device=device)
+        self.track_off = e(n_views + 1, torch.int32)
+        self.members = e(max(members_capacity if members_capacity is not None else n_grains, 1), torch.int32)
+        self.fits = e(cap * FIT_DTYPE.itemsize, torch.uint8)
+        self.counts = torch.zeros(8, dtype=torch.int64, device=device)
+        self.status = torch.zeros(1, dtype=torch.int64, device=device)
+        self.ws = e(max(bin_b, find_b), torch.uint8)
+
+
+@dataclass
+class PathResult:
+    """Device buffers of one pass of the path; .host() copies the valid parts back."""
+    buffers: PathBuffers
+
+    def host(self) -> dict:
+        B = self.buffers
+        counts = B.counts.cpu().numpy().copy()
+        counts[EMU_CNT["status"]] |= int(B.status.cpu()[0])
+        nt, nm = int(counts[EMU_CNT["tracks"]]), int(counts[EMU_CNT["members"]])
+        nm = min(nm, B.members.numel())
+        tracks = B.tracks[:nt].cpu().numpy().view(TRACK_DTYPE).reshape(-1)
+        fits = B.fits[:nt * FIT_DTYPE.itemsize].cpu().numpy().view(FIT_DTYPE).reshape(-1)
+        return dict(tracks=tracks, fits=fits, members=B.members[:nm].cpu().numpy(),
+                    track_off=B.track_off.cpu().numpy(), counts=counts,
+                    sorted=B.sorted, cell_start=B.cell_start)
+
+
+def run_path(params: emu_params, d_grains, d_view_off, n_views: int, buffers: PathBuffers | None = None,
+             fit: bool = True) -> PathResult:
+    """One pass of the hot path on the current stream: emu_bin_grains -> emu_find_tracks -> emu_fit_tracks."""
+    n_grains = int(d_grains.shape[0])
+    B = buffers if buffers is not None else PathBuffers(params, n_grains, n_views, device=d_grains.device)
+    B.status.zero_()
+    emu_bin_grains(params, d_grains, d_view_off, n_grains, n_views, B.sorted, B.cell_start, B.status, B.ws)
+    emu_find_tracks(params, B.sorted, B.cell_start, d_view_off, n_grains, n_views, B.tracks, B.track_off, B.members,
+                    B.counts, B.ws)
+    if fit:
+        emu_fit_tracks(params, d_grains, B.tracks, B.track_off, B.members, n_views, B.fits)
+    return PathResult(B)

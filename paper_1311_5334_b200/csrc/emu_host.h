@@ -1,0 +1,34 @@
+// emu_host.h - host-side helpers and the launcher prototypes behind the C ABI (emu_api.cu).
+#pragma once
+#include <cuda_runtime.h>
+#include <stddef.h>
+#include <stdint.h>
+
+#include "emu_dev.cuh"
+
+static inline size_t emu_align256(size_t x) { return (x + 255) & ~(size_t)255; }
+static inline void* emu_align_ptr(void* p) { return (void*)(((uintptr_t)p + 255) & ~(uintptr_t)255); }
+static inline int64_t emu_min64(int64_t a, int64_t b) { return a < b ? a : b; }
+static inline int64_t emu_max64(int64_t a, int64_t b) { return a > b ? a : b; }
+
+// emu_bin.cu
+size_t emu_bin_ws_bytes(const EmuDev& P, int64_t n_grains, int32_t n_views);
+int emu_bin_launch(const EmuDev& P, const int32_t* d_grains, const int32_t* d_view_off, int64_t n_grains,
+                   int32_t n_views, int32_t* d_sorted, int32_t* d_cell_start, int64_t* d_status, void* d_ws,
+                   size_t ws_bytes, cudaStream_t st);
+
+// emu_find.cu
+size_t emu_find_ws_min_bytes(const EmuDev& P, int64_t n_grains, int32_t n_views);
+size_t emu_find_ws_recommended_bytes(const EmuDev& P, int64_t n_grains, int32_t n_views, int cand_per_grain);
+int emu_find_launch(const EmuDev& P, int cand_per_grain, const int32_t* d_sorted, const int32_t* d_cell_start,
+                    const int32_t* d_view_off, int64_t n_grains, int32_t n_views, emu_track* d_tracks,
+                    int32_t* d_track_off, int32_t* d_members, int64_t members_capacity, int64_t* d_counts,
+                    void* d_ws, size_t ws_bytes, cudaStream_t st);
+int emu_count_seeds_launch(const EmuDev& P, const int32_t* d_sorted, const int32_t* d_cell_start,
+                           const int32_t* d_view_off, int64_t n_grains, int32_t n_views, int32_t* d_seed_dump,
+                           int64_t dump_capacity, int64_t* d_counts, void* d_ws, size_t ws_bytes,
+                           cudaStream_t st);
+
+// emu_fit.cu
+int emu_fit_launch(const int32_t* d_grains, const emu_track* d_tracks, const int32_t* d_track_off,
+                   const int32_t* d_members, int32_t n_views, emu_fit* d_fits, cudaStream_t st);

@@ -1,0 +1,157 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element.
+
+Bars (north_star): track lists, offsets, member lists, per-seed counts and the binning output are
+bit-exact (integer work); fitted slopes / intercepts agree within 1e-5 relative.
+"""
+import json
+import os
+
+import numpy as np
+import pytest
+
+from emu_synth import CONFIGS, default_params, make_batch, make_config, noiseless_track_view
+from gpu_helpers import assert_same_tracks, run_gpu, seed_dump_gpu
+
+pytestmark = pytest.mark.gpu
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+@pytest.fixture(scope="module")
+def E():
+    import torch
+    assert torch.cuda.is_available(), "the gpu tests need a CUDA device"
+    import paper_1311_5334_b200 as E
+    E.exported_symbols()
+    return E
+
+
+def _mess_up(g, size_q):
+    """push a share of the grains outside the box (legal, reading Q13) and set junk payloads"""
+    g = g.copy()
+    g[::7, 0] -= size_q[0] // 3; g[::11, 1] += size_q[1] // 2; g[::13, 2] -= 4000
+    g[:, 3] = np.arange(len(g))[::-1] * 7 + 3
+    return g
+
+
+@pytest.mark.parametrize("cfg,cell_um,messy", [(0, (8.0, 8.0, 8.0), False), (0, (3.0, 17.0, 5.5), True),
+                                               (1, (8.0, 8.0, 8.0), False), (1, (4.0, 4.0, 4.0), True),
+                                               (3, (40.0, 2.0, 60.0), False)])
+def test_binning_bit_exact(E, oracle_mod, cfg, cell_um, messy):
+    b = make_batch(CONFIGS[cfg], cfg, n_views=3 if cfg == 0 else 1)
+    p = default_params(cfg, cell_um=cell_um)
+    g = _mess_up(b.grains, p["view_size_q"]) if messy else b.grains
+    srt, cs = oracle_mod.bin_grains(p, g, b.view_off)
+    import torch
+    prm = E.make_params(**{k: p[k] for k in ("view_size_q", "cell_size_q", "sep_min_q", "sep_max_q", "tube_r2_q", "min_grains")})
+    B = E.PathBuffers(prm, len(g), b.n_views)
+    E.emu_bin_grains(prm, torch.from_numpy(np.ascontiguousarray(g)).cuda(), torch.from_numpy(b.view_off).cuda(),
+                     len(g), b.n_views, B.sorted, B.cell_start, B.status, B.ws)
+    torch.cuda.synchronize()
+    assert int(B.status.cpu()[0]) == 0
+    assert np.array_equal(B.cell_start.cpu().numpy(), cs)
+    assert np.array_equal(B.sorted.cpu().numpy(), srt)
+
+
+@pytest.mark.parametrize("cfg", [0, 1, 2, 3])
+def test_per_seed_counts_bit_exact(E, config_oracle, cfg):
+    b, p, ref = config_oracle(cfg)
+    dump, counts = seed_dump_gpu(E, p, b.grains, b.view_off, ref.counters["seeds"] + 16)
+    assert int(counts[E.EMU_CNT["seeds"]]) == ref.counters["seeds"]
+    a = dump[np.lexsort((dump[:, 2], dump[:, 1], dump[:, 0]))]
+    r = ref.seed_dump[np.lexsort((ref.seed_dump[:, 2], ref.seed_dump[:, 1], ref.seed_dump[:, 0]))]
+    assert np.array_equal(a, r)
+
+
+@pytest.mark.parametrize("cfg", [0, 1, 2, 3])
+def test_track_list_bit_exact(E, config_oracle, cfg):
+    b, p, ref = config_oracle(cfg)
+    got = run_gpu(E, p, b.grains, b.view_off)
+    assert_same_tracks(E, got, ref)
+    assert len(got["tracks"]) > 0
+
+
+@pytest.mark.parametrize("cell_um", [(4.0, 4.0, 4.0), (2.0, 16.0, 3.0), (100.0, 100.0, 50.0), (1.0, 9.0, 25.0)])
+def test_cell_size_has_no_effect_on_gpu(E, config_oracle, cell_um):
+    b, p, ref = config_oracle(0)
+    got = run_gpu(E, default_params(0, cell_um=cell_um), b.grains, b.view_off)
+    assert_same_tracks(E, got, ref)
+
+
+def test_batch_of_views_in_several_chunks(E, oracle_mod):
+    """7 views of config 0; a tight workspace forces several internal chunks; track_off/member_off continue."""
+    b = make_batch(CONFIGS[0], 0, n_views=7)
+    p = default_params(0)
+    ref = oracle_mod.track_views(p, b.grains, b.view_off, "cells", 0)
+    prm = E.make_params(**{k: p[k] for k in ("view_size_q", "cell_size_q", "sep_min_q", "sep_max_q", "tube_r2_q", "min_grains")})
+    _, rec = E.emu_workspace_bytes(prm, b.n_grains, b.n_views)
+    for ws in (None, rec // 3):
+        got = run_gpu(E, p, b.grains, b.view_off, find_ws_bytes=ws)
+        assert_same_tracks(E, got, ref)
+
+
+def test_out_of_box_grains_and_payload_ignored(E, oracle_mod):
+    b = make_config(0)
+    p = default_params(0)
+    g = _mess_up(b.grains, p["view_size_q"])
+    ref = oracle_mod.track_views(p, g, b.view_off, "cells", 1)
+    assert_same_tracks(E, run_gpu(E, p, g, b.view_off), ref)
+
+
+def test_e1_and_ties(E, oracle_mod):
+    """The constructed example and noiseless equally spaced tracks: every candidate ties on (n_tube, D2)
+    with others, so the (kmin, kmax) tie path decides."""
+    with open(os.path.join(HERE, "golden", "e1_constructed_example.json")) as f:
+        e1 = json.load(f)
+    g = np.zeros((len(e1["grains"]), 4), np.int32); g[:, :3] = e1["grains"]
+    off = np.asarray([0, len(g)], np.int32)
+    got = run_gpu(E, e1["params"], g, off)
+    ref = oracle_mod.track_views(e1["params"], g, off, "brute", 1)
+    assert_same_tracks(E, got, ref)
+    t = got["tracks"][0]
+    assert (int(t["seed_a"]), int(t["seed_b"]), int(t["n_tube"])) == (0, 3, 10)
+
+    lines = []
+    for d, s in (((300, 0, 0), (500, 4000, 1600)), ((0, 280, 40), (4000, 600, 300)), ((170, 170, 170), (900, 900, 200)),
+                 ((300, 0, 0), (500, 4000, 1650))):          # the last one runs 50 q beside the first: shared grains
+        lines.append([(s[0] + i * d[0], s[1] + i * d[1], s[2] + i * d[2]) for i in range(14)])
+    b = noiseless_track_view((8000, 8000, 3200), lines, n_fog=300)
+    p = dict(e1["params"], view_size_q=(8000, 8000, 3200))
+    ref = oracle_mod.track_views(p, b.grains, b.view_off, "brute", 1)
+    assert len(ref.tracks) >= 3
+    assert_same_tracks(E, run_gpu(E, p, b.grains, b.view_off), ref)
+
+
+def test_degenerate_inputs(E, oracle_mod):
+    p = default_params(0)
+    # no grains at all, one view / three views with an empty one in the middle / a single grain
+    for grains, off in ((np.zeros((0, 4), np.int32), [0, 0]),
+                        (make_config(0).grains, None),
+                        (np.asarray([[5, 5, 5, 0]], np.int32), [0, 1])):
+        if off is None:
+            n = len(grains)
+            off = [0, n // 2, n // 2, n]
+        off = np.asarray(off, np.int32)
+        ref = oracle_mod.track_views(p, grains, off, "cells", 1)
+        got = run_gpu(E, p, grains, off)
+        assert_same_tracks(E, got, ref)
+    # all grains coincide (D2 = 0 is never a seed, reading Q12) / all in one cell
+    g = np.zeros((50, 4), np.int32); g[:, :3] = (777, 888, 999)
+    off = np.asarray([0, 50], np.int32)
+    assert_same_tracks(E, run_gpu(E, p, g, off), oracle_mod.track_views(p, g, off, "brute", 1))
+    b = make_config(0)
+    p1 = default_params(0, cell_um=(200.0, 200.0, 100.0))
+    assert_same_tracks(E, run_gpu(E, p1, b.grains, b.view_off), oracle_mod.track_views(p1, b.grains, b.view_off, "cells", 1))
+
+
+def test_capacity_and_range_errors_are_reported(E):
+    import torch
+    b = make_config(0)
+    p = default_params(0, max_tracks_per_view=3)
+    got = run_gpu(E, p, b.grains, b.view_off)
+    assert int(got["counts"][E.EMU_CNT["status"]]) & E.EMU_ST["track_overflow"]
+    g = b.grains.copy(); g[5, 0] = 1 << 17
+    got = run_gpu(E, default_params(0), g, b.view_off)
+    assert int(got["counts"][E.EMU_CNT["status"]]) & E.EMU_ST["coord"]
+    prm = E.make_params((6400, 6400, 3200), (512, 512, 512), 256, 1280, 2621, 8, tube_ext_q=100)
+    with pytest.raises(E.EmuError):
+        E.emu_workspace_bytes(prm, 10, 1)
