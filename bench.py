@@ -1,0 +1,338 @@
+#!/usr/bin/env python
+"""bench.py - one "step" = one pass of the whole hot path (A1 bin -> A2..A5,A7 find -> A6 fit) over the
+throughput batch of BASELINE.json configs[4]: 1,024 independent views of 350x300x50 um, fog 10 per 1000 um^3,
+300 isotropic through-going tracks per view (about 64 k grains per view, 66 M grains per GPU), seeded synthetic.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--views V] [--impl reference]
+
+N > 1 is launched by torchrun, one rank per GPU; every rank processes its own V views (weak scaling, no
+data-path collective - the views are independent).  Rank 0 prints ONE JSON line.
+`--impl reference` times the CPU oracle (oracle/) on a bounded sample of the same workload instead.
+DESIGN.md section 8 states every formula used here.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+CFG = 4                          # BASELINE.json configs[4] "throughput batch"
+CELL_UM = (8.0, 8.0, 8.0)        # cell size of the 3D hash (a pure speed knob: no effect on the track list)
+VIEW_AREA_CM2 = 350e-4 * 300e-4  # 350 x 300 um = 1.05e-3 cm^2 per view
+# Algorithmic work of the voting kernel: lane-instructions per seed
+#   = tests/seed * 18 + pair-tests/seed * 9, with tests/seed and pair-tests/seed the ORACLE's own counters
+# (oracle mode "cells", same cell size) on views 0..7 of this workload.  The cpu_baseline leg re-measures
+# them live; the constants serve the runs that have no such leg (N > 1).
+ALG_PER_SEED = {(8.0, 8.0, 8.0): (317.7, 2.88)}
+INSTR_PER_TEST, INSTR_PER_PAIR = 18, 9
+BIN_BYTES_PER_GRAIN = 32.7       # 16 B read + 16 B written + 4 B per cell
+
+
+def _gen_view(v):
+    from emu_synth import CONFIGS, make_view
+    g, _, _ = make_view(CONFIGS[CFG], CFG, v)
+    return g
+
+
+def make_workload(first_view: int, n_views: int):
+    """grains int32 [N,4], view_off int32 [n_views+1] for views first_view.. of config 4 (key (4, v))."""
+    import multiprocessing as mp
+    nproc = max(1, min(len(os.sched_getaffinity(0)), 32, n_views))
+    if nproc > 1:
+        with mp.get_context("fork").Pool(nproc) as pool:
+            gs = pool.map(_gen_view, range(first_view, first_view + n_views), chunksize=max(1, n_views // (4 * nproc)))
+    else:
+        gs = [_gen_view(v) for v in range(first_view, first_view + n_views)]
+    off = np.zeros(n_views + 1, np.int32)
+    off[1:] = np.cumsum([len(g) for g in gs])
+    return np.concatenate(gs), off
+
+
+def params_dict():
+    from emu_synth import default_params
+    return default_params(CFG, cell_um=CELL_UM, max_tracks_per_view=4096)
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc, self.thread = index, [], None, None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+            return
+        self.thread = threading.Thread(target=self._read, daemon=True)
+        self.thread.start()
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        for r in self.rows:
+            if len(r) < 7:
+                continue
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1])); pw.append(float(r[2]))
+            except ValueError:
+                continue
+            for name, val in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def measured_peaks() -> dict:
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        d["_source"] = "measured"
+        return d
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "_source": "fallback"}
+
+
+def oracle_sample(n_sample_views: int, threads: int):
+    """The oracle as it stands (mode 'cells', g++ -O2, one OpenMP thread per view) on the first views of the
+    workload.  Returns (seconds, grains, counters)."""
+    import oracle
+    oracle.build()
+    grains, off = make_workload(0, n_sample_views)
+    t0 = time.perf_counter()
+    r = oracle.track_views(params_dict(), grains, off, "cells", threads)
+    dt = time.perf_counter() - t0
+    return dt, int(off[-1]), r.counters
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle on the host cores, same metric / unit / config."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    cores = len(os.sched_getaffinity(0))
+    nv = args.sample_views if args.sample_views else max(1, min(cores, 16))
+    times = []
+    cnt, ng = None, 0
+    for _ in range(args.warmup if args.reference_warmup else 0):
+        oracle_sample(nv, cores)
+    for _ in range(max(1, min(args.steps, args.reference_steps))):
+        dt, ng, cnt = oracle_sample(nv, cores)
+        times.append(dt)
+    t = float(np.mean(times))
+    val = ng / t
+    line = {
+        "impl": "reference", "metric": "grains_per_s", "value": val, "unit": "grains/s", "n_gpus": args.gpus,
+        "steps": len(times), "warmup": 0, "ms_per_step": t * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "int64", "data": "synthetic",
+        "config": workload_config(nv, 1),
+        "views_per_s": nv / t, "cm2_per_hour": nv / t * 3600 * VIEW_AREA_CM2,
+        "cpu_baseline": {"value": val, "unit": "grains/s", "cores": min(cores, nv), "kind": "oracle",
+                         "sample": f"views 0..{nv - 1} of the workload ({ng} grains), one OpenMP thread per view, "
+                                   f"oracle mode 'cells' at cell {CELL_UM} um; each step = this sample"},
+        "e2e": {"value": val, "unit": "grains/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "oracle_counters": cnt,
+    }
+    print(json.dumps(line))
+
+
+def workload_config(views_per_gpu: int, n_gpus: int) -> dict:
+    return {"workload": "BASELINE.json configs[4] throughput batch: independent 350x300x50 um views, fog 10/1000 um^3, "
+                        "300 isotropic through tracks per view, int32 coords at 1/64 um, seeded synthetic (key (4, view))",
+            "views_per_gpu": views_per_gpu, "views_total": views_per_gpu * n_gpus,
+            "tracking": "tube r2 2621 q^2 (0.8 um), pair separation 256..1280 q (4..20 um), min 8 grains, whole-line tube",
+            "cell_um": list(CELL_UM), "parallelism": f"views sharded over {n_gpus} GPU(s), no collective",
+            "l2": "inputs (about 1 GB of grains per step) exceed the 126 MB L2; no flush needed"}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--views", type=int, default=1024, help="views per GPU (BASELINE.json configs[4]: 1024)")
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--sample-views", type=int, default=0, help="views in the oracle sample (default: one per core, <= 16)")
+    ap.add_argument("--reference-steps", type=int, default=2)
+    ap.add_argument("--reference-warmup", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+        return
+
+    import torch
+    import torch.distributed as dist
+    import paper_1311_5334_b200 as E   # raises if libemu4pi.so is missing: there is no fallback
+    E.exported_symbols()
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    assert world == args.gpus, f"--gpus {args.gpus} but WORLD_SIZE={world}: launch with torchrun"
+
+    p = params_dict()
+    V = args.views
+    grains, off = make_workload(rank * V, V)
+    n = int(off[-1])
+    prm = E.make_params(**{k: p[k] for k in ("view_size_q", "cell_size_q", "sep_min_q", "sep_max_q", "tube_r2_q",
+                                             "min_grains", "max_tracks_per_view")})
+    d_grains = torch.from_numpy(grains).cuda()
+    d_off = torch.from_numpy(off).cuda()
+    B = E.PathBuffers(prm, n, V)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        E.run_path(prm, d_grains, d_off, V, B)
+    barrier()
+    counts = B.counts.cpu().numpy().copy()
+    status = int(counts[E.EMU_CNT["status"]]) | int(B.status.cpu()[0])
+    assert status == 0, f"device status {status} (capacity / range): the step is not valid"
+
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    prof = E.Profile()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    ev0.record()
+    with prof:
+        for _ in range(args.steps):
+            E.run_path(prm, d_grains, d_off, V, B)
+    ev1.record()
+    barrier()
+    ms_total = ev0.elapsed_time(ev1)
+    clocks = sampler.stop() if rank == 0 else None
+    stage_ms, stage_launches = prof.read()
+    t_ms = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t_ms, op=dist.ReduceOp.MAX)
+    ms_total = float(t_ms.item())
+    n_all = torch.tensor([n], dtype=torch.int64, device="cuda")
+    if world > 1:
+        dist.all_reduce(n_all, op=dist.ReduceOp.SUM)
+    n_total = int(n_all.item())
+    ms_step = ms_total / args.steps
+    counts = B.counts.cpu().numpy().copy()
+
+    # end to end: ONE C-ABI call on pinned host buffers per step (H2D + path + D2H inside the call)
+    e2e = None
+    if not args.no_e2e:
+        H = E.HostPath(prm, n, V)
+        H.h_grains[:n].copy_(torch.from_numpy(grains))
+        H.h_view_off.copy_(torch.from_numpy(off))
+        nt, nm = H.call()                                   # warm-up
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            nt, nm = H.call()                               # synchronous: returns with the outputs on the host
+        barrier()
+        dt = time.perf_counter() - t0
+        t_e = torch.tensor([dt], dtype=torch.float64, device="cuda")
+        if world > 1:
+            dist.all_reduce(t_e, op=dist.ReduceOp.MAX)
+        e2e = {"value": n_total * args.steps / float(t_e.item()), "unit": "grains/s",
+               "h2d_bytes_per_step": H.h2d_bytes(), "d2h_bytes_per_step": H.d2h_bytes(nt, nm),
+               "ms_per_step": float(t_e.item()) / args.steps * 1e3,
+               "call": "emu_track_views_host (pinned host buffers; copies inside the timed call)"}
+        assert int(H.h_counts[E.EMU_CNT["status"]]) == 0
+        assert nt == int(counts[E.EMU_CNT["tracks"]]), "host path and device path disagree"
+        del H
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    peaks = measured_peaks()
+    seeds = int(counts[E.EMU_CNT["seeds"]])
+    cpu = None
+    alg = ALG_PER_SEED.get(tuple(CELL_UM))
+    if world == 1 and not args.no_cpu_baseline:
+        cores = len(os.sched_getaffinity(0))
+        nv_s = args.sample_views if args.sample_views else max(1, min(cores, 16, V))
+        dt, ng, cnt = oracle_sample(nv_s, cores)
+        cpu = {"value": ng / dt, "unit": "grains/s", "cores": min(cores, nv_s), "kind": "oracle",
+               "sample": f"views 0..{nv_s - 1} of the workload ({ng} grains), one OpenMP thread per view, oracle mode "
+                         f"'cells' at cell {CELL_UM} um, {dt:.1f} s",
+               "views_per_s": nv_s / dt}
+        alg = (cnt["tube_tests"] / cnt["seeds"], cnt["pair_tests"] / cnt["seeds"])
+
+    sm_max = float(peaks.get("sm_max_mhz") or 1965.0)
+    alu_peak = 148 * 4 * 32 * sm_max * 1e6 / 1e12            # Tlane-instr/s
+    vote_ms = stage_ms["vote"] / max(1, stage_launches["vote"])
+    roofline = None
+    if alg is not None and stage_launches["vote"]:
+        alg_instr = seeds * (alg[0] * INSTR_PER_TEST + alg[1] * INSTR_PER_PAIR)   # per step, all vote launches
+        achieved = alg_instr / (stage_ms["vote"] / args.steps * 1e-3) / 1e12
+        roofline = {"kernel": "k_vote", "bound": "alu", "achieved": achieved, "peak": alu_peak,
+                    "unit": "Tlane-instr/s", "frac": achieved / alu_peak, "traffic": None,
+                    "peak_source": f"148 SM x 4 schedulers x 32 lanes x {sm_max:.0f} MHz ({peaks['_source']} max SM clock)",
+                    "algorithmic": f"{seeds} seeds x ({alg[0]:.1f} tests x {INSTR_PER_TEST} + {alg[1]:.2f} pair tests x "
+                                   f"{INSTR_PER_PAIR}) lane-instr, oracle counters at the same cell size",
+                    "launches_per_step": stage_launches["vote"] / args.steps, "avg_launch_ms": vote_ms,
+                    "share_of_step": stage_ms["vote"] / args.steps / ms_step}
+    bin_ms = sum(stage_ms[k] for k in ("bin_count", "bin_scan", "bin_scatter", "bin_place")) / args.steps
+    hbm = float(peaks["hbm_gbs"])
+    bin_gbs = BIN_BYTES_PER_GRAIN * n / (bin_ms * 1e-3) / 1e9 if bin_ms > 0 else 0.0
+    roofline_bin = {"kernel": "emu_bin_grains (count+scan+scatter+place)", "bound": "hbm", "achieved": bin_gbs,
+                    "peak": hbm, "unit": "GB/s", "frac": bin_gbs / hbm, "traffic": None, "ms": bin_ms,
+                    "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peaks['_source']})"}
+
+    val = n_total / (ms_step * 1e-3)
+    line = {
+        "metric": "grains_per_s", "value": val, "unit": "grains/s", "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "int32", "data": "synthetic", "config": workload_config(V, world),
+        "views_per_s": V * world / (ms_step * 1e-3),
+        "cm2_per_hour": V * world / (ms_step * 1e-3) * 3600 * VIEW_AREA_CM2,
+        "grains_per_gpu": n, "seeds": seeds, "candidates": int(counts[E.EMU_CNT["candidates"]]),
+        "tracks": int(counts[E.EMU_CNT["tracks"]]),
+        "gpu_launches": int(sum(stage_launches.values())),
+        "stage_ms_per_step": {k: v / args.steps for k, v in stage_ms.items()},
+        "roofline": roofline, "roofline_bin": roofline_bin, "cpu_baseline": cpu, "e2e": e2e, "clocks": clocks,
+    }
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

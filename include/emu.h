@@ -132,6 +132,51 @@ int emu_fit_tracks(const emu_params* params, const int32_t* d_grains, const emu_
                    const int32_t* d_track_off, const int32_t* d_members, int32_t n_views,
                    emu_fit* d_fits, void* stream);
 
+/* ---- the whole path on HOST buffers (the end-to-end call: copies in, A1..A7, copies out) --------
+ * h_* are HOST pointers owned by the caller (pinned memory makes the copies asynchronous and fast;
+ * pageable memory works).  d_arena is one caller-owned DEVICE allocation of at least
+ * emu_host_arena_bytes() bytes from which the call carves every device buffer it needs (input copy,
+ * sorted grains, cell_start, outputs, workspaces).  Unlike the device calls above this one is
+ * SYNCHRONOUS: it enqueues the host->device copies, emu_bin_grains, emu_find_tracks and
+ * emu_fit_tracks on `stream`, reads d_counts back, copies the valid part of every output to the
+ * host and returns after the stream has drained.
+ *  out: h_tracks[<= tracks_capacity], h_fits[<= tracks_capacity], h_track_off[n_views+1],
+ *       h_members[<= members_capacity], h_counts[8] (EMU_CNT_*; status includes EMU_ST_COORD).
+ *  Returns EMU_ERR_CAPACITY if the arena or a host output array is too small for what was found
+ *  (h_counts then still holds the required sizes), else as the device calls. */
+int emu_host_arena_bytes(const emu_params* params, int64_t n_grains, int32_t n_views, size_t* arena_bytes);
+int emu_track_views_host(const emu_params* params, const int32_t* h_grains, const int32_t* h_view_off,
+                         int64_t n_grains, int32_t n_views, emu_track* h_tracks, emu_fit* h_fits,
+                         int64_t tracks_capacity, int32_t* h_track_off, int32_t* h_members,
+                         int64_t members_capacity, int64_t* h_counts, void* d_arena, size_t arena_bytes,
+                         void* stream);
+
+/* ---- optional per-stage timing (measurement aid for bench.py) -------------
+ * An emu_profile is a host-side object that owns CUDA events.  Between emu_profile_begin(p) and
+ * emu_profile_end() every kernel the library launches FROM THE CALLING HOST THREAD is bracketed by
+ * a pair of events on its launch stream and counted under its stage; nothing else changes (same
+ * kernels, same launch configuration).  This is the only state the library keeps, and only while
+ * the caller asks for it.  emu_profile_read synchronises on the recorded events and ADDS, per
+ * stage, the elapsed milliseconds to ms[EMU_STAGE_COUNT] and the launch counts to
+ * launches[EMU_STAGE_COUNT] (either may be NULL), then forgets the recorded events. */
+#define EMU_STAGE_BIN_COUNT 0    /* A1 histogram                                                    */
+#define EMU_STAGE_BIN_SCAN 1     /* A1 exclusive scan -> cell_start                                 */
+#define EMU_STAGE_BIN_SCATTER 2  /* A1 scatter into cell order                                      */
+#define EMU_STAGE_BIN_PLACE 3    /* A1 canonical order inside a cell                                */
+#define EMU_STAGE_PREP 4         /* bounding boxes, resets, bookkeeping kernels                     */
+#define EMU_STAGE_VOTE 5         /* A2 + A3 + A4: seeds, tube count, threshold (the hot loop)       */
+#define EMU_STAGE_ASSOC 6        /* A5: exclusive association (priority max, tie settlement)        */
+#define EMU_STAGE_SELECT 7       /* A5: wins per candidate, threshold again                         */
+#define EMU_STAGE_EMIT 8         /* A7: ordered track list and member lists                         */
+#define EMU_STAGE_FIT 9          /* A6                                                              */
+#define EMU_STAGE_COUNT 16
+typedef struct emu_profile emu_profile;
+emu_profile* emu_profile_create(void);              /* NULL on failure                              */
+void emu_profile_destroy(emu_profile* p);           /* p may be NULL                                */
+int emu_profile_begin(emu_profile* p);              /* EMU_ERR_INVALID if p is NULL or one is active */
+int emu_profile_end(void);
+int emu_profile_read(emu_profile* p, double* ms, int64_t* launches);
+
 #ifdef __cplusplus
 }
 #endif

@@ -37,7 +37,10 @@ class emu_params(C.Structure):
 
 
 _SYMBOLS = ["emu_workspace_bytes", "emu_grid_cells", "emu_bin_grains", "emu_find_tracks", "emu_count_seeds",
-            "emu_fit_tracks"]
+            "emu_fit_tracks", "emu_host_arena_bytes", "emu_track_views_host", "emu_profile_create", "emu_profile_destroy", "emu_profile_begin", "emu_profile_end",
+            "emu_profile_read"]
+EMU_STAGE = dict(bin_count=0, bin_scan=1, bin_scatter=2, bin_place=3, prep=4, vote=5, assoc=6, select=7, emit=8, fit=9)
+EMU_STAGE_COUNT = 16
 _lib = None
 
 
@@ -65,6 +68,20 @@ def _load():
         L.emu_count_seeds.argtypes = [vp, vp, vp, vp, i64, i32, vp, i64, vp, vp, sz, vp]
         L.emu_fit_tracks.restype = C.c_int
         L.emu_fit_tracks.argtypes = [vp, vp, vp, vp, vp, i32, vp, vp]
+        L.emu_host_arena_bytes.restype = C.c_int
+        L.emu_host_arena_bytes.argtypes = [vp, i64, i32, C.POINTER(sz)]
+        L.emu_track_views_host.restype = C.c_int
+        L.emu_track_views_host.argtypes = [vp, vp, vp, i64, i32, vp, vp, i64, vp, vp, i64, vp, vp, sz, vp]
+        L.emu_profile_create.restype = vp
+        L.emu_profile_create.argtypes = []
+        L.emu_profile_destroy.restype = None
+        L.emu_profile_destroy.argtypes = [vp]
+        L.emu_profile_begin.restype = C.c_int
+        L.emu_profile_begin.argtypes = [vp]
+        L.emu_profile_end.restype = C.c_int
+        L.emu_profile_end.argtypes = []
+        L.emu_profile_read.restype = C.c_int
+        L.emu_profile_read.argtypes = [vp, vp, vp]
         _lib = L
     return _lib
 
@@ -163,6 +180,103 @@ def emu_fit_tracks(params, d_grains, d_tracks, d_track_off, d_members, n_views, 
     _dev(d_members, torch.int32); _dev(d_fits)
     _check(_load().emu_fit_tracks(C.byref(params), _ptr(d_grains), _ptr(d_tracks), _ptr(d_track_off),
                                   _ptr(d_members), n_views, _ptr(d_fits), _stream()), "emu_fit_tracks")
+
+
+def emu_host_arena_bytes(params: emu_params, n_grains: int, n_views: int) -> int:
+    b = C.c_size_t(0)
+    _check(_load().emu_host_arena_bytes(C.byref(params), n_grains, n_views, C.byref(b)), "emu_host_arena_bytes")
+    return int(b.value)
+
+
+class HostPath:
+    """emu_track_views_host with its buffers: pinned host arrays for inputs / outputs and one device arena,
+    allocated once for a batch shape.  run() copies the caller's grains into the pinned input, makes the ONE
+    C-ABI call (H2D, bin, find, fit, D2H inside it) and returns numpy views of the pinned outputs."""
+
+    def __init__(self, params: emu_params, n_grains: int, n_views: int, tracks_capacity: int | None = None):
+        import torch
+        self.params, self.n_grains, self.n_views = params, n_grains, n_views
+        tcap = tracks_capacity if tracks_capacity is not None else max(n_views, 1) * params.max_tracks_per_view
+        self.tcap = tcap
+
+        def pin(shape, dt):
+            return torch.empty(shape, dtype=dt, pin_memory=True)
+        self.h_grains = pin((max(n_grains, 1), 4), torch.int32)
+        self.h_view_off = pin(n_views + 1, torch.int32)
+        self.h_tracks = pin((max(tcap, 1), 8), torch.int32)
+        self.h_fits = pin(max(tcap, 1) * FIT_DTYPE.itemsize, torch.uint8)
+        self.h_track_off = pin(n_views + 1, torch.int32)
+        self.h_members = pin(max(n_grains, 1), torch.int32)
+        self.h_counts = pin(8, torch.int64)
+        self.arena = torch.empty(emu_host_arena_bytes(params, n_grains, n_views), dtype=torch.uint8, device="cuda")
+
+    def h2d_bytes(self) -> int:
+        return self.n_grains * 16 + (self.n_views + 1) * 4
+
+    def call(self):
+        """the C-ABI call alone, on what already sits in the pinned input arrays"""
+        rc = _load().emu_track_views_host(C.byref(self.params), C.c_void_p(self.h_grains.data_ptr()),
+                                          C.c_void_p(self.h_view_off.data_ptr()), self.n_grains, self.n_views,
+                                          C.c_void_p(self.h_tracks.data_ptr()), C.c_void_p(self.h_fits.data_ptr()),
+                                          self.tcap, C.c_void_p(self.h_track_off.data_ptr()),
+                                          C.c_void_p(self.h_members.data_ptr()), self.h_members.numel(),
+                                          C.c_void_p(self.h_counts.data_ptr()), _ptr(self.arena), _nbytes(self.arena),
+                                          _stream())
+        _check(rc, "emu_track_views_host")
+        c = self.h_counts.numpy()
+        nt, nm = int(c[EMU_CNT["tracks"]]), int(c[EMU_CNT["members"]])
+        return nt, nm
+
+    def d2h_bytes(self, nt: int, nm: int) -> int:
+        return 64 + 8 + (self.n_views + 1) * 4 + nt * (TRACK_DTYPE.itemsize + FIT_DTYPE.itemsize) + nm * 4
+
+    def run(self, grains: np.ndarray, view_off: np.ndarray) -> dict:
+        import torch
+        if self.n_grains:
+            self.h_grains[:self.n_grains].copy_(torch.from_numpy(np.ascontiguousarray(grains, np.int32).reshape(-1, 4)))
+        self.h_view_off.copy_(torch.from_numpy(np.ascontiguousarray(view_off, np.int32)))
+        nt, nm = self.call()
+        return dict(tracks=self.h_tracks[:nt].numpy().view(TRACK_DTYPE).reshape(-1).copy(),
+                    fits=self.h_fits[:nt * FIT_DTYPE.itemsize].numpy().view(FIT_DTYPE).reshape(-1).copy(),
+                    members=self.h_members[:nm].numpy().copy(), track_off=self.h_track_off.numpy().copy(),
+                    counts=self.h_counts.numpy().copy())
+
+
+class Profile:
+    """emu_profile_* of include/emu.h: per-stage CUDA-event timing of the library's own launches.
+
+    with Profile() as prof: ...calls...; prof.read() -> ({stage: ms}, {stage: launches}) accumulated."""
+
+    def __init__(self):
+        self._h = _load().emu_profile_create()
+        if not self._h:
+            raise EmuError("emu_profile_create failed")
+        self.ms = np.zeros(EMU_STAGE_COUNT, np.float64)
+        self.launches = np.zeros(EMU_STAGE_COUNT, np.int64)
+
+    def __enter__(self):
+        _check(_load().emu_profile_begin(self._h), "emu_profile_begin")
+        return self
+
+    def __exit__(self, *exc):
+        _load().emu_profile_end()
+        return False
+
+    def read(self):
+        _check(_load().emu_profile_read(self._h, self.ms.ctypes.data, self.launches.ctypes.data), "emu_profile_read")
+        inv = {v: k for k, v in EMU_STAGE.items()}
+        return ({inv[i]: float(self.ms[i]) for i in inv}, {inv[i]: int(self.launches[i]) for i in inv})
+
+    def close(self):
+        if self._h:
+            _load().emu_profile_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
 
 
 class PathBuffers:

@@ -2,6 +2,9 @@
 // the path runs in the kernels of emu_bin.cu / emu_find.cu / emu_fit.cu.
 #include <math.h>
 
+#include <new>
+#include <vector>
+
 #include "emu_dev.cuh"
 #include "emu_host.h"
 
@@ -52,7 +55,58 @@ int cand_per_grain(const emu_params* p) { return p->reserved[0] > 0 ? p->reserve
 
 }  // namespace
 
+// ---- per-stage timing ---------------------------------------------------------------------------
+struct emu_profile {
+  struct Rec { int stage; cudaEvent_t a, b; };
+  std::vector<Rec> recs;              // recorded since the last read
+  std::vector<cudaEvent_t> pool;      // events free for reuse
+  cudaEvent_t take() {
+    if (!pool.empty()) { cudaEvent_t e = pool.back(); pool.pop_back(); return e; }
+    cudaEvent_t e = nullptr;
+    cudaEventCreate(&e);
+    return e;
+  }
+};
+static thread_local emu_profile* g_prof = nullptr;
+emu_profile* emu_prof_current() { return g_prof; }
+void emu_prof_before(emu_profile* p, int stage, cudaStream_t st) {
+  emu_profile::Rec r; r.stage = stage; r.a = p->take(); r.b = p->take();
+  cudaEventRecord(r.a, st);
+  p->recs.push_back(r);
+}
+void emu_prof_after(emu_profile* p, int, cudaStream_t st) { cudaEventRecord(p->recs.back().b, st); }
+
 extern "C" {
+
+emu_profile* emu_profile_create(void) { return new (std::nothrow) emu_profile(); }
+void emu_profile_destroy(emu_profile* p) {
+  if (!p) return;
+  if (g_prof == p) g_prof = nullptr;
+  for (auto& r : p->recs) { cudaEventDestroy(r.a); cudaEventDestroy(r.b); }
+  for (auto e : p->pool) cudaEventDestroy(e);
+  delete p;
+}
+int emu_profile_begin(emu_profile* p) {
+  if (!p || g_prof) return EMU_ERR_INVALID;
+  g_prof = p;
+  return EMU_OK;
+}
+int emu_profile_end(void) { g_prof = nullptr; return EMU_OK; }
+int emu_profile_read(emu_profile* p, double* ms, int64_t* launches) {
+  if (!p) return EMU_ERR_INVALID;
+  int rc = EMU_OK;
+  for (auto& r : p->recs) {
+    float t = 0.f;
+    if (cudaEventSynchronize(r.b) != cudaSuccess || cudaEventElapsedTime(&t, r.a, r.b) != cudaSuccess) rc = EMU_ERR_CUDA;
+    if (r.stage >= 0 && r.stage < EMU_STAGE_COUNT) {
+      if (ms) ms[r.stage] += (double)t;
+      if (launches) launches[r.stage] += 1;
+    }
+    p->pool.push_back(r.a); p->pool.push_back(r.b);
+  }
+  p->recs.clear();
+  return rc;
+}
 
 int emu_workspace_bytes(const emu_params* params, int64_t n_grains, int32_t n_views, size_t* bin_bytes,
                         size_t* find_bytes) {
@@ -114,6 +168,88 @@ int emu_count_seeds(const emu_params* params, const int32_t* d_sorted, const int
   if (!aligned16(d_sorted) || !aligned16(d_seed_dump)) return EMU_ERR_INVALID;
   return emu_count_seeds_launch(d, d_sorted, d_cell_start, d_view_off, n_grains, n_views, d_seed_dump, dump_capacity,
                                 d_counts, d_ws, ws_bytes, (cudaStream_t)stream);
+}
+
+namespace {
+struct HostArena {
+  int32_t *grains, *view_off, *sorted, *cell_start, *track_off, *members;
+  emu_track* tracks; emu_fit* fits; int64_t* counts; int64_t* status; void* ws;
+  size_t ws_bytes, total;
+};
+// carve (base may be NULL: then only the sizes are computed)
+void carve_host_arena(const emu_params* p, const EmuDev& d, int64_t n, int32_t nv, char* base, HostArena& A) {
+  size_t off = 0;
+  auto take = [&](size_t bytes) { char* r = base ? base + off : nullptr; off += emu_align256(bytes ? bytes : 1); return r; };
+  const size_t tcap = (size_t)(nv > 0 ? nv : 1) * (size_t)p->max_tracks_per_view;
+  A.grains = (int32_t*)take((size_t)n * 16);
+  A.view_off = (int32_t*)take(((size_t)nv + 1) * 4);
+  A.sorted = (int32_t*)take((size_t)n * 16);
+  A.cell_start = (int32_t*)take(((size_t)nv * d.ncell + 1) * 4);
+  A.tracks = (emu_track*)take(tcap * sizeof(emu_track));
+  A.fits = (emu_fit*)take(tcap * sizeof(emu_fit));
+  A.track_off = (int32_t*)take(((size_t)nv + 1) * 4);
+  A.members = (int32_t*)take((size_t)n * 4);
+  A.counts = (int64_t*)take(8 * 8);
+  A.status = (int64_t*)take(8);
+  size_t b = emu_bin_ws_bytes(d, n, nv), f = emu_find_ws_recommended_bytes(d, n, nv, cand_per_grain(p));
+  A.ws_bytes = b > f ? b : f;
+  A.ws = take(A.ws_bytes);
+  A.total = off + 256;
+}
+}  // namespace
+
+int emu_host_arena_bytes(const emu_params* params, int64_t n_grains, int32_t n_views, size_t* arena_bytes) {
+  if (!params_ok(params) || !arena_bytes) return EMU_ERR_INVALID;
+  EmuDev d = make_dev(params);
+  if (!shape_ok(d, n_grains, n_views)) return EMU_ERR_INVALID;
+  HostArena A;
+  carve_host_arena(params, d, n_grains, n_views, nullptr, A);
+  *arena_bytes = A.total;
+  return EMU_OK;
+}
+
+int emu_track_views_host(const emu_params* params, const int32_t* h_grains, const int32_t* h_view_off,
+                         int64_t n_grains, int32_t n_views, emu_track* h_tracks, emu_fit* h_fits,
+                         int64_t tracks_capacity, int32_t* h_track_off, int32_t* h_members,
+                         int64_t members_capacity, int64_t* h_counts, void* d_arena, size_t arena_bytes,
+                         void* stream) {
+  if (!params_ok(params)) return EMU_ERR_INVALID;
+  EmuDev d = make_dev(params);
+  if (!shape_ok(d, n_grains, n_views)) return EMU_ERR_INVALID;
+  if (!h_view_off || !h_track_off || !h_counts || !d_arena || tracks_capacity < 0 || members_capacity < 0) return EMU_ERR_INVALID;
+  if (n_grains > 0 && !h_grains) return EMU_ERR_INVALID;
+  HostArena A;
+  carve_host_arena(params, d, n_grains, n_views, (char*)emu_align_ptr(d_arena), A);
+  if (arena_bytes < A.total) return EMU_ERR_CAPACITY;
+  cudaStream_t st = (cudaStream_t)stream;
+  if (n_grains > 0 && cudaMemcpyAsync(A.grains, h_grains, (size_t)n_grains * 16, cudaMemcpyHostToDevice, st) != cudaSuccess) return EMU_ERR_CUDA;
+  if (cudaMemcpyAsync(A.view_off, h_view_off, ((size_t)n_views + 1) * 4, cudaMemcpyHostToDevice, st) != cudaSuccess) return EMU_ERR_CUDA;
+  if (cudaMemsetAsync(A.status, 0, 8, st) != cudaSuccess) return EMU_ERR_CUDA;
+  int rc = emu_bin_launch(d, A.grains, A.view_off, n_grains, n_views, A.sorted, A.cell_start, A.status, A.ws, A.ws_bytes, st);
+  if (rc != EMU_OK) return rc;
+  rc = emu_find_launch(d, cand_per_grain(params), A.sorted, A.cell_start, A.view_off, n_grains, n_views, A.tracks,
+                       A.track_off, A.members, n_grains, A.counts, A.ws, A.ws_bytes, st);
+  if (rc != EMU_OK) return rc;
+  rc = emu_fit_launch(A.grains, A.tracks, A.track_off, A.members, n_views, A.fits, st);
+  if (rc != EMU_OK) return rc;
+  int64_t status = 0;
+  if (cudaMemcpyAsync(h_counts, A.counts, 64, cudaMemcpyDeviceToHost, st) != cudaSuccess) return EMU_ERR_CUDA;
+  if (cudaMemcpyAsync(&status, A.status, 8, cudaMemcpyDeviceToHost, st) != cudaSuccess) return EMU_ERR_CUDA;
+  if (cudaMemcpyAsync(h_track_off, A.track_off, ((size_t)n_views + 1) * 4, cudaMemcpyDeviceToHost, st) != cudaSuccess) return EMU_ERR_CUDA;
+  if (cudaStreamSynchronize(st) != cudaSuccess) return EMU_ERR_CUDA;
+  h_counts[EMU_CNT_STATUS] |= status;
+  const int64_t nt = h_counts[EMU_CNT_TRACKS], nm = h_counts[EMU_CNT_MEMBERS];
+  if (h_counts[EMU_CNT_STATUS] != 0) return EMU_OK;            // device-side condition: outputs unspecified
+  if (nt > tracks_capacity || nm > members_capacity) return EMU_ERR_CAPACITY;
+  if (nt > 0 && (!h_tracks || !h_fits)) return EMU_ERR_INVALID;
+  if (nm > 0 && !h_members) return EMU_ERR_INVALID;
+  if (nt > 0) {
+    if (cudaMemcpyAsync(h_tracks, A.tracks, (size_t)nt * sizeof(emu_track), cudaMemcpyDeviceToHost, st) != cudaSuccess) return EMU_ERR_CUDA;
+    if (cudaMemcpyAsync(h_fits, A.fits, (size_t)nt * sizeof(emu_fit), cudaMemcpyDeviceToHost, st) != cudaSuccess) return EMU_ERR_CUDA;
+  }
+  if (nm > 0 && cudaMemcpyAsync(h_members, A.members, (size_t)nm * 4, cudaMemcpyDeviceToHost, st) != cudaSuccess) return EMU_ERR_CUDA;
+  if (cudaStreamSynchronize(st) != cudaSuccess) return EMU_ERR_CUDA;
+  return EMU_OK;
 }
 
 int emu_fit_tracks(const emu_params* params, const int32_t* d_grains, const emu_track* d_tracks,

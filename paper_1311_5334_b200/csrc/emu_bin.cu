@@ -109,10 +109,10 @@ int emu_bin_launch(const EmuDev& P, const int32_t* d_grains, const int32_t* d_vi
   if (cudaMemsetAsync(count, 0, (size_t)n_views * P.ncell * sizeof(int), st) != cudaSuccess) return EMU_ERR_CUDA;
   int blocks = (int)emu_min64((n_grains + kBinThreads - 1) / kBinThreads, 148 * 16);
   if (blocks < 1) blocks = 1;
-  k_bin_count<<<blocks, kBinThreads, 0, st>>>(P, (const int4*)d_grains, d_view_off, n_views, n, count,
-                                              (unsigned long long*)d_status);
-  k_bin_scan<<<(int)emu_min64(n_views > 0 ? n_views : 1, 148 * 2), 1024, 0, st>>>(P, d_view_off, n_views, n, count, d_cell_start);
-  k_bin_scatter<<<blocks, kBinThreads, 0, st>>>(P, (const int4*)d_grains, d_view_off, n_views, n, count, d_cell_start, tmp);
-  k_bin_place<<<blocks, kBinThreads, 0, st>>>(P, tmp, d_view_off, n_views, n, d_cell_start, (int4*)d_sorted);
+  EMU_LAUNCH(EMU_STAGE_BIN_COUNT, st, k_bin_count<<<blocks, kBinThreads, 0, st>>>(P, (const int4*)d_grains, d_view_off, n_views, n, count,
+                                              (unsigned long long*)d_status));
+  EMU_LAUNCH(EMU_STAGE_BIN_SCAN, st, k_bin_scan<<<(int)emu_min64(n_views > 0 ? n_views : 1, 148 * 2), 1024, 0, st>>>(P, d_view_off, n_views, n, count, d_cell_start));
+  EMU_LAUNCH(EMU_STAGE_BIN_SCATTER, st, k_bin_scatter<<<blocks, kBinThreads, 0, st>>>(P, (const int4*)d_grains, d_view_off, n_views, n, count, d_cell_start, tmp));
+  EMU_LAUNCH(EMU_STAGE_BIN_PLACE, st, k_bin_place<<<blocks, kBinThreads, 0, st>>>(P, tmp, d_view_off, n_views, n, d_cell_start, (int4*)d_sorted));
   return cudaGetLastError() == cudaSuccess ? EMU_OK : EMU_ERR_CUDA;
 }

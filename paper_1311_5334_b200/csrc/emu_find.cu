@@ -572,31 +572,31 @@ int emu_find_launch(const EmuDev& P, int cand_per_grain, const int32_t* d_sorted
   if (cudaMemsetAsync(W.keyA, 0, (size_t)n_grains * sizeof(unsigned long long), st) != cudaSuccess) return EMU_ERR_CUDA;
   if (cudaMemsetAsync(W.keyB, 0, (size_t)n_grains * sizeof(unsigned long long), st) != cudaSuccess) return EMU_ERR_CUDA;
   if (cudaMemsetAsync(W.owner, 0xff, (size_t)n_grains * sizeof(unsigned), st) != cudaSuccess) return EMU_ERR_CUDA;
-  k_bbox_init<<<grid_for(n_views, 256, 1 << 20), 256, 0, st>>>(W.bbox, n_views);
-  k_bbox<<<grid_for(n, 256, kSM * 8), 256, 0, st>>>(sorted, d_view_off, n_views, n, W.bbox);
+  EMU_LAUNCH(EMU_STAGE_PREP, st, k_bbox_init<<<grid_for(n_views, 256, 1 << 20), 256, 0, st>>>(W.bbox, n_views));
+  EMU_LAUNCH(EMU_STAGE_PREP, st, k_bbox<<<grid_for(n, 256, kSM * 8), 256, 0, st>>>(sorted, d_view_off, n_views, n, W.bbox));
 
   for (int v0 = 0; v0 < n_views; v0 += W.views_per_chunk) {
     const int v1 = (int)emu_min64(n_views, (int64_t)v0 + W.views_per_chunk);
     const int nv = v1 - v0;
     if (cudaMemsetAsync(W.ctl, 0, sizeof(FindCtl), st) != cudaSuccess) return EMU_ERR_CUDA;
     if (cudaMemsetAsync(W.view_ntracks, 0, (size_t)nv * sizeof(int), st) != cudaSuccess) return EMU_ERR_CUDA;
-    k_vote<false><<<kSM * 16, kVoteThreads, 0, st>>>(P, sorted, d_cell_start, d_view_off, W.bbox, v0, v1, W.cands,
-                                                     (unsigned)W.cand_cap, W.ctl, nullptr, 0, counts);
-    k_vote_finish<<<1, 1, 0, st>>>(W.ctl, (unsigned)W.cand_cap, counts);
-    k_reset_cand_arrays<<<kSM * 8, 256, 0, st>>>(W.ctl, W.wins, W.cand_track);
-    k_assoc<0><<<kSM * 16, kVoteThreads, 0, st>>>(P, sorted, d_cell_start, W.bbox, v0, W.cands, W.ctl, W.keyA, W.keyB, W.owner);
-    k_tie_detect<<<kSM * 4, 256, 0, st>>>(d_view_off, v0, v1, W.keyA, W.keyB, W.ctl);
-    k_assoc<1><<<kSM * 16, kVoteThreads, 0, st>>>(P, sorted, d_cell_start, W.bbox, v0, W.cands, W.ctl, W.keyA, W.keyB, W.owner);
-    k_wins<<<kSM * 4, 256, 0, st>>>(d_view_off, v0, v1, W.ctl, W.keyA, W.owner, W.wins);
-    k_select<<<kSM * 8, 256, 0, st>>>(P, W.cands, W.ctl, W.wins, W.view_ntracks, W.view_tracks, counts);
-    k_track_scan<<<1, 1024, 0, st>>>(P, v0, v1, W.view_ntracks, d_track_off);
-    k_track_emit<<<grid_for(nv, 1, kSM * 8), 256, 0, st>>>(P, sorted, v0, v1, W.cands, W.wins, W.view_ntracks,
-                                                          W.view_tracks, d_track_off, d_tracks, W.cand_track);
+    EMU_LAUNCH(EMU_STAGE_VOTE, st, k_vote<false><<<kSM * 16, kVoteThreads, 0, st>>>(P, sorted, d_cell_start, d_view_off, W.bbox, v0, v1, W.cands,
+                                                     (unsigned)W.cand_cap, W.ctl, nullptr, 0, counts));
+    EMU_LAUNCH(EMU_STAGE_PREP, st, k_vote_finish<<<1, 1, 0, st>>>(W.ctl, (unsigned)W.cand_cap, counts));
+    EMU_LAUNCH(EMU_STAGE_PREP, st, k_reset_cand_arrays<<<kSM * 8, 256, 0, st>>>(W.ctl, W.wins, W.cand_track));
+    EMU_LAUNCH(EMU_STAGE_ASSOC, st, k_assoc<0><<<kSM * 16, kVoteThreads, 0, st>>>(P, sorted, d_cell_start, W.bbox, v0, W.cands, W.ctl, W.keyA, W.keyB, W.owner));
+    EMU_LAUNCH(EMU_STAGE_ASSOC, st, k_tie_detect<<<kSM * 4, 256, 0, st>>>(d_view_off, v0, v1, W.keyA, W.keyB, W.ctl));
+    EMU_LAUNCH(EMU_STAGE_ASSOC, st, k_assoc<1><<<kSM * 16, kVoteThreads, 0, st>>>(P, sorted, d_cell_start, W.bbox, v0, W.cands, W.ctl, W.keyA, W.keyB, W.owner));
+    EMU_LAUNCH(EMU_STAGE_SELECT, st, k_wins<<<kSM * 4, 256, 0, st>>>(d_view_off, v0, v1, W.ctl, W.keyA, W.owner, W.wins));
+    EMU_LAUNCH(EMU_STAGE_SELECT, st, k_select<<<kSM * 8, 256, 0, st>>>(P, W.cands, W.ctl, W.wins, W.view_ntracks, W.view_tracks, counts));
+    EMU_LAUNCH(EMU_STAGE_EMIT, st, k_track_scan<<<1, 1024, 0, st>>>(P, v0, v1, W.view_ntracks, d_track_off));
+    EMU_LAUNCH(EMU_STAGE_EMIT, st, k_track_emit<<<grid_for(nv, 1, kSM * 8), 256, 0, st>>>(P, sorted, v0, v1, W.cands, W.wins, W.view_ntracks,
+                                                          W.view_tracks, d_track_off, d_tracks, W.cand_track));
     // the per-track fill cursors reuse view_tracks (its contents are dead after k_track_emit)
-    k_member_scan<<<1, 1024, 0, st>>>(v0, v1, d_track_off, d_tracks, (int*)W.view_tracks, counts, members_capacity);
-    k_member_scatter<<<kSM * 4, 256, 0, st>>>(sorted, d_view_off, v0, v1, W.ctl, W.keyA, W.owner, W.cand_track,
-                                              d_track_off, d_tracks, (int*)W.view_tracks, d_members, members_capacity);
-    k_member_sort<<<kSM * 4, 256, 0, st>>>(v0, v1, d_track_off, d_tracks, d_members, members_capacity);
+    EMU_LAUNCH(EMU_STAGE_EMIT, st, k_member_scan<<<1, 1024, 0, st>>>(v0, v1, d_track_off, d_tracks, (int*)W.view_tracks, counts, members_capacity));
+    EMU_LAUNCH(EMU_STAGE_EMIT, st, k_member_scatter<<<kSM * 4, 256, 0, st>>>(sorted, d_view_off, v0, v1, W.ctl, W.keyA, W.owner, W.cand_track,
+                                              d_track_off, d_tracks, (int*)W.view_tracks, d_members, members_capacity));
+    EMU_LAUNCH(EMU_STAGE_EMIT, st, k_member_sort<<<kSM * 4, 256, 0, st>>>(v0, v1, d_track_off, d_tracks, d_members, members_capacity));
   }
   return cudaGetLastError() == cudaSuccess ? EMU_OK : EMU_ERR_CUDA;
 }
@@ -608,10 +608,10 @@ int emu_count_seeds_launch(const EmuDev& P, const int32_t* d_sorted, const int32
   EmuBox* bbox = (EmuBox*)emu_align_ptr(d_ws);
   const int n = (int)n_grains;
   if (cudaMemsetAsync(d_counts, 0, 8 * sizeof(int64_t), st) != cudaSuccess) return EMU_ERR_CUDA;
-  k_bbox_init<<<grid_for(n_views, 256, 1 << 20), 256, 0, st>>>(bbox, n_views);
-  k_bbox<<<grid_for(n, 256, 148 * 8), 256, 0, st>>>((const int4*)d_sorted, d_view_off, n_views, n, bbox);
-  k_vote<true><<<148 * 16, kVoteThreads, 0, st>>>(P, (const int4*)d_sorted, d_cell_start, d_view_off, bbox, 0, n_views,
+  EMU_LAUNCH(EMU_STAGE_PREP, st, k_bbox_init<<<grid_for(n_views, 256, 1 << 20), 256, 0, st>>>(bbox, n_views));
+  EMU_LAUNCH(EMU_STAGE_PREP, st, k_bbox<<<grid_for(n, 256, 148 * 8), 256, 0, st>>>((const int4*)d_sorted, d_view_off, n_views, n, bbox));
+  EMU_LAUNCH(EMU_STAGE_VOTE, st, k_vote<true><<<148 * 16, kVoteThreads, 0, st>>>(P, (const int4*)d_sorted, d_cell_start, d_view_off, bbox, 0, n_views,
                                                   nullptr, 0, nullptr, (int4*)d_seed_dump, dump_capacity,
-                                                  (unsigned long long*)d_counts);
+                                                  (unsigned long long*)d_counts));
   return cudaGetLastError() == cudaSuccess ? EMU_OK : EMU_ERR_CUDA;
 }

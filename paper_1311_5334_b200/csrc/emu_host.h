@@ -11,6 +11,22 @@ static inline void* emu_align_ptr(void* p) { return (void*)(((uintptr_t)p + 255)
 static inline int64_t emu_min64(int64_t a, int64_t b) { return a < b ? a : b; }
 static inline int64_t emu_max64(int64_t a, int64_t b) { return a > b ? a : b; }
 
+// ---- optional per-stage timing (emu_profile_* of include/emu.h) -------------------------------
+// While a profile is active on the calling host thread, every kernel launch of the library is
+// bracketed by a pair of CUDA events on the launch stream and counted.  Without one, EMU_LAUNCH
+// is just the launch.
+struct emu_profile;
+emu_profile* emu_prof_current();
+void emu_prof_before(emu_profile* p, int stage, cudaStream_t st);
+void emu_prof_after(emu_profile* p, int stage, cudaStream_t st);
+#define EMU_LAUNCH(stage, st, ...)                          \
+  do {                                                      \
+    emu_profile* prof__ = emu_prof_current();               \
+    if (prof__) emu_prof_before(prof__, (stage), (st));     \
+    __VA_ARGS__;                                            \
+    if (prof__) emu_prof_after(prof__, (stage), (st));      \
+  } while (0)
+
 // emu_bin.cu
 size_t emu_bin_ws_bytes(const EmuDev& P, int64_t n_grains, int32_t n_views);
 int emu_bin_launch(const EmuDev& P, const int32_t* d_grains, const int32_t* d_view_off, int64_t n_grains,
