@@ -184,7 +184,11 @@ def main():
     ap.add_argument("--reference-warmup", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--cell-um", type=float, nargs=3, default=None, help="override the cell size of the 3D hash (um)")
     args = ap.parse_args()
+    if args.cell_um is not None:
+        global CELL_UM
+        CELL_UM = tuple(float(x) for x in args.cell_um)
     if args.impl == "reference":
         run_reference(args)
         return

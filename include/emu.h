@@ -45,8 +45,9 @@ typedef struct emu_params {
   int32_t tube_ext_q;          /* -1 = count along the whole line (reading Q4).  >= 0: EMU_ERR_INVALID     */
   int32_t min_grains;          /* threshold, >= 2: n >= min_grains (reading Q6; "e.g. 5")             */
   int32_t max_tracks_per_view; /* capacity of the track list per view, 1..65536                            */
-  int32_t reserved[4];         /* [0] = expected candidates per grain used to size internal chunks         */
-                               /* (0 = default 48); the rest must be 0                                     */
+  int32_t reserved[4];         /* sizing hints for the internal chunks of emu_find_tracks:                 */
+                               /* [0] = expected candidates per grain (0 = default 48),                    */
+                               /* [1] = expected seeds per grain (0 = default 192); [2], [3] must be 0     */
 } emu_params;
 
 typedef struct emu_track {     /* 32 B */
@@ -74,12 +75,13 @@ typedef struct emu_fit {       /* 48 B */
 #define EMU_CNT_MEMBERS 4
 #define EMU_CNT_STATUS 5       /* 0 = fine, else OR of the EMU_ST_* bits                                   */
 #define EMU_CNT_PAIR_TESTS 6   /* pair-distance tests executed (implementation figure)                     */
-#define EMU_CNT_NEED 7         /* largest candidate count one internal chunk needed                        */
+#define EMU_CNT_NEED 7         /* largest seed count one internal chunk needed                             */
 #define EMU_ST_CAND_OVERFLOW 1    /* candidate workspace too small: give more workspace / raise reserved[0] */
 #define EMU_ST_TRACK_OVERFLOW 2   /* a view has more than max_tracks_per_view tracks                       */
 #define EMU_ST_MEMBER_OVERFLOW 4  /* members_capacity too small                                            */
 #define EMU_ST_RANGE 8            /* a count does not fit its field (n_tube >= 8192)                       */
 #define EMU_ST_COORD 16           /* emu_bin_grains saw |coordinate| >= 2^17                               */
+#define EMU_ST_SEED_OVERFLOW 32   /* seed workspace too small: give more workspace / raise reserved[1]     */
 
 /* Host-only (no CUDA call).  Workspace each call needs for this batch shape; both outputs optional.
  * find_bytes is a recommendation (internal view chunks adapt to whatever >= the minimum is given). */
@@ -118,7 +120,8 @@ int emu_find_tracks(const emu_params* params, const int32_t* d_sorted, const int
 /* A2 + A3 only, for per-seed parity checks: writes (view, row_a, row_b, n_tube), row_a < row_b, for
  * every seed, in no particular order, to d_seed_dump int32[dump_capacity][4].  d_counts[EMU_CNT_SEEDS]
  * receives the number of seeds (which may exceed dump_capacity; the excess is not written).
- * d_ws: scratch of at least 32*n_views + 512 bytes. */
+ * d_ws: scratch of the find_bytes emu_workspace_bytes reports; the batch must fit ONE internal chunk
+ * (a test aid for a few views), else EMU_ERR_CAPACITY. */
 int emu_count_seeds(const emu_params* params, const int32_t* d_sorted, const int32_t* d_cell_start,
                     const int32_t* d_view_off, int64_t n_grains, int32_t n_views,
                     int32_t* d_seed_dump, int64_t dump_capacity, int64_t* d_counts,
@@ -169,6 +172,8 @@ int emu_track_views_host(const emu_params* params, const int32_t* h_grains, cons
 #define EMU_STAGE_SELECT 7       /* A5: wins per candidate, threshold again                         */
 #define EMU_STAGE_EMIT 8         /* A7: ordered track list and member lists                         */
 #define EMU_STAGE_FIT 9          /* A6                                                              */
+#define EMU_STAGE_SEEDS 10       /* A2: seed pairs (count, offsets, fill)                           */
+#define EMU_STAGE_CANDS 11       /* A4: threshold -> candidate list                                 */
 #define EMU_STAGE_COUNT 16
 typedef struct emu_profile emu_profile;
 emu_profile* emu_profile_create(void);              /* NULL on failure                              */

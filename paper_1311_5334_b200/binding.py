@@ -16,7 +16,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libemu4pi.so")
 
 EMU_CNT = dict(seeds=0, tests=1, candidates=2, tracks=3, members=4, status=5, pair_tests=6, need=7)
-EMU_ST = dict(cand_overflow=1, track_overflow=2, member_overflow=4, range=8, coord=16)
+EMU_ST = dict(cand_overflow=1, track_overflow=2, member_overflow=4, range=8, coord=16, seed_overflow=32)
 _ERR = {-1: "EMU_ERR_INVALID", -2: "EMU_ERR_CAPACITY", -3: "EMU_ERR_CUDA"}
 
 TRACK_DTYPE = np.dtype([("view", "<i4"), ("seed_a", "<i4"), ("seed_b", "<i4"), ("n_tube", "<i4"),
@@ -39,7 +39,8 @@ class emu_params(C.Structure):
 _SYMBOLS = ["emu_workspace_bytes", "emu_grid_cells", "emu_bin_grains", "emu_find_tracks", "emu_count_seeds",
             "emu_fit_tracks", "emu_host_arena_bytes", "emu_track_views_host", "emu_profile_create", "emu_profile_destroy", "emu_profile_begin", "emu_profile_end",
             "emu_profile_read"]
-EMU_STAGE = dict(bin_count=0, bin_scan=1, bin_scatter=2, bin_place=3, prep=4, vote=5, assoc=6, select=7, emit=8, fit=9)
+EMU_STAGE = dict(bin_count=0, bin_scan=1, bin_scatter=2, bin_place=3, prep=4, vote=5, assoc=6, select=7, emit=8, fit=9,
+                 seeds=10, cands=11)
 EMU_STAGE_COUNT = 16
 _lib = None
 
@@ -95,7 +96,7 @@ def exported_symbols() -> list:
 
 
 def make_params(view_size_q, cell_size_q, sep_min_q, sep_max_q, tube_r2_q, min_grains,
-                max_tracks_per_view=4096, tube_ext_q=-1, cand_per_grain=0) -> emu_params:
+                max_tracks_per_view=4096, tube_ext_q=-1, cand_per_grain=0, seeds_per_grain=0) -> emu_params:
     p = emu_params()
     p.struct_size = C.sizeof(emu_params)
     p.view_size_q[:] = [int(x) for x in view_size_q]
@@ -103,6 +104,7 @@ def make_params(view_size_q, cell_size_q, sep_min_q, sep_max_q, tube_r2_q, min_g
     p.sep_min_q, p.sep_max_q, p.tube_r2_q = int(sep_min_q), int(sep_max_q), int(tube_r2_q)
     p.tube_ext_q, p.min_grains, p.max_tracks_per_view = int(tube_ext_q), int(min_grains), int(max_tracks_per_view)
     p.reserved[0] = int(cand_per_grain)
+    p.reserved[1] = int(seeds_per_grain)
     return p
 
 

@@ -19,7 +19,7 @@ bool params_ok(const emu_params* p) {
   if (p->tube_ext_q != -1) return false;            // bounded tube: DESIGN.md "next" row, not built
   if (p->min_grains < 2 || p->min_grains > 8191) return false;
   if (p->max_tracks_per_view < 1 || p->max_tracks_per_view > 65536) return false;
-  if (p->reserved[0] < 0 || p->reserved[1] || p->reserved[2] || p->reserved[3]) return false;
+  if (p->reserved[0] < 0 || p->reserved[1] < 0 || p->reserved[2] || p->reserved[3]) return false;
   return true;
 }
 
@@ -52,6 +52,7 @@ bool shape_ok(const EmuDev& d, int64_t n_grains, int32_t n_views) {
 
 bool aligned16(const void* p) { return ((uintptr_t)p & 15) == 0; }
 int cand_per_grain(const emu_params* p) { return p->reserved[0] > 0 ? p->reserved[0] : 48; }
+int seeds_per_grain(const emu_params* p) { return p->reserved[1] > 0 ? p->reserved[1] : 192; }
 
 }  // namespace
 
@@ -114,7 +115,7 @@ int emu_workspace_bytes(const emu_params* params, int64_t n_grains, int32_t n_vi
   EmuDev d = make_dev(params);
   if (!shape_ok(d, n_grains, n_views)) return EMU_ERR_INVALID;
   if (bin_bytes) *bin_bytes = emu_bin_ws_bytes(d, n_grains, n_views);
-  if (find_bytes) *find_bytes = emu_find_ws_recommended_bytes(d, n_grains, n_views, cand_per_grain(params));
+  if (find_bytes) *find_bytes = emu_find_ws_recommended_bytes(d, n_grains, n_views, seeds_per_grain(params), cand_per_grain(params));
   return EMU_OK;
 }
 
@@ -153,7 +154,7 @@ int emu_find_tracks(const emu_params* params, const int32_t* d_sorted, const int
   if (!d_view_off || !d_cell_start || !d_track_off || !d_counts || !d_ws || !d_tracks || !d_members) return EMU_ERR_INVALID;
   if (n_grains > 0 && !d_sorted) return EMU_ERR_INVALID;
   if (!aligned16(d_sorted) || !aligned16(d_tracks) || members_capacity < 0) return EMU_ERR_INVALID;
-  return emu_find_launch(d, cand_per_grain(params), d_sorted, d_cell_start, d_view_off, n_grains, n_views, d_tracks,
+  return emu_find_launch(d, seeds_per_grain(params), cand_per_grain(params), d_sorted, d_cell_start, d_view_off, n_grains, n_views, d_tracks,
                          d_track_off, d_members, members_capacity, d_counts, d_ws, ws_bytes, (cudaStream_t)stream);
 }
 
@@ -166,7 +167,7 @@ int emu_count_seeds(const emu_params* params, const int32_t* d_sorted, const int
   if (!d_view_off || !d_cell_start || !d_counts || !d_ws || dump_capacity < 0) return EMU_ERR_INVALID;
   if (dump_capacity > 0 && !d_seed_dump) return EMU_ERR_INVALID;
   if (!aligned16(d_sorted) || !aligned16(d_seed_dump)) return EMU_ERR_INVALID;
-  return emu_count_seeds_launch(d, d_sorted, d_cell_start, d_view_off, n_grains, n_views, d_seed_dump, dump_capacity,
+  return emu_count_seeds_launch(d, seeds_per_grain(params), cand_per_grain(params), d_sorted, d_cell_start, d_view_off, n_grains, n_views, d_seed_dump, dump_capacity,
                                 d_counts, d_ws, ws_bytes, (cudaStream_t)stream);
 }
 
@@ -191,7 +192,7 @@ void carve_host_arena(const emu_params* p, const EmuDev& d, int64_t n, int32_t n
   A.members = (int32_t*)take((size_t)n * 4);
   A.counts = (int64_t*)take(8 * 8);
   A.status = (int64_t*)take(8);
-  size_t b = emu_bin_ws_bytes(d, n, nv), f = emu_find_ws_recommended_bytes(d, n, nv, cand_per_grain(p));
+  size_t b = emu_bin_ws_bytes(d, n, nv), f = emu_find_ws_recommended_bytes(d, n, nv, seeds_per_grain(p), cand_per_grain(p));
   A.ws_bytes = b > f ? b : f;
   A.ws = take(A.ws_bytes);
   A.total = off + 256;
@@ -227,7 +228,7 @@ int emu_track_views_host(const emu_params* params, const int32_t* h_grains, cons
   if (cudaMemsetAsync(A.status, 0, 8, st) != cudaSuccess) return EMU_ERR_CUDA;
   int rc = emu_bin_launch(d, A.grains, A.view_off, n_grains, n_views, A.sorted, A.cell_start, A.status, A.ws, A.ws_bytes, st);
   if (rc != EMU_OK) return rc;
-  rc = emu_find_launch(d, cand_per_grain(params), A.sorted, A.cell_start, A.view_off, n_grains, n_views, A.tracks,
+  rc = emu_find_launch(d, seeds_per_grain(params), cand_per_grain(params), A.sorted, A.cell_start, A.view_off, n_grains, n_views, A.tracks,
                        A.track_off, A.members, n_grains, A.counts, A.ws, A.ws_bytes, st);
   if (rc != EMU_OK) return rc;
   rc = emu_fit_launch(A.grains, A.tracks, A.track_off, A.members, n_views, A.fits, st);

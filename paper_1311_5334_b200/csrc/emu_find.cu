@@ -1,26 +1,43 @@
 // emu_find.cu - A2..A5 + A7: seeds, tube vote, threshold, exclusive association, threshold, order.
 // (P:72 and Fig. 4; readings Q1-Q8, Q15 in DESIGN.md section 3.)
 //
-// Views are processed in chunks sized by the candidate workspace.  Per chunk:
-//   k_vote        every seed of the chunk: walk its tube, count; n_tube >= min -> candidate list
-//   k_assoc_max   every candidate: walk again, atomicMax a packed priority into each member grain
-//   k_tie_detect  does any grain see two different top candidates with equal (n_tube, D2)?
-//   k_assoc_tie   (only then) every candidate: walk, settle the ties by (kmin, kmax) with a CAS-min
-//   k_wins        every grain: +1 for its owner
-//   k_select      every candidate: wins >= min -> per-view track list
-//   k_track_scan / k_track_emit / k_member_scan / k_member_scatter / k_member_sort: ordered output
+// Views are processed in chunks sized by the workspace.  Per chunk:
+//   k_seed_pairs<0>   every grain A: number of seeds {A,B}, B behind A in cell order          (A2)
+//   k_view_scan, k_chunk_offsets   per-grain / per-view seed offsets (deterministic seed layout)
+//   k_seed_pairs<1>   the seeds themselves: packed geometry (A, d) + the two sorted positions
+//   k_plan            cut every view into BRICKS (a tile of cell columns x a run of z layers) that fit
+//                     shared memory
+//   k_brick<VOTE>     persistent blocks: stage one brick's grains + cell table in shared memory, stream
+//                     all seeds of the view past it; every lane walks its own seed's tube through the
+//                     brick (uniform-grid ray traversal) and counts with the exact integer test   (A3)
+//   k_cands<0/1>      n_tube >= min_grains -> candidate list grouped by view                     (A4)
+//   k_brick<ASSOC>    the candidates again: atomicMax of a packed priority into each member grain (A5)
+//   k_tie_detect, k_assoc_generic<1>   exact settlement of priority ties by (kmin, kmax)
+//   k_wins, k_select  members won per candidate, threshold again
+//   k_track_scan / k_track_emit / k_member_scan / k_member_scatter / k_member_sort: ordered output (A7)
+// If a view cannot be cut into bricks (pathological density) the chunk falls back to the generic
+// kernels k_vote_generic / k_assoc_generic<0> that walk the cells in global memory.
 // Everything is a max / min / sum over a total order, so the result does not depend on the order in
 // which threads run (reading Q7: "one-shot, order-free").
+#include <math.h>
+
 #include "emu_dev.cuh"
 #include "emu_host.h"
 
 namespace {
 
-constexpr int kVoteThreads = 128;
+constexpr int kVoteThreads = 128;                 // generic walkers and the pair kernels
 constexpr int kCiBits = 29;                       // candidate index inside a chunk
 constexpr unsigned kCiMask = (1u << kCiBits) - 1u;
 constexpr unsigned kNone = 0xffffffffu;
 constexpr int kMaxTube = 8191;                    // n_tube field of the packed priority: 13 bits
+
+constexpr int kBrickThreads = 512;                // one persistent block per SM
+constexpr int kCapG = 11776;                      // grains a brick may hold   (16 B each)
+constexpr int kCapC = 16384;                      // cells a brick may hold    (2 B each)
+constexpr int kGrab = 128;                        // seeds a warp takes from the block's stream at a time
+constexpr size_t kBrickSmem = (size_t)kCapG * 16 + (size_t)(kCapC + 2) * 2;
+constexpr int kTieBits = 1 << 16;                 // bitmap of tied priorities
 
 struct Cand {            // 16 B
   int a, b;              // sorted positions of the seed grains, a < b
@@ -28,10 +45,20 @@ struct Cand {            // 16 B
   int d2;
 };
 
-struct FindCtl {         // device scalars of one emu_find_tracks call
-  unsigned cand_count;   // candidates of the current chunk
-  unsigned tie;          // 1 if the current chunk has a priority tie on some grain
-  unsigned pad[2];
+struct Brick {           // 32 B: cells [cx0..cx1] x [cy0..cy1] x [cz0..cz1] of one view, n grains
+  int view, cx0, cx1, cy0, cy1, cz0, cz1, n;
+};
+
+struct Tiling { int tx, ty, w, h; };   // tiles per view in x and y, tile width / height in cells
+
+struct FindCtl {         // device scalars of one chunk
+  unsigned cand_count;   // candidates of the chunk
+  unsigned tie;          // 1 if some grain sees two top candidates with equal (n_tube, D2)
+  unsigned seed_count;   // seeds of the chunk
+  unsigned n_bricks;
+  unsigned generic;      // 1: the brick plan failed, the generic kernels do the chunk
+  unsigned skip;         // 1: capacity overflow, nothing more is done for the chunk
+  unsigned work[2];      // work-item counters of the two brick passes
 };
 
 __device__ __forceinline__ unsigned long long cand_k1(int n_tube, int d2) {
@@ -66,6 +93,21 @@ __device__ bool cand_better(const int4* __restrict__ sorted, const Cand& c, cons
   if (nc != ne) return nc > ne;
   if (c.d2 != e.d2) return c.d2 > e.d2;
   return cand_kless(sorted, c, e);
+}
+
+// Packed seed geometry, 16 B: the line A + t*d and (for candidates) its n_tube.
+//   x = n_tube << 19 | Ax (19 bits, signed)      y = Ay
+//   z = Az << 12 | dz (12 bits, signed)          w = dx (12 bits, signed) << 12 | dy (12 bits, signed)
+// |A| < 2^17 and |d| < 2^11 (D2 < sep_max^2 <= 2^22), so every field fits.
+__device__ __forceinline__ int4 geo_pack(int ax, int ay, int az, int dx, int dy, int dz) {
+  int4 g;
+  g.x = ax & 0x7ffff; g.y = ay; g.z = (az << 12) | (dz & 0xfff); g.w = ((dx & 0xfff) << 12) | (dy & 0xfff);
+  return g;
+}
+__device__ __forceinline__ int sbfe(int v, int pos, int len) {
+  int r;
+  asm("bfe.s32 %0, %1, %2, %3;" : "=r"(r) : "r"(v), "r"(pos), "r"(len));
+  return r;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -112,21 +154,561 @@ k_bbox(const int4* __restrict__ sorted, const int* __restrict__ view_off, int n_
 }
 
 // ---------------------------------------------------------------------------------------------
-// A2 + A3 + A4.  One warp per grain A: the lanes scan the cells around A for partners B behind A in
-// sorted order (each unordered pair once, reading Q2), queue the pairs inside the separation window
-// (reading Q1), and then every lane walks the tube of one queued seed.
+// A2.  One warp per grain A: the lanes scan the cells around A for partners B behind A in sorted
+// order (each unordered pair once, reading Q2) inside the separation window (reading Q1).
+//   kFill = 0: seed_off[a] = number of seeds of A
+//   kFill = 1: the seeds are written at view_seed_off[v - v0] + seed_off[a] + rank (seed_off now holds
+//              the exclusive prefix inside the view): a deterministic layout, grouped by A.
+template <int kFill>
+__global__ void __launch_bounds__(kVoteThreads)
+k_seed_pairs(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ cell_start,
+             const int* __restrict__ view_off, int v0, int v1, unsigned* __restrict__ seed_off,
+             const unsigned* __restrict__ view_seed_off, const FindCtl* __restrict__ ctl,
+             int4* __restrict__ geo, int2* __restrict__ ab, unsigned long long* __restrict__ counts) {
+  if (kFill && ctl->skip) return;
+  const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+  const int nwarps = gridDim.x * (kVoteThreads / 32);
+  const int g0 = __ldg(view_off + v0), g1 = __ldg(view_off + v1);
+  unsigned long long n_pairs = 0;
+  for (int a = g0 + blockIdx.x * (kVoteThreads / 32) + wib; a < g1; a += nwarps) {
+    const int v = emu_find_view(view_off, v0, v1, a);
+    const int4 A = __ldg(sorted + a);
+    const int vbase = v * P.ncell;
+    const int cxa = emu_cell_axis(A.x - P.sep_max, P.cs[0], P.inv_cs[0], P.n[0]);
+    const int cxb = emu_cell_axis(A.x + P.sep_max, P.cs[0], P.inv_cs[0], P.n[0]);
+    const int cya = emu_cell_axis(A.y - P.sep_max, P.cs[1], P.inv_cs[1], P.n[1]);
+    const int cyb = emu_cell_axis(A.y + P.sep_max, P.cs[1], P.inv_cs[1], P.n[1]);
+    const int czA = emu_cell_axis(A.z, P.cs[2], P.inv_cs[2], P.n[2]);   // partners behind A: cell >= cell(A)
+    const int czb = emu_cell_axis(A.z + P.sep_max, P.cs[2], P.inv_cs[2], P.n[2]);
+    unsigned n = 0;
+    unsigned base = 0;
+    if (kFill) base = view_seed_off[v - v0] + seed_off[a];
+    for (int cz = czA; cz <= czb; ++cz) {
+      for (int cy = cya; cy <= cyb; ++cy) {
+        const int rb = vbase + (cz * P.n[1] + cy) * P.n[0];
+        int s = __ldg(cell_start + rb + cxa);
+        const int e = __ldg(cell_start + rb + cxb + 1);
+        s = max(s, a + 1);
+        for (int j0 = s; j0 < e; j0 += 32) {
+          const int j = j0 + lane;
+          bool ok = false;
+          int dx = 0, dy = 0, dz = 0;
+          if (j < e) {
+            int4 B = __ldg(sorted + j);
+            dx = B.x - A.x; dy = B.y - A.y; dz = B.z - A.z;
+            // |d| can exceed 2^15 for far out-of-box grains: compare in 64 bits
+            long long d2 = (long long)dx * dx + (long long)dy * dy + (long long)dz * dz;
+            ok = (d2 >= P.sep_min2) && (d2 < P.sep_max2);
+            ++n_pairs;
+          }
+          const unsigned m = __ballot_sync(EMU_FULL, ok);
+          if (kFill && ok) {
+            const unsigned idx = base + n + __popc(m & ((1u << lane) - 1u));
+            geo[idx] = geo_pack(A.x, A.y, A.z, dx, dy, dz);
+            ab[idx] = make_int2(a, j);
+          }
+          n += __popc(m);
+        }
+      }
+    }
+    if (!kFill && lane == 0) seed_off[a] = n;
+  }
+  if (!kFill) {
+    for (int o = 16; o; o >>= 1) n_pairs += __shfl_xor_sync(EMU_FULL, n_pairs, o);
+    if (lane == 0) atomicAdd(counts + EMU_CNT_PAIR_TESTS, n_pairs);
+  }
+}
+
+// per-view exclusive scan (in place) of the per-grain seed counts; view_tot[v - v0] = seeds of the view
+__global__ void __launch_bounds__(1024)
+k_view_scan(const int* __restrict__ view_off, int v0, int v1, unsigned* __restrict__ seed_off,
+            unsigned* __restrict__ view_tot, unsigned long long* __restrict__ counts) {
+  __shared__ unsigned warp_sum[32];
+  __shared__ unsigned carry_s;
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  for (int v = v0 + blockIdx.x; v < v1; v += gridDim.x) {
+    const int g0 = __ldg(view_off + v), g1 = __ldg(view_off + v + 1);
+    if (threadIdx.x == 0) carry_s = 0;
+    __syncthreads();
+    for (int b = g0; b < g1; b += blockDim.x) {
+      const int g = b + threadIdx.x;
+      unsigned x = (g < g1) ? seed_off[g] : 0u;
+      unsigned incl = x;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) { unsigned y = __shfl_up_sync(EMU_FULL, incl, o); if (lane >= o) incl += y; }
+      if (lane == 31) warp_sum[wid] = incl;
+      __syncthreads();
+      if (wid == 0) {
+        unsigned w = warp_sum[lane], wi = w;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { unsigned y = __shfl_up_sync(EMU_FULL, wi, o); if (lane >= o) wi += y; }
+        warp_sum[lane] = wi - w;
+      }
+      __syncthreads();
+      const unsigned carry = carry_s;
+      const unsigned mine = carry + warp_sum[wid] + incl;
+      if (g < g1) {
+        if (mine < carry) atomicOr(counts + EMU_CNT_STATUS, (unsigned long long)EMU_ST_SEED_OVERFLOW);  // >= 2^32 seeds in a view
+        seed_off[g] = mine - x;
+      }
+      __syncthreads();
+      if (threadIdx.x == blockDim.x - 1) carry_s = mine;
+      __syncthreads();
+    }
+    if (threadIdx.x == 0) view_tot[v - v0] = carry_s;
+    __syncthreads();
+  }
+}
+
+// exclusive scan over the views of a chunk (one block): off[0..nv], total -> *total_out; capacity check
+__global__ void __launch_bounds__(1024)
+k_chunk_offsets(int nv, const unsigned* __restrict__ tot, unsigned* __restrict__ off, unsigned* __restrict__ total_out,
+                unsigned cap, unsigned status_bit, FindCtl* __restrict__ ctl, unsigned long long* __restrict__ counts,
+                int count_slot) {
+  __shared__ unsigned warp_sum[32];
+  __shared__ unsigned long long carry_s;
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  if (threadIdx.x == 0) carry_s = 0;
+  __syncthreads();
+  for (int b = 0; b < nv; b += blockDim.x) {
+    const int v = b + threadIdx.x;
+    unsigned x = (v < nv) ? tot[v] : 0u;
+    unsigned incl = x;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { unsigned y = __shfl_up_sync(EMU_FULL, incl, o); if (lane >= o) incl += y; }
+    if (lane == 31) warp_sum[wid] = incl;
+    __syncthreads();
+    if (wid == 0) {
+      unsigned w = warp_sum[lane], wi = w;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) { unsigned y = __shfl_up_sync(EMU_FULL, wi, o); if (lane >= o) wi += y; }
+      warp_sum[lane] = wi - w;
+    }
+    __syncthreads();
+    const unsigned long long carry = carry_s;
+    const unsigned long long mine = carry + warp_sum[wid] + incl;   // (a 1024-view tile of the scan stays below 2^32 when it fits)
+    if (v < nv) off[v] = (unsigned)min(mine - x, 0xffffffffull);
+    __syncthreads();
+    if (threadIdx.x == blockDim.x - 1) carry_s = mine;
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) {
+    const unsigned long long total = carry_s;
+    off[nv] = (unsigned)min(total, 0xffffffffull);
+    atomicAdd(counts + count_slot, total);
+    if (status_bit == (unsigned)EMU_ST_SEED_OVERFLOW) atomicMax(counts + EMU_CNT_NEED, total);
+    if (total > cap) {
+      atomicOr(counts + EMU_CNT_STATUS, (unsigned long long)status_bit);
+      ctl->skip = 1;
+      *total_out = 0;
+    } else {
+      *total_out = (unsigned)total;
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Brick plan: one warp per view.  Every tile (tx, ty) of cell columns is cut into runs of z layers
+// that hold at most kCapG grains and kCapC cells; empty bricks are dropped.
+__global__ void __launch_bounds__(128)
+k_plan(EmuDev P, Tiling T, const int* __restrict__ cell_start, int v0, int v1, Brick* __restrict__ bricks,
+       unsigned brick_cap, FindCtl* __restrict__ ctl) {
+  const int lane = threadIdx.x & 31;
+  const int v = v0 + blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  if (v >= v1 || ctl->skip) return;
+  const int nx = P.n[0], ny = P.n[1], nz = P.n[2];
+  const int vbase = v * P.ncell;
+  for (int t = 0; t < T.tx * T.ty; ++t) {
+    const int cx0 = (t % T.tx) * T.w, cy0 = (t / T.tx) * T.h;
+    const int cx1 = min(nx, cx0 + T.w) - 1, cy1 = min(ny, cy0 + T.h) - 1;
+    if (cx0 > cx1 || cy0 > cy1) continue;
+    const int layer_cells = (cx1 - cx0 + 1) * (cy1 - cy0 + 1);
+    if (layer_cells > kCapC) { if (lane == 0) ctl->generic = 1; return; }
+    int z_first = 0, acc = 0;
+    for (int cz = 0; cz <= nz; ++cz) {
+      int cnt = 0;
+      if (cz < nz) {
+        for (int cy = cy0 + lane; cy <= cy1; cy += 32) {
+          const int rb = vbase + (cz * ny + cy) * nx;
+          cnt += __ldg(cell_start + rb + cx1 + 1) - __ldg(cell_start + rb + cx0);
+        }
+        cnt = __reduce_add_sync(EMU_FULL, cnt);
+        if (cnt > kCapG) { if (lane == 0) ctl->generic = 1; return; }
+      }
+      const bool flush = (cz == nz) || (acc + cnt > kCapG) || ((cz - z_first + 1) * layer_cells > kCapC);
+      if (flush) {
+        if (acc > 0 && lane == 0) {
+          const unsigned slot = atomicAdd(&ctl->n_bricks, 1u);
+          if (slot < brick_cap) {
+            Brick b; b.view = v; b.cx0 = cx0; b.cx1 = cx1; b.cy0 = cy0; b.cy1 = cy1; b.cz0 = z_first; b.cz1 = cz - 1; b.n = acc;
+            bricks[slot] = b;
+          }
+        }
+        z_first = cz; acc = 0;
+      }
+      acc += cnt;
+    }
+  }
+}
+
+__global__ void k_plan_finish(FindCtl* ctl, unsigned brick_cap) {
+  if (ctl->n_bricks > brick_cap) ctl->generic = 1;
+  if (ctl->generic) ctl->n_bricks = 0;
+}
+
+// ---------------------------------------------------------------------------------------------
+// A3 / A5 on shared-memory bricks.
+//
+// A persistent block takes work items (brick, slice of the view's seed list).  It stages the brick
+// - the grains of its cells in (cz, cy, cx) order and a 16-bit local cell table - in shared memory
+// and streams the seeds of the slice past it.  Each LANE owns one seed at a time and is in one of
+// three states; the warp repeatedly executes the phase most of its lanes wait for (persistent-thread
+// ray traversal):
+//   SEED  fetch the next seed of the warp's range, unpack it, clip the line against the brick
+//   ROW   advance the traversal: next z layer of the brick, next row of cells (cy) in it, giving a run
+//         [j, e) of consecutive grains of the cells cx0..cx1 the tube can touch in that row
+//   TEST  one exact integer point-line test of grain j (emu_in_tube); VOTE counts, ASSOC takes part in
+//         the priority maximum of the grain
+// The traversal bounds are conservative float intervals (a grain in the tube is within R of its foot
+// on the line in every coordinate), widened by Rw = R + 2 q against rounding; only the integer test
+// decides, so the bounds only have to be a superset.  Boundary cells of the VIEW are open-ended
+// because out-of-box grains are clamped into them (reading Q13): they reach to the view's bounding box.
+enum { kVote = 0, kAssoc = 1 };
+enum { S_NEED = 0, S_ROW = 1, S_TEST = 2 };
+
+struct BrickShared {
+  int row_gs[kBrickThreads];
+  int row_off[kBrickThreads];
+  unsigned warp_sum[kBrickThreads / 32];
+  unsigned work;
+  unsigned next, end;
+  int carry;
+};
+
+template <int kMode>
+__global__ void __launch_bounds__(kBrickThreads, 1)
+k_brick(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ cell_start,
+        const EmuBox* __restrict__ bbox, int v0, const Brick* __restrict__ bricks, FindCtl* __restrict__ ctl,
+        int slices, const int4* __restrict__ geo, const unsigned* __restrict__ view_item_off,
+        unsigned* __restrict__ seed_cnt, unsigned long long* __restrict__ keyA,
+        unsigned long long* __restrict__ keyB, unsigned long long* __restrict__ counts) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  int4* sg = reinterpret_cast<int4*>(smem_raw);
+  unsigned short* lcs = reinterpret_cast<unsigned short*>(smem_raw + (size_t)kCapG * 16);
+  __shared__ BrickShared sh;
+
+  if (ctl->skip || ctl->generic) return;
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  const unsigned n_items = ctl->n_bricks * (unsigned)slices;
+  const float R = P.Rw;
+  unsigned long long n_tests = 0;
+  int cur_brick = -1;
+  Brick B;
+  B.view = 0; B.cx0 = B.cx1 = B.cy0 = B.cy1 = B.cz0 = B.cz1 = B.n = 0;
+  int W = 1, H = 1;
+  float blo[3] = {0.f, 0.f, 0.f}, bhi[3] = {0.f, 0.f, 0.f};   // brick extent widened by R
+  int elo[3] = {0, 0, 0}, ehi[3] = {0, 0, 0};                 // open-ended extent of the view's boundary cells
+
+  for (;;) {
+    __syncthreads();                                  // everyone is done with the previous item
+    if (tid == 0) sh.work = atomicAdd(&ctl->work[kMode], 1u);
+    __syncthreads();
+    const unsigned w = sh.work;
+    if (w >= n_items) break;
+    const int b = (int)(w / (unsigned)slices), sl = (int)(w % (unsigned)slices);
+
+    if (b != cur_brick) {
+      // ---- stage brick b ----
+      cur_brick = b;
+      B = bricks[b];
+      W = B.cx1 - B.cx0 + 1; H = B.cy1 - B.cy0 + 1;
+      const int rows = H * (B.cz1 - B.cz0 + 1);
+      const int vbase = B.view * P.ncell;
+      const EmuBox bb = bbox[B.view];
+#pragma unroll
+      for (int a = 0; a < 3; ++a) {
+        elo[a] = min(bb.lo[a], 0);
+        ehi[a] = max(bb.hi[a], P.n[a] * P.cs[a] - 1);
+      }
+      {
+        const int c0[3] = {B.cx0, B.cy0, B.cz0}, c1[3] = {B.cx1, B.cy1, B.cz1};
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+          const int lo = (c0[a] == 0) ? elo[a] : c0[a] * P.cs[a];
+          const int hi = (c1[a] == P.n[a] - 1) ? ehi[a] : (c1[a] + 1) * P.cs[a] - 1;
+          blo[a] = (float)lo - R; bhi[a] = (float)hi + R;
+        }
+      }
+      if (tid == 0) sh.carry = 0;
+      __syncthreads();
+      for (int r0 = 0; r0 < rows; r0 += kBrickThreads) {
+        const int r = r0 + tid;
+        int gs = 0, len = 0;
+        if (r < rows) {
+          const int cz = B.cz0 + r / H, cy = B.cy0 + r % H;
+          const int rb = vbase + (cz * P.n[1] + cy) * P.n[0];
+          gs = __ldg(cell_start + rb + B.cx0);
+          len = __ldg(cell_start + rb + B.cx1 + 1) - gs;
+        }
+        int incl = len;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(EMU_FULL, incl, o); if (lane >= o) incl += y; }
+        if (lane == 31) sh.warp_sum[wid] = (unsigned)incl;
+        __syncthreads();
+        if (wid == 0) {
+          unsigned x = (lane < kBrickThreads / 32) ? sh.warp_sum[lane] : 0u, xi = x;
+#pragma unroll
+          for (int o = 1; o < 32; o <<= 1) { unsigned y = __shfl_up_sync(EMU_FULL, xi, o); if (lane >= o) xi += y; }
+          if (lane < kBrickThreads / 32) sh.warp_sum[lane] = xi - x;
+        }
+        __syncthreads();
+        const int carry = sh.carry;
+        sh.row_gs[tid] = gs;
+        sh.row_off[tid] = carry + (int)sh.warp_sum[wid] + incl - len;
+        __syncthreads();
+        if (tid == kBrickThreads - 1) sh.carry = carry + (int)sh.warp_sum[wid] + incl;
+        const int nr = min(kBrickThreads, rows - r0);
+        for (int k = wid; k < nr; k += kBrickThreads / 32) {
+          const int rgs = sh.row_gs[k], roff = sh.row_off[k];
+          const int rr = r0 + k;
+          const int cz = B.cz0 + rr / H, cy = B.cy0 + rr % H;
+          const int rb = vbase + (cz * P.n[1] + cy) * P.n[0] + B.cx0;
+          for (int i = lane; i < W; i += 32) lcs[rr * W + i] = (unsigned short)(roff + (__ldg(cell_start + rb + i) - rgs));
+          const int rlen = __ldg(cell_start + rb + W) - rgs;
+          for (int i = lane; i < rlen; i += 32) {
+            int4 g = __ldg(sorted + rgs + i);
+            g.w = rgs + i;                               // the grain's sorted position (ASSOC needs it)
+            sg[roff + i] = g;
+          }
+        }
+        __syncthreads();
+      }
+      if (tid == 0) lcs[rows * W] = (unsigned short)sh.carry;
+    }
+    // ---- the slice of the view's items ----
+    {
+      const int vl = B.view - v0;
+      const unsigned lo = view_item_off[vl], hi = view_item_off[vl + 1];
+      const unsigned per = (hi - lo + (unsigned)slices - 1u) / (unsigned)slices;
+      const unsigned s0 = min(hi, lo + per * (unsigned)sl), s1 = min(hi, s0 + per);
+      if (tid == 0) { sh.next = s0; sh.end = s1; }
+    }
+    __syncthreads();
+    const unsigned s_end = sh.end;
+
+    // ---- per-lane traversal state ----
+    int st = S_NEED;
+    int ax = 0, ay = 0, az = 0, dx = 0, dy = 0, dz = 0;
+    long long r2D2 = 0;
+    float fax = 0.f, fay = 0.f, faz = 0.f, fdx = 0.f, fdy = 0.f, inv_dy = 0.f, inv_dz = 0.f;
+    float t0 = 0.f, t1 = 0.f, tl0 = 0.f, tl1 = 0.f;
+    int cz = 0, cz_hi = -1, cy = 1, cy_hi = 0, j = 0, e = 0;
+    unsigned sidx = 0;
+    int count = 0;
+    unsigned long long ka = 0, kb = 0;
+    unsigned wcur = 0, wend = 0;
+    bool exhausted = false;
+
+    unsigned item_tests = 0;
+    for (;;) {
+      unsigned mS = __ballot_sync(EMU_FULL, st == S_NEED);
+      const unsigned mR = __ballot_sync(EMU_FULL, st == S_ROW);
+      const unsigned mT = __ballot_sync(EMU_FULL, st == S_TEST);
+      if (exhausted) mS = 0;
+      if (!(mS | mR | mT)) break;
+      const int nS = __popc(mS), nR = __popc(mR), nT = __popc(mT);
+      // the phase most lanes wait for; it is repeated while at least 3/4 of them still want it
+      if (nT >= nR && nT >= nS) {
+        // ---------------- TEST ----------------
+        const int keep = (3 * nT + 3) >> 2;
+        do {
+          if (st == S_TEST) {
+            const int4 p = sg[j];
+            if (emu_in_tube(p.x, p.y, p.z, ax, ay, az, dx, dy, dz, r2D2)) {
+              if (kMode == kVote) ++count;
+              else { atomicMax(keyA + p.w, ka); atomicMax(keyB + p.w, kb); }
+            }
+            ++j; ++item_tests;
+            if (j >= e) st = S_ROW;
+          }
+        } while (__popc(__ballot_sync(EMU_FULL, st == S_TEST)) >= keep);
+      } else if (nR >= nS) {
+        // ---------------- ROW ----------------
+        const int keep = (3 * nR + 3) >> 2;
+        do {
+          if (st == S_ROW) {
+            if (cy > cy_hi) {                               // next z layer of the brick
+              ++cz;
+              if (cz > cz_hi) {                             // the seed is finished
+                if (kMode == kVote && count) atomicAdd(seed_cnt + sidx, (unsigned)count);
+                st = S_NEED;
+              } else {
+                tl0 = t0; tl1 = t1;
+                if (dz != 0) {
+                  const int lo = (cz == 0) ? elo[2] : cz * P.cs[2];
+                  const int hi = (cz == P.n[2] - 1) ? ehi[2] : (cz + 1) * P.cs[2] - 1;
+                  const float a = ((float)lo - R - faz) * inv_dz, bq = ((float)hi + R - faz) * inv_dz;
+                  tl0 = fmaxf(t0, fminf(a, bq)); tl1 = fminf(t1, fmaxf(a, bq));
+                }
+                if (tl0 <= tl1) {
+                  const float ya = fmaf(tl0, fdy, fay), yb = fmaf(tl1, fdy, fay);
+                  cy = max(B.cy0, emu_clampcell_f(fminf(ya, yb) - R, P.inv_cs[1], P.n[1]));
+                  cy_hi = min(B.cy1, emu_clampcell_f(fmaxf(ya, yb) + R, P.inv_cs[1], P.n[1]));
+                }                                           // else: cy > cy_hi stays, the next step moves on
+              }
+            }
+            if (st == S_ROW && cy <= cy_hi) {               // row cy of layer cz
+              float tr0 = tl0, tr1 = tl1;
+              if (dy != 0) {
+                const int lo = (cy == 0) ? elo[1] : cy * P.cs[1];
+                const int hi = (cy == P.n[1] - 1) ? ehi[1] : (cy + 1) * P.cs[1] - 1;
+                const float a = ((float)lo - R - fay) * inv_dy, bq = ((float)hi + R - fay) * inv_dy;
+                tr0 = fmaxf(tl0, fminf(a, bq)); tr1 = fminf(tl1, fmaxf(a, bq));
+              }
+              if (tr0 <= tr1) {
+                const float xa = fmaf(tr0, fdx, fax), xb = fmaf(tr1, fdx, fax);
+                const int cx0 = max(B.cx0, emu_clampcell_f(fminf(xa, xb) - R, P.inv_cs[0], P.n[0]));
+                const int cx1 = min(B.cx1, emu_clampcell_f(fmaxf(xa, xb) + R, P.inv_cs[0], P.n[0]));
+                if (cx0 <= cx1) {
+                  const int rl = ((cz - B.cz0) * H + (cy - B.cy0)) * W - B.cx0;
+                  j = lcs[rl + cx0]; e = lcs[rl + cx1 + 1];
+                  if (j < e) st = S_TEST;
+                }
+              }
+              ++cy;
+            }
+          }
+        } while (__popc(__ballot_sync(EMU_FULL, st == S_ROW)) >= keep);
+      } else {
+        // ---------------- SEED ----------------
+        const int keep = (3 * nS + 3) >> 2;
+        for (;;) {
+          if (wcur == wend) {
+            unsigned base = 0;
+            if (lane == 0) base = atomicAdd(&sh.next, (unsigned)kGrab);
+            base = __shfl_sync(EMU_FULL, base, 0);
+            if (base >= s_end) { exhausted = true; break; }
+            wcur = base; wend = min(base + (unsigned)kGrab, s_end);
+          }
+          const unsigned idx = wcur + (unsigned)__popc(mS & ((1u << lane) - 1u));
+          const bool take = (st == S_NEED) && (idx < wend);
+          wcur = min(wend, wcur + (unsigned)__popc(mS));
+          if (take) {
+            const int4 q = __ldg(geo + idx);
+            ax = sbfe(q.x, 0, 19); ay = q.y; az = q.z >> 12;
+            dz = sbfe(q.z, 0, 12); dx = sbfe(q.w, 12, 12); dy = sbfe(q.w, 0, 12);
+            const int d2 = dx * dx + dy * dy + dz * dz;
+            r2D2 = (long long)P.r2 * d2;
+            sidx = idx; count = 0;
+            if (kMode == kAssoc) {
+              const unsigned long long k1 = cand_k1((int)((unsigned)q.x >> 19), d2);
+              ka = (k1 << kCiBits) | (unsigned long long)(kCiMask - idx);
+              kb = (k1 << kCiBits) | (unsigned long long)idx;
+            }
+            fax = (float)ax; fay = (float)ay; faz = (float)az; fdx = (float)dx; fdy = (float)dy;
+            const float fdz = (float)dz;
+            const float inv_dx = dx ? 1.0f / fdx : 0.0f;
+            inv_dy = dy ? 1.0f / fdy : 0.0f;
+            inv_dz = dz ? 1.0f / fdz : 0.0f;
+            // clip the line against the brick's extent (already widened by R)
+            t0 = -1.0e9f; t1 = 1.0e9f;
+            bool hit = true;
+            if (dx != 0) { const float a = (blo[0] - fax) * inv_dx, bq = (bhi[0] - fax) * inv_dx; t0 = fmaxf(t0, fminf(a, bq)); t1 = fminf(t1, fmaxf(a, bq)); }
+            else hit = hit && (fax >= blo[0]) && (fax <= bhi[0]);
+            if (dy != 0) { const float a = (blo[1] - fay) * inv_dy, bq = (bhi[1] - fay) * inv_dy; t0 = fmaxf(t0, fminf(a, bq)); t1 = fminf(t1, fmaxf(a, bq)); }
+            else hit = hit && (fay >= blo[1]) && (fay <= bhi[1]);
+            if (dz != 0) { const float a = (blo[2] - faz) * inv_dz, bq = (bhi[2] - faz) * inv_dz; t0 = fmaxf(t0, fminf(a, bq)); t1 = fminf(t1, fmaxf(a, bq)); }
+            else hit = hit && (faz >= blo[2]) && (faz <= bhi[2]);
+            if (hit && t0 <= t1) {
+              const float za = fmaf(t0, fdz, faz), zb = fmaf(t1, fdz, faz);
+              cz = max(B.cz0, emu_clampcell_f(fminf(za, zb) - R, P.inv_cs[2], P.n[2])) - 1;
+              cz_hi = min(B.cz1, emu_clampcell_f(fmaxf(za, zb) + R, P.inv_cs[2], P.n[2]));
+              cy = 1; cy_hi = 0;                            // forces a layer step first
+              st = S_ROW;
+            }
+          }
+          mS = __ballot_sync(EMU_FULL, st == S_NEED);
+          if (__popc(mS) < keep) break;
+        }
+      }
+    }
+    n_tests += item_tests;
+  }
+
+  for (int o = 16; o; o >>= 1) n_tests += __shfl_xor_sync(EMU_FULL, n_tests, o);
+  if (lane == 0 && n_tests) atomicAdd(counts + EMU_CNT_TESTS, n_tests);
+}
+
+// ---------------------------------------------------------------------------------------------
+// A4: candidates = seeds with n_tube >= min_grains, grouped by view.  grid = (blocks, views of chunk).
+template <int kFill>
+__global__ void __launch_bounds__(256)
+k_cands(EmuDev P, int v0, const FindCtl* __restrict__ ctl, const unsigned* __restrict__ view_seed_off,
+        const unsigned* __restrict__ seed_cnt, const int4* __restrict__ geo, const int2* __restrict__ ab,
+        unsigned* __restrict__ view_cand_cnt, const unsigned* __restrict__ view_cand_off,
+        Cand* __restrict__ cands, int4* __restrict__ cand_geo, unsigned long long* __restrict__ counts) {
+  if (ctl->skip || ctl->generic) return;
+  const int vl = blockIdx.y, lane = threadIdx.x & 31;
+  const unsigned lo = view_seed_off[vl], hi = view_seed_off[vl + 1];
+  const unsigned span = gridDim.x * blockDim.x;
+  unsigned status = 0;
+  for (unsigned i0 = lo + blockIdx.x * blockDim.x + (threadIdx.x & ~31u); i0 < hi; i0 += span) {
+    const unsigned i = i0 + lane;
+    const unsigned n = (i < hi) ? seed_cnt[i] : 0u;
+    const bool is = n >= (unsigned)P.min_grains;
+    const unsigned m = __ballot_sync(EMU_FULL, is);
+    if (!m) continue;
+    unsigned base = 0;
+    if (lane == 0) base = atomicAdd(view_cand_cnt + vl, (unsigned)__popc(m));
+    if (!kFill) continue;
+    base = __shfl_sync(EMU_FULL, base, 0);
+    if (is) {
+      const unsigned ci = view_cand_off[vl] + base + (unsigned)__popc(m & ((1u << lane) - 1u));
+      int4 g = geo[i];
+      const int2 p = ab[i];
+      const int dz = sbfe(g.z, 0, 12), dx = sbfe(g.w, 12, 12), dy = sbfe(g.w, 0, 12);
+      if (n > (unsigned)kMaxTube) status |= EMU_ST_RANGE;
+      Cand c; c.a = p.x; c.b = p.y; c.n_tube_view = (int)min(n, 0xffffu) | (vl << 16); c.d2 = dx * dx + dy * dy + dz * dz;
+      cands[ci] = c;
+      g.x = (int)(((unsigned)g.x & 0x7ffffu) | (min(n, (unsigned)kMaxTube) << 19));
+      cand_geo[ci] = g;
+    }
+  }
+  if (kFill && __any_sync(EMU_FULL, status != 0) && lane == 0) atomicOr(counts + EMU_CNT_STATUS, (unsigned long long)EMU_ST_RANGE);
+}
+
+// seed dump for emu_count_seeds: (view, row_a, row_b, n_tube), rows ordered
+__global__ void __launch_bounds__(256)
+k_seed_dump(int v0, const FindCtl* __restrict__ ctl, const int4* __restrict__ sorted,
+            const unsigned* __restrict__ view_seed_off, const unsigned* __restrict__ seed_cnt,
+            const int2* __restrict__ ab, int4* __restrict__ dump, long long dump_cap) {
+  if (ctl->skip || ctl->generic) return;
+  const int vl = blockIdx.y;
+  const unsigned lo = view_seed_off[vl], hi = view_seed_off[vl + 1];
+  for (unsigned i = lo + blockIdx.x * blockDim.x + threadIdx.x; i < hi; i += gridDim.x * blockDim.x) {
+    if ((long long)i >= dump_cap) continue;
+    const int2 p = ab[i];
+    const int ra = sorted[p.x].w, rb = sorted[p.y].w;
+    dump[i] = make_int4(v0 + vl, min(ra, rb), max(ra, rb), (int)seed_cnt[i]);
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Generic fallback (global-memory walker): A2 + A3 + A4 in one kernel, one warp per grain A.
 template <bool kDump>
 __global__ void __launch_bounds__(kVoteThreads)
-k_vote(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ cell_start,
-       const int* __restrict__ view_off, const EmuBox* __restrict__ bbox, int v0, int v1,
-       Cand* __restrict__ cands, unsigned cand_cap, FindCtl* __restrict__ ctl,
-       int4* __restrict__ dump, long long dump_cap, unsigned long long* __restrict__ counts) {
+k_vote_generic(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ cell_start,
+               const int* __restrict__ view_off, const EmuBox* __restrict__ bbox, int v0, int v1,
+               Cand* __restrict__ cands, unsigned cand_cap, FindCtl* __restrict__ ctl,
+               int4* __restrict__ dump, long long dump_cap, unsigned long long* __restrict__ dump_cursor,
+               unsigned long long* __restrict__ counts) {
   __shared__ int queue_s[kVoteThreads / 32][64];
+  if (ctl->skip || !ctl->generic) return;
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
   int* queue = queue_s[wib];
   const int nwarps = gridDim.x * (kVoteThreads / 32);
   const int g0 = __ldg(view_off + v0), g1 = __ldg(view_off + v1);
-  unsigned long long n_tests = 0, n_pairs = 0, n_seeds = 0, n_cands = 0;
+  unsigned long long n_tests = 0, n_cands = 0;
   unsigned status = 0;
 
   for (int a = g0 + blockIdx.x * (kVoteThreads / 32) + wib; a < g1; a += nwarps) {
@@ -138,7 +720,7 @@ k_vote(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ cell_s
     const int cxb = emu_cell_axis(A.x + P.sep_max, P.cs[0], P.inv_cs[0], P.n[0]);
     const int cya = emu_cell_axis(A.y - P.sep_max, P.cs[1], P.inv_cs[1], P.n[1]);
     const int cyb = emu_cell_axis(A.y + P.sep_max, P.cs[1], P.inv_cs[1], P.n[1]);
-    const int czA = emu_cell_axis(A.z, P.cs[2], P.inv_cs[2], P.n[2]);   // partners behind A: cell >= cell(A)
+    const int czA = emu_cell_axis(A.z, P.cs[2], P.inv_cs[2], P.n[2]);
     const int czb = emu_cell_axis(A.z + P.sep_max, P.cs[2], P.inv_cs[2], P.n[2]);
     int qhead = 0, qn = 0;
 
@@ -154,10 +736,9 @@ k_vote(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ cell_s
         n_tests += emu_walk_tube(P, bb, sorted, cell_start, vbase, A.x, A.y, A.z, dx, dy, dz, r2D2,
                                  [&](int) { ++n_tube; });
       }
-      n_seeds += (b >= 0);
       if (kDump) {
         unsigned long long base = 0;
-        if (lane == 0) base = atomicAdd(counts + EMU_CNT_NEED, (unsigned long long)cnt);   // dump cursor
+        if (lane == 0) base = atomicAdd(dump_cursor, (unsigned long long)cnt);
         base = __shfl_sync(EMU_FULL, base, 0);
         if (b >= 0 && (long long)(base + lane) < dump_cap)
           dump[base + lane] = make_int4(v, min(A.w, B.w), max(A.w, B.w), n_tube);
@@ -192,10 +773,8 @@ k_vote(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ cell_s
           if (j < e) {
             int4 B = __ldg(sorted + j);
             int dx = B.x - A.x, dy = B.y - A.y, dz = B.z - A.z;
-            // |d| can exceed 2^15 for far out-of-box grains: compare in 64 bits
             long long d2 = (long long)dx * dx + (long long)dy * dy + (long long)dz * dz;
             ok = (d2 >= P.sep_min2) && (d2 < P.sep_max2);
-            ++n_pairs;
           }
           unsigned m = __ballot_sync(EMU_FULL, ok);
           if (ok) queue[(qhead + qn + __popc(m & ((1u << lane) - 1u))) & 63] = j;
@@ -207,52 +786,59 @@ k_vote(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ cell_s
     }
     if (qn) { process(qn); __syncwarp(); }
   }
-
-  // one set of atomics per warp
   for (int o = 16; o; o >>= 1) {
     n_tests += __shfl_xor_sync(EMU_FULL, n_tests, o);
-    n_pairs += __shfl_xor_sync(EMU_FULL, n_pairs, o);
-    n_seeds += __shfl_xor_sync(EMU_FULL, n_seeds, o);
     n_cands += __shfl_xor_sync(EMU_FULL, n_cands, o);
     status |= __shfl_xor_sync(EMU_FULL, status, o);
   }
   if (lane == 0) {
-    atomicAdd(counts + EMU_CNT_SEEDS, n_seeds);
     atomicAdd(counts + EMU_CNT_TESTS, n_tests);
-    atomicAdd(counts + EMU_CNT_PAIR_TESTS, n_pairs);
-    atomicAdd(counts + EMU_CNT_CANDIDATES, n_cands);
+    if (!kDump) atomicAdd(counts + EMU_CNT_CANDIDATES, n_cands);
     if (status) atomicOr(counts + EMU_CNT_STATUS, (unsigned long long)status);
   }
 }
 
-// after k_vote: clamp the candidate count to the capacity and record overflow / need
-__global__ void k_vote_finish(FindCtl* ctl, unsigned cand_cap, unsigned long long* counts) {
+// after the candidates of a chunk are known: capacity check, reset of the tie flag
+__global__ void k_cands_finish(FindCtl* ctl, unsigned cand_cap, unsigned long long* counts) {
   unsigned n = ctl->cand_count;
-  atomicMax(counts + EMU_CNT_NEED, (unsigned long long)n);
-  if (n > cand_cap) { atomicOr(counts + EMU_CNT_STATUS, (unsigned long long)EMU_ST_CAND_OVERFLOW); ctl->cand_count = cand_cap; }
+  if (n > cand_cap) { atomicOr(counts + EMU_CNT_STATUS, (unsigned long long)EMU_ST_CAND_OVERFLOW); ctl->cand_count = 0; ctl->skip = 1; }
   ctl->tie = 0;
 }
 
 // ---------------------------------------------------------------------------------------------
-// A5 part 1: every member grain of every candidate receives max over candidates of
-//   keyA = K1 << 29 | (mask - ci)   and   keyB = K1 << 29 | ci,   K1 = n_tube << 22 | D2.
+// A5 with the generic walker.  kPass 0: priority maximum (only when the chunk runs generic).
+// kPass 1: settlement of ties - every candidate whose (n_tube, D2) is flagged in the tie bitmap walks
+// its tube again and competes for the tied grains by (kmin, kmax) with a CAS-min.
+//   keyA = K1 << 29 | (mask - ci)   keyB = K1 << 29 | ci,   K1 = n_tube << 22 | D2.
 // The top K1 of a grain is unique; keyA and keyB then name the same candidate unless several
-// candidates tie on K1 for that grain (settled exactly in k_assoc_tie).
+// candidates tie on K1 for that grain.
+__device__ __forceinline__ unsigned tie_hash(unsigned long long k1, int vl) {
+  unsigned long long h = (k1 ^ ((unsigned long long)vl << 40)) * 0x9E3779B97F4A7C15ull;
+  return (unsigned)(h >> 48) & (kTieBits - 1);
+}
+
 template <int kPass>
 __global__ void __launch_bounds__(kVoteThreads)
-k_assoc(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ cell_start,
-        const EmuBox* __restrict__ bbox, int v0, const Cand* __restrict__ cands, const FindCtl* __restrict__ ctl,
-        unsigned long long* __restrict__ keyA, unsigned long long* __restrict__ keyB,
-        unsigned* __restrict__ owner) {
+k_assoc_generic(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ cell_start,
+                const EmuBox* __restrict__ bbox, int v0, const Cand* __restrict__ cands, const FindCtl* __restrict__ ctl,
+                const unsigned* __restrict__ tie_bits, unsigned long long* __restrict__ keyA,
+                unsigned long long* __restrict__ keyB, unsigned* __restrict__ owner) {
+  if (ctl->skip) return;
+  if (kPass == 0 && !ctl->generic) return;
   if (kPass == 1 && ctl->tie == 0) return;
   const unsigned n = ctl->cand_count;
   const unsigned stride = gridDim.x * blockDim.x;
   for (unsigned ci = blockIdx.x * blockDim.x + threadIdx.x; ci < n; ci += stride) {
     const Cand c = cands[ci];
-    const int v = v0 + (c.n_tube_view >> 16);
+    const int vl = c.n_tube_view >> 16;
+    const unsigned long long k1 = cand_k1(c.n_tube_view & 0xffff, c.d2);
+    if (kPass == 1) {
+      const unsigned h = tie_hash(k1, vl);
+      if (!((tie_bits[h >> 5] >> (h & 31)) & 1u)) continue;
+    }
+    const int v = v0 + vl;
     const int4 A = __ldg(sorted + c.a), B = __ldg(sorted + c.b);
     const int dx = B.x - A.x, dy = B.y - A.y, dz = B.z - A.z;
-    const unsigned long long k1 = cand_k1(c.n_tube_view & 0xffff, c.d2);
     const EmuBox bb = bbox[v];
     if (kPass == 0) {
       const unsigned long long ka = (k1 << kCiBits) | (unsigned long long)(kCiMask - ci);
@@ -274,32 +860,44 @@ k_assoc(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ cell_
   }
 }
 
+// a grain whose keyA and keyB name different candidates has a tie at its top priority: flag that
+// priority in the bitmap (the settlement pass re-walks only candidates with a flagged priority)
 __global__ void __launch_bounds__(256)
 k_tie_detect(const int* __restrict__ view_off, int v0, int v1, const unsigned long long* __restrict__ keyA,
-             const unsigned long long* __restrict__ keyB, FindCtl* __restrict__ ctl) {
+             const unsigned long long* __restrict__ keyB, FindCtl* __restrict__ ctl, unsigned* __restrict__ tie_bits) {
+  if (ctl->skip) return;
   const int g0 = __ldg(view_off + v0), g1 = __ldg(view_off + v1);
   bool tie = false;
   for (int g = g0 + blockIdx.x * blockDim.x + threadIdx.x; g < g1; g += gridDim.x * blockDim.x) {
     unsigned long long ka = keyA[g], kb = keyB[g];
-    if (ka) tie |= (kCiMask - (unsigned)(ka & kCiMask)) != (unsigned)(kb & kCiMask);
+    if (ka && (kCiMask - (unsigned)(ka & kCiMask)) != (unsigned)(kb & kCiMask)) {
+      tie = true;
+      const int vl = emu_find_view(view_off, v0, v1, g) - v0;
+      const unsigned h = tie_hash(ka >> kCiBits, vl);
+      atomicOr(tie_bits + (h >> 5), 1u << (h & 31));
+    }
   }
   if (__any_sync(EMU_FULL, tie) && (threadIdx.x & 31) == 0) ctl->tie = 1;
 }
 
 __device__ __forceinline__ unsigned owner_of(int g, const FindCtl* ctl, const unsigned long long* keyA,
-                                             const unsigned* owner) {
-  unsigned long long ka = keyA[g];
+                                             const unsigned long long* keyB, const unsigned* owner) {
+  const unsigned long long ka = keyA[g];
   if (!ka) return kNone;
-  return ctl->tie ? owner[g] : (kCiMask - (unsigned)(ka & kCiMask));
+  const unsigned ca = kCiMask - (unsigned)(ka & kCiMask);
+  if (ctl->tie && ca != (unsigned)(keyB[g] & kCiMask)) return owner[g];
+  return ca;
 }
 
 // A5 part 2: members won per candidate
 __global__ void __launch_bounds__(256)
 k_wins(const int* __restrict__ view_off, int v0, int v1, const FindCtl* __restrict__ ctl,
-       const unsigned long long* __restrict__ keyA, const unsigned* __restrict__ owner, int* __restrict__ wins) {
+       const unsigned long long* __restrict__ keyA, const unsigned long long* __restrict__ keyB,
+       const unsigned* __restrict__ owner, int* __restrict__ wins) {
+  if (ctl->skip) return;
   const int g0 = __ldg(view_off + v0), g1 = __ldg(view_off + v1);
   for (int g = g0 + blockIdx.x * blockDim.x + threadIdx.x; g < g1; g += gridDim.x * blockDim.x) {
-    unsigned ci = owner_of(g, ctl, keyA, owner);
+    unsigned ci = owner_of(g, ctl, keyA, keyB, owner);
     if (ci != kNone) atomicAdd(wins + ci, 1);
   }
 }
@@ -308,6 +906,7 @@ k_wins(const int* __restrict__ view_off, int v0, int v1, const FindCtl* __restri
 __global__ void __launch_bounds__(256)
 k_select(EmuDev P, const Cand* __restrict__ cands, const FindCtl* __restrict__ ctl, const int* __restrict__ wins,
          int* __restrict__ view_ntracks, unsigned* __restrict__ view_tracks, unsigned long long* __restrict__ counts) {
+  if (ctl->skip) return;
   const unsigned n = ctl->cand_count;
   for (unsigned ci = blockIdx.x * blockDim.x + threadIdx.x; ci < n; ci += gridDim.x * blockDim.x) {
     if (wins[ci] >= P.min_grains) {
@@ -425,13 +1024,15 @@ k_member_scan(int v0, int v1, const int* __restrict__ track_off, emu_track* __re
 __global__ void __launch_bounds__(256)
 k_member_scatter(const int4* __restrict__ sorted, const int* __restrict__ view_off, int v0, int v1,
                  const FindCtl* __restrict__ ctl, const unsigned long long* __restrict__ keyA,
-                 const unsigned* __restrict__ owner, const unsigned* __restrict__ cand_track,
-                 const int* __restrict__ track_off, const emu_track* __restrict__ tracks,
-                 int* __restrict__ cursor, int* __restrict__ members, long long members_capacity) {
+                 const unsigned long long* __restrict__ keyB, const unsigned* __restrict__ owner,
+                 const unsigned* __restrict__ cand_track, const int* __restrict__ track_off,
+                 const emu_track* __restrict__ tracks, int* __restrict__ cursor, int* __restrict__ members,
+                 long long members_capacity) {
+  if (ctl->skip) return;
   const int g0 = __ldg(view_off + v0), g1 = __ldg(view_off + v1);
   const int t0 = track_off[v0];
   for (int g = g0 + blockIdx.x * blockDim.x + threadIdx.x; g < g1; g += gridDim.x * blockDim.x) {
-    unsigned ci = owner_of(g, ctl, keyA, owner);
+    unsigned ci = owner_of(g, ctl, keyA, keyB, owner);
     if (ci == kNone) continue;
     unsigned t = cand_track[ci];
     if (t == kNone) continue;
@@ -483,70 +1084,140 @@ __global__ void k_reset_cand_arrays(const FindCtl* ctl, int* wins, unsigned* can
   for (unsigned i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) { wins[i] = 0; cand_track[i] = kNone; }
 }
 
+// ---------------------------------------------------------------------------------------------
+// workspace
 struct FindWs {
-  EmuBox* bbox; unsigned long long* keyA; unsigned long long* keyB; unsigned* owner; FindCtl* ctl;
-  int* view_ntracks; unsigned* view_tracks; Cand* cands; int* wins; unsigned* cand_track;
-  size_t cand_cap; int views_per_chunk;
+  EmuBox* bbox; unsigned long long* keyA; unsigned long long* keyB; unsigned* owner; unsigned* seed_off;
+  FindCtl* ctl; unsigned* tie_bits; unsigned long long* dump_cursor;
+  unsigned* view_seed_tot; unsigned* view_seed_off; unsigned* view_cand_cnt; unsigned* view_cand_off;
+  int* view_ntracks; unsigned* view_tracks; Brick* bricks;
+  int4* geo; int2* ab; unsigned* seed_cnt;
+  Cand* cands; int4* cand_geo; int* wins; unsigned* cand_track;
+  size_t seed_cap, cand_cap, brick_cap; int views_per_chunk;
 };
 
-size_t fixed_bytes(const EmuDev& P, int64_t n_grains, int32_t n_views, int views_per_chunk) {
+constexpr size_t kSeedBytes = sizeof(int4) + sizeof(int2) + sizeof(unsigned);                    // 28
+constexpr size_t kCandBytes = sizeof(Cand) + sizeof(int4) + sizeof(int) + sizeof(unsigned);      // 40
+constexpr size_t kMinSeedCap = 1u << 20, kMinCandCap = 1u << 16;
+
+size_t bricks_per_view(const EmuDev& P, const Tiling& T) { return (size_t)T.tx * T.ty * (size_t)P.n[2]; }
+
+size_t fixed_bytes(const EmuDev& P, const Tiling& T, int64_t n_grains, int32_t n_views, int vpc) {
   size_t b = 0;
   b += emu_align256((size_t)n_views * sizeof(EmuBox));
   b += 2 * emu_align256((size_t)n_grains * sizeof(unsigned long long));
-  b += emu_align256((size_t)n_grains * sizeof(unsigned));
-  b += emu_align256(sizeof(FindCtl));
-  b += emu_align256((size_t)views_per_chunk * sizeof(int));
-  b += emu_align256((size_t)views_per_chunk * P.max_tracks * sizeof(unsigned));
+  b += 2 * emu_align256((size_t)n_grains * sizeof(unsigned));
+  b += emu_align256(sizeof(FindCtl)) + emu_align256(kTieBits / 8) + 256;
+  b += 4 * emu_align256(((size_t)vpc + 1) * sizeof(unsigned));
+  b += emu_align256((size_t)vpc * sizeof(int));
+  b += emu_align256((size_t)vpc * P.max_tracks * sizeof(unsigned));
+  b += emu_align256((size_t)vpc * bricks_per_view(P, T) * sizeof(Brick));
   return b + 256;
 }
 
-constexpr size_t kCandBytes = sizeof(Cand) + sizeof(int) + sizeof(unsigned);
-constexpr size_t kMinCandCap = 1u << 16;
+// Tiles per view: enough that an average tile holds about 70 % of kCapG grains and one layer of it fits
+// the cell table; among the factorisations of that count the one whose whole z extent fits the cell
+// table, then the squarest in physical size.
+Tiling choose_tiling(const EmuDev& P, int64_t n_grains, int32_t n_views) {
+  const double avg = n_views > 0 ? (double)n_grains / n_views : 0.0;
+  int need = (int)ceil(avg / (0.70 * kCapG));
+  if (need < 1) need = 1;
+  Tiling fallback; fallback.tx = P.n[0]; fallback.ty = P.n[1]; fallback.w = 1; fallback.h = 1;   // one column per tile
+  bool have_fallback = false;
+  const int64_t max_t = (int64_t)P.n[0] * P.n[1];
+  for (int64_t t = need; t <= emu_min64(max_t, (int64_t)need + 4096); ++t) {
+    Tiling best; best.tx = best.ty = best.w = best.h = 0;
+    double best_score = -1.0;
+    for (int64_t tx = 1; tx <= t; ++tx) {
+      if (t % tx) continue;
+      const int64_t ty = t / tx;
+      if (tx > P.n[0] || ty > P.n[1]) continue;
+      const int w = (int)((P.n[0] + tx - 1) / tx), h = (int)((P.n[1] + ty - 1) / ty);
+      if ((int64_t)w * h > kCapC) continue;
+      const double sx = (double)w * P.cs[0], sy = (double)h * P.cs[1];
+      const double score = (sx < sy ? sx / sy : sy / sx) + (((int64_t)w * h * P.n[2] <= kCapC) ? 1.0 : 0.0);
+      if (score > best_score) { best_score = score; best.tx = (int)tx; best.ty = (int)ty; best.w = w; best.h = h; }
+    }
+    if (best_score >= 1.0) return best;                       // every z layer of a tile fits the cell table
+    if (best_score >= 0.0 && !have_fallback) { fallback = best; have_fallback = true; }
+    if (have_fallback && t >= (int64_t)need + 64) break;
+  }
+  return fallback;
+}
+
+struct Hints { int seeds_per_grain, cand_per_grain; };
 
 }  // namespace
 
 size_t emu_find_ws_min_bytes(const EmuDev& P, int64_t n_grains, int32_t n_views) {
-  return fixed_bytes(P, n_grains, n_views, 1) + kMinCandCap * kCandBytes + 3 * 256;
+  Tiling T = choose_tiling(P, n_grains, n_views);
+  return fixed_bytes(P, T, n_grains, n_views, 1) + kMinSeedCap * kSeedBytes + kMinCandCap * kCandBytes + 8 * 256;
 }
 
-size_t emu_find_ws_recommended_bytes(const EmuDev& P, int64_t n_grains, int32_t n_views, int cand_per_grain) {
-  int64_t want = emu_max64((int64_t)kMinCandCap, emu_min64(n_grains * (int64_t)cand_per_grain, (int64_t)1 << 27));
-  int64_t per_view = emu_max64(1, n_grains / emu_max64(1, n_views)) * cand_per_grain;
-  int vpc = (int)emu_max64(1, emu_min64(n_views, want / emu_max64(1, per_view)));
-  return fixed_bytes(P, n_grains, n_views, vpc) + (size_t)want * kCandBytes + 3 * 256;
+size_t emu_find_ws_recommended_bytes(const EmuDev& P, int64_t n_grains, int32_t n_views, int seeds_per_grain,
+                                     int cand_per_grain) {
+  Tiling T = choose_tiling(P, n_grains, n_views);
+  const int64_t per_view_g = emu_max64(1, (n_grains + emu_max64(1, n_views) - 1) / emu_max64(1, n_views));
+  const int64_t spv = per_view_g * seeds_per_grain, cpv = per_view_g * cand_per_grain;
+  const int64_t per_view_bytes = spv * (int64_t)kSeedBytes + cpv * (int64_t)kCandBytes;
+  // as many views per chunk as fit 24 GiB of seed / candidate storage (at least one)
+  int64_t vpc = emu_max64(1, emu_min64(emu_max64(1, n_views), ((int64_t)24 << 30) / emu_max64(1, per_view_bytes)));
+  vpc = emu_min64(vpc, 65535);
+  const size_t seed_cap = (size_t)emu_max64((int64_t)kMinSeedCap, spv * vpc);
+  const size_t cand_cap = (size_t)emu_max64((int64_t)kMinCandCap, cpv * vpc);
+  return fixed_bytes(P, T, n_grains, n_views, (int)vpc) + seed_cap * kSeedBytes + cand_cap * kCandBytes + 16 * 256;
 }
 
-static int carve(const EmuDev& P, int cand_per_grain, int64_t n_grains, int32_t n_views, void* d_ws, size_t ws_bytes,
-                 FindWs& W) {
+static int carve(const EmuDev& P, const Tiling& T, Hints hints, int64_t n_grains, int32_t n_views, void* d_ws,
+                 size_t ws_bytes, FindWs& W) {
   if (ws_bytes < emu_find_ws_min_bytes(P, n_grains, n_views)) return EMU_ERR_CAPACITY;
-  // choose views per chunk: as many as the candidate estimate allows in what is left after the fixed part
-  int64_t per_view = emu_max64(1, n_grains / emu_max64(1, n_views)) * cand_per_grain;
-  int vpc = n_views > 0 ? n_views : 1;
-  size_t cap = 0;
+  const int64_t per_view_g = emu_max64(1, (n_grains + emu_max64(1, n_views) - 1) / emu_max64(1, n_views));
+  const int64_t spv = per_view_g * hints.seeds_per_grain, cpv = per_view_g * hints.cand_per_grain;
+  // views per chunk: the most whose expected seeds and candidates fit what is left after the fixed part
+  int vpc = n_views > 0 ? (int)emu_min64(n_views, 65535) : 1;
+  size_t seed_cap = 0, cand_cap = 0;
   for (;;) {
-    size_t fx = fixed_bytes(P, n_grains, n_views, vpc);
-    if (fx + kMinCandCap * kCandBytes + 3 * 256 <= ws_bytes) {
-      cap = (ws_bytes - fx - 3 * 256) / kCandBytes;
-      if ((int64_t)cap >= per_view * vpc || vpc == 1) break;
+    const size_t fx = fixed_bytes(P, T, n_grains, n_views, vpc) + 16 * 256;
+    if (fx + kMinSeedCap * kSeedBytes + kMinCandCap * kCandBytes <= ws_bytes) {
+      const size_t avail = ws_bytes - fx;
+      // what is available is split between seeds and candidates in the proportion of the hints
+      const double ws_seed = (double)spv * kSeedBytes, ws_cand = (double)cpv * kCandBytes;
+      seed_cap = (size_t)((double)avail * ws_seed / (ws_seed + ws_cand) / kSeedBytes);
+      if (seed_cap < kMinSeedCap) seed_cap = kMinSeedCap;
+      cand_cap = (avail - seed_cap * kSeedBytes) / kCandBytes;
+      if (cand_cap >= kMinCandCap && ((int64_t)seed_cap >= spv * vpc || vpc == 1)) break;
     }
     if (vpc == 1) return EMU_ERR_CAPACITY;
     vpc = (vpc + 1) / 2;
   }
-  if (cap > (size_t)kCiMask) cap = kCiMask;
-  if (vpc > 65535) vpc = 65535;                      // view-in-chunk field of Cand: 16 bits
+  if (cand_cap > (size_t)kCiMask) cand_cap = kCiMask;
+  if (seed_cap > (size_t)0x7fffffff) seed_cap = 0x7fffffff;
   char* p = (char*)emu_align_ptr(d_ws);
   auto take = [&](size_t bytes) { char* r = p; p += emu_align256(bytes); return r; };
   W.bbox = (EmuBox*)take((size_t)n_views * sizeof(EmuBox));
   W.keyA = (unsigned long long*)take((size_t)n_grains * sizeof(unsigned long long));
   W.keyB = (unsigned long long*)take((size_t)n_grains * sizeof(unsigned long long));
   W.owner = (unsigned*)take((size_t)n_grains * sizeof(unsigned));
+  W.seed_off = (unsigned*)take((size_t)n_grains * sizeof(unsigned));
   W.ctl = (FindCtl*)take(sizeof(FindCtl));
+  W.tie_bits = (unsigned*)take(kTieBits / 8);
+  W.dump_cursor = (unsigned long long*)take(256);
+  W.view_seed_tot = (unsigned*)take(((size_t)vpc + 1) * sizeof(unsigned));
+  W.view_seed_off = (unsigned*)take(((size_t)vpc + 1) * sizeof(unsigned));
+  W.view_cand_cnt = (unsigned*)take(((size_t)vpc + 1) * sizeof(unsigned));
+  W.view_cand_off = (unsigned*)take(((size_t)vpc + 1) * sizeof(unsigned));
   W.view_ntracks = (int*)take((size_t)vpc * sizeof(int));
   W.view_tracks = (unsigned*)take((size_t)vpc * P.max_tracks * sizeof(unsigned));
-  W.cands = (Cand*)take(cap * sizeof(Cand));
-  W.wins = (int*)take(cap * sizeof(int));
-  W.cand_track = (unsigned*)take(cap * sizeof(unsigned));
-  W.cand_cap = cap; W.views_per_chunk = vpc;
+  W.brick_cap = (size_t)vpc * bricks_per_view(P, T);
+  W.bricks = (Brick*)take(W.brick_cap * sizeof(Brick));
+  W.geo = (int4*)take(seed_cap * sizeof(int4));
+  W.ab = (int2*)take(seed_cap * sizeof(int2));
+  W.seed_cnt = (unsigned*)take(seed_cap * sizeof(unsigned));
+  W.cands = (Cand*)take(cand_cap * sizeof(Cand));
+  W.cand_geo = (int4*)take(cand_cap * sizeof(int4));
+  W.wins = (int*)take(cand_cap * sizeof(int));
+  W.cand_track = (unsigned*)take(cand_cap * sizeof(unsigned));
+  W.seed_cap = seed_cap; W.cand_cap = cand_cap; W.views_per_chunk = vpc;
   return EMU_OK;
 }
 
@@ -556,62 +1227,147 @@ static int grid_for(int64_t n, int threads, int max_blocks) {
   return (int)emu_min64(b, max_blocks);
 }
 
-int emu_find_launch(const EmuDev& P, int cand_per_grain, const int32_t* d_sorted, const int32_t* d_cell_start,
-                    const int32_t* d_view_off, int64_t n_grains, int32_t n_views, emu_track* d_tracks,
-                    int32_t* d_track_off, int32_t* d_members, int64_t members_capacity, int64_t* d_counts,
-                    void* d_ws, size_t ws_bytes, cudaStream_t st) {
+static int sm_count() {
+  int dev = 0, v = 0;
+  if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && v > 0) return v;
+  return 148;
+}
+
+#define EMU_CK(x) do { if ((x) != cudaSuccess) return EMU_ERR_CUDA; } while (0)
+
+static int choose_slices(const Tiling& T, int nv, int n_sm) {
+  // enough work items that every SM gets several even when the chunk holds few views
+  const int64_t bricks = emu_max64(1, (int64_t)nv * T.tx * T.ty);
+  int64_t s = (4 * (int64_t)n_sm + bricks - 1) / bricks;
+  if (s < 1) s = 1;
+  if (s > 256) s = 256;
+  return (int)s;
+}
+
+// seeds + votes of the chunk [v0, v1): leaves geo / ab / seed_cnt / view_seed_off filled (brick path), or
+// ctl->generic set
+static int vote_chunk(const EmuDev& P, const Tiling& T, FindWs& W, const int4* sorted, const int32_t* d_cell_start,
+                      const int32_t* d_view_off, int v0, int v1, int slices, int kSM, unsigned long long* counts,
+                      cudaStream_t st) {
+  const int nv = v1 - v0;
+  EMU_CK(cudaMemsetAsync(W.ctl, 0, sizeof(FindCtl), st));
+  EMU_CK(cudaMemsetAsync(W.view_cand_cnt, 0, ((size_t)nv + 1) * sizeof(unsigned), st));
+  EMU_LAUNCH(EMU_STAGE_SEEDS, st, k_seed_pairs<0><<<kSM * 16, kVoteThreads, 0, st>>>(
+      P, sorted, d_cell_start, d_view_off, v0, v1, W.seed_off, nullptr, W.ctl, nullptr, nullptr, counts));
+  EMU_LAUNCH(EMU_STAGE_SEEDS, st, k_view_scan<<<grid_for(nv, 1, kSM * 2), 1024, 0, st>>>(
+      d_view_off, v0, v1, W.seed_off, W.view_seed_tot, counts));
+  EMU_LAUNCH(EMU_STAGE_SEEDS, st, k_chunk_offsets<<<1, 1024, 0, st>>>(
+      nv, W.view_seed_tot, W.view_seed_off, &W.ctl->seed_count, (unsigned)W.seed_cap, (unsigned)EMU_ST_SEED_OVERFLOW,
+      W.ctl, counts, EMU_CNT_SEEDS));
+  EMU_LAUNCH(EMU_STAGE_SEEDS, st, k_seed_pairs<1><<<kSM * 16, kVoteThreads, 0, st>>>(
+      P, sorted, d_cell_start, d_view_off, v0, v1, W.seed_off, W.view_seed_off, W.ctl, W.geo, W.ab, counts));
+  EMU_CK(cudaMemsetAsync(W.seed_cnt, 0, W.seed_cap * sizeof(unsigned), st));
+  EMU_LAUNCH(EMU_STAGE_PREP, st, k_plan<<<grid_for(nv, 4, 1 << 20), 128, 0, st>>>(
+      P, T, d_cell_start, v0, v1, W.bricks, (unsigned)W.brick_cap, W.ctl));
+  EMU_LAUNCH(EMU_STAGE_PREP, st, k_plan_finish<<<1, 1, 0, st>>>(W.ctl, (unsigned)W.brick_cap));
+  EMU_CK(cudaFuncSetAttribute(k_brick<kVote>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kBrickSmem));
+  EMU_LAUNCH(EMU_STAGE_VOTE, st, k_brick<kVote><<<kSM, kBrickThreads, kBrickSmem, st>>>(
+      P, sorted, d_cell_start, W.bbox, v0, W.bricks, W.ctl, slices, W.geo, W.view_seed_off, W.seed_cnt, nullptr, nullptr,
+      counts));
+  return EMU_OK;
+}
+
+int emu_find_launch(const EmuDev& P, int seeds_per_grain, int cand_per_grain, const int32_t* d_sorted,
+                    const int32_t* d_cell_start, const int32_t* d_view_off, int64_t n_grains, int32_t n_views,
+                    emu_track* d_tracks, int32_t* d_track_off, int32_t* d_members, int64_t members_capacity,
+                    int64_t* d_counts, void* d_ws, size_t ws_bytes, cudaStream_t st) {
   FindWs W;
-  int rc = carve(P, cand_per_grain, n_grains, n_views, d_ws, ws_bytes, W);
+  const Tiling T = choose_tiling(P, n_grains, n_views);
+  Hints hints; hints.seeds_per_grain = seeds_per_grain; hints.cand_per_grain = cand_per_grain;
+  int rc = carve(P, T, hints, n_grains, n_views, d_ws, ws_bytes, W);
   if (rc != EMU_OK) return rc;
   const int4* sorted = (const int4*)d_sorted;
   unsigned long long* counts = (unsigned long long*)d_counts;
   const int n = (int)n_grains;
-  const int kSM = 148;
-  if (cudaMemsetAsync(d_counts, 0, 8 * sizeof(int64_t), st) != cudaSuccess) return EMU_ERR_CUDA;
-  if (cudaMemsetAsync(d_track_off, 0, ((size_t)n_views + 1) * sizeof(int32_t), st) != cudaSuccess) return EMU_ERR_CUDA;
-  if (cudaMemsetAsync(W.keyA, 0, (size_t)n_grains * sizeof(unsigned long long), st) != cudaSuccess) return EMU_ERR_CUDA;
-  if (cudaMemsetAsync(W.keyB, 0, (size_t)n_grains * sizeof(unsigned long long), st) != cudaSuccess) return EMU_ERR_CUDA;
-  if (cudaMemsetAsync(W.owner, 0xff, (size_t)n_grains * sizeof(unsigned), st) != cudaSuccess) return EMU_ERR_CUDA;
+  const int kSM = sm_count();
+  EMU_CK(cudaMemsetAsync(d_counts, 0, 8 * sizeof(int64_t), st));
+  EMU_CK(cudaMemsetAsync(d_track_off, 0, ((size_t)n_views + 1) * sizeof(int32_t), st));
+  EMU_CK(cudaMemsetAsync(W.keyA, 0, (size_t)n_grains * sizeof(unsigned long long), st));
+  EMU_CK(cudaMemsetAsync(W.keyB, 0, (size_t)n_grains * sizeof(unsigned long long), st));
+  EMU_CK(cudaMemsetAsync(W.owner, 0xff, (size_t)n_grains * sizeof(unsigned), st));
   EMU_LAUNCH(EMU_STAGE_PREP, st, k_bbox_init<<<grid_for(n_views, 256, 1 << 20), 256, 0, st>>>(W.bbox, n_views));
   EMU_LAUNCH(EMU_STAGE_PREP, st, k_bbox<<<grid_for(n, 256, kSM * 8), 256, 0, st>>>(sorted, d_view_off, n_views, n, W.bbox));
 
   for (int v0 = 0; v0 < n_views; v0 += W.views_per_chunk) {
     const int v1 = (int)emu_min64(n_views, (int64_t)v0 + W.views_per_chunk);
     const int nv = v1 - v0;
-    if (cudaMemsetAsync(W.ctl, 0, sizeof(FindCtl), st) != cudaSuccess) return EMU_ERR_CUDA;
-    if (cudaMemsetAsync(W.view_ntracks, 0, (size_t)nv * sizeof(int), st) != cudaSuccess) return EMU_ERR_CUDA;
-    EMU_LAUNCH(EMU_STAGE_VOTE, st, k_vote<false><<<kSM * 16, kVoteThreads, 0, st>>>(P, sorted, d_cell_start, d_view_off, W.bbox, v0, v1, W.cands,
-                                                     (unsigned)W.cand_cap, W.ctl, nullptr, 0, counts));
-    EMU_LAUNCH(EMU_STAGE_PREP, st, k_vote_finish<<<1, 1, 0, st>>>(W.ctl, (unsigned)W.cand_cap, counts));
+    const int slices = choose_slices(T, nv, kSM);
+    EMU_CK(cudaMemsetAsync(W.view_ntracks, 0, (size_t)nv * sizeof(int), st));
+    EMU_CK(cudaMemsetAsync(W.tie_bits, 0, kTieBits / 8, st));
+    rc = vote_chunk(P, T, W, sorted, d_cell_start, d_view_off, v0, v1, slices, kSM, counts, st);
+    if (rc != EMU_OK) return rc;
+    // A4: candidates grouped by view
+    EMU_LAUNCH(EMU_STAGE_CANDS, st, k_cands<0><<<dim3(64, nv), 256, 0, st>>>(
+        P, v0, W.ctl, W.view_seed_off, W.seed_cnt, W.geo, W.ab, W.view_cand_cnt, nullptr, nullptr, nullptr, counts));
+    EMU_LAUNCH(EMU_STAGE_CANDS, st, k_chunk_offsets<<<1, 1024, 0, st>>>(
+        nv, W.view_cand_cnt, W.view_cand_off, &W.ctl->cand_count, (unsigned)W.cand_cap, (unsigned)EMU_ST_CAND_OVERFLOW,
+        W.ctl, counts, EMU_CNT_CANDIDATES));
+    EMU_CK(cudaMemsetAsync(W.view_cand_cnt, 0, ((size_t)nv + 1) * sizeof(unsigned), st));
+    EMU_LAUNCH(EMU_STAGE_CANDS, st, k_cands<1><<<dim3(64, nv), 256, 0, st>>>(
+        P, v0, W.ctl, W.view_seed_off, W.seed_cnt, W.geo, W.ab, W.view_cand_cnt, W.view_cand_off, W.cands, W.cand_geo,
+        counts));
+    // generic fallback for the whole chunk (returns at once unless the brick plan failed)
+    EMU_LAUNCH(EMU_STAGE_VOTE, st, k_vote_generic<false><<<kSM * 16, kVoteThreads, 0, st>>>(
+        P, sorted, d_cell_start, d_view_off, W.bbox, v0, v1, W.cands, (unsigned)W.cand_cap, W.ctl, nullptr, 0, nullptr,
+        counts));
+    EMU_LAUNCH(EMU_STAGE_PREP, st, k_cands_finish<<<1, 1, 0, st>>>(W.ctl, (unsigned)W.cand_cap, counts));
     EMU_LAUNCH(EMU_STAGE_PREP, st, k_reset_cand_arrays<<<kSM * 8, 256, 0, st>>>(W.ctl, W.wins, W.cand_track));
-    EMU_LAUNCH(EMU_STAGE_ASSOC, st, k_assoc<0><<<kSM * 16, kVoteThreads, 0, st>>>(P, sorted, d_cell_start, W.bbox, v0, W.cands, W.ctl, W.keyA, W.keyB, W.owner));
-    EMU_LAUNCH(EMU_STAGE_ASSOC, st, k_tie_detect<<<kSM * 4, 256, 0, st>>>(d_view_off, v0, v1, W.keyA, W.keyB, W.ctl));
-    EMU_LAUNCH(EMU_STAGE_ASSOC, st, k_assoc<1><<<kSM * 16, kVoteThreads, 0, st>>>(P, sorted, d_cell_start, W.bbox, v0, W.cands, W.ctl, W.keyA, W.keyB, W.owner));
-    EMU_LAUNCH(EMU_STAGE_SELECT, st, k_wins<<<kSM * 4, 256, 0, st>>>(d_view_off, v0, v1, W.ctl, W.keyA, W.owner, W.wins));
+    // A5
+    EMU_CK(cudaFuncSetAttribute(k_brick<kAssoc>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kBrickSmem));
+    EMU_LAUNCH(EMU_STAGE_ASSOC, st, k_brick<kAssoc><<<kSM, kBrickThreads, kBrickSmem, st>>>(
+        P, sorted, d_cell_start, W.bbox, v0, W.bricks, W.ctl, slices, W.cand_geo, W.view_cand_off, nullptr, W.keyA, W.keyB,
+        counts));
+    EMU_LAUNCH(EMU_STAGE_ASSOC, st, k_assoc_generic<0><<<kSM * 16, kVoteThreads, 0, st>>>(
+        P, sorted, d_cell_start, W.bbox, v0, W.cands, W.ctl, W.tie_bits, W.keyA, W.keyB, W.owner));
+    EMU_LAUNCH(EMU_STAGE_ASSOC, st, k_tie_detect<<<kSM * 4, 256, 0, st>>>(d_view_off, v0, v1, W.keyA, W.keyB, W.ctl, W.tie_bits));
+    EMU_LAUNCH(EMU_STAGE_ASSOC, st, k_assoc_generic<1><<<kSM * 16, kVoteThreads, 0, st>>>(
+        P, sorted, d_cell_start, W.bbox, v0, W.cands, W.ctl, W.tie_bits, W.keyA, W.keyB, W.owner));
+    EMU_LAUNCH(EMU_STAGE_SELECT, st, k_wins<<<kSM * 4, 256, 0, st>>>(d_view_off, v0, v1, W.ctl, W.keyA, W.keyB, W.owner, W.wins));
     EMU_LAUNCH(EMU_STAGE_SELECT, st, k_select<<<kSM * 8, 256, 0, st>>>(P, W.cands, W.ctl, W.wins, W.view_ntracks, W.view_tracks, counts));
     EMU_LAUNCH(EMU_STAGE_EMIT, st, k_track_scan<<<1, 1024, 0, st>>>(P, v0, v1, W.view_ntracks, d_track_off));
-    EMU_LAUNCH(EMU_STAGE_EMIT, st, k_track_emit<<<grid_for(nv, 1, kSM * 8), 256, 0, st>>>(P, sorted, v0, v1, W.cands, W.wins, W.view_ntracks,
-                                                          W.view_tracks, d_track_off, d_tracks, W.cand_track));
+    EMU_LAUNCH(EMU_STAGE_EMIT, st, k_track_emit<<<grid_for(nv, 1, kSM * 8), 256, 0, st>>>(
+        P, sorted, v0, v1, W.cands, W.wins, W.view_ntracks, W.view_tracks, d_track_off, d_tracks, W.cand_track));
     // the per-track fill cursors reuse view_tracks (its contents are dead after k_track_emit)
     EMU_LAUNCH(EMU_STAGE_EMIT, st, k_member_scan<<<1, 1024, 0, st>>>(v0, v1, d_track_off, d_tracks, (int*)W.view_tracks, counts, members_capacity));
-    EMU_LAUNCH(EMU_STAGE_EMIT, st, k_member_scatter<<<kSM * 4, 256, 0, st>>>(sorted, d_view_off, v0, v1, W.ctl, W.keyA, W.owner, W.cand_track,
-                                              d_track_off, d_tracks, (int*)W.view_tracks, d_members, members_capacity));
+    EMU_LAUNCH(EMU_STAGE_EMIT, st, k_member_scatter<<<kSM * 4, 256, 0, st>>>(
+        sorted, d_view_off, v0, v1, W.ctl, W.keyA, W.keyB, W.owner, W.cand_track, d_track_off, d_tracks, (int*)W.view_tracks,
+        d_members, members_capacity));
     EMU_LAUNCH(EMU_STAGE_EMIT, st, k_member_sort<<<kSM * 4, 256, 0, st>>>(v0, v1, d_track_off, d_tracks, d_members, members_capacity));
   }
   return cudaGetLastError() == cudaSuccess ? EMU_OK : EMU_ERR_CUDA;
 }
 
-int emu_count_seeds_launch(const EmuDev& P, const int32_t* d_sorted, const int32_t* d_cell_start,
-                           const int32_t* d_view_off, int64_t n_grains, int32_t n_views, int32_t* d_seed_dump,
-                           int64_t dump_capacity, int64_t* d_counts, void* d_ws, size_t ws_bytes, cudaStream_t st) {
-  if (ws_bytes < emu_align256((size_t)n_views * sizeof(EmuBox)) + 256) return EMU_ERR_CAPACITY;
-  EmuBox* bbox = (EmuBox*)emu_align_ptr(d_ws);
+int emu_count_seeds_launch(const EmuDev& P, int seeds_per_grain, int cand_per_grain, const int32_t* d_sorted,
+                           const int32_t* d_cell_start, const int32_t* d_view_off, int64_t n_grains, int32_t n_views,
+                           int32_t* d_seed_dump, int64_t dump_capacity, int64_t* d_counts, void* d_ws, size_t ws_bytes,
+                           cudaStream_t st) {
+  FindWs W;
+  const Tiling T = choose_tiling(P, n_grains, n_views);
+  Hints hints; hints.seeds_per_grain = seeds_per_grain; hints.cand_per_grain = cand_per_grain;
+  int rc = carve(P, T, hints, n_grains, n_views, d_ws, ws_bytes, W);
+  if (rc != EMU_OK) return rc;
+  if (W.views_per_chunk < n_views) return EMU_ERR_CAPACITY;      // the per-seed dump is a one-chunk test aid
+  const int4* sorted = (const int4*)d_sorted;
+  unsigned long long* counts = (unsigned long long*)d_counts;
   const int n = (int)n_grains;
-  if (cudaMemsetAsync(d_counts, 0, 8 * sizeof(int64_t), st) != cudaSuccess) return EMU_ERR_CUDA;
-  EMU_LAUNCH(EMU_STAGE_PREP, st, k_bbox_init<<<grid_for(n_views, 256, 1 << 20), 256, 0, st>>>(bbox, n_views));
-  EMU_LAUNCH(EMU_STAGE_PREP, st, k_bbox<<<grid_for(n, 256, 148 * 8), 256, 0, st>>>((const int4*)d_sorted, d_view_off, n_views, n, bbox));
-  EMU_LAUNCH(EMU_STAGE_VOTE, st, k_vote<true><<<148 * 16, kVoteThreads, 0, st>>>(P, (const int4*)d_sorted, d_cell_start, d_view_off, bbox, 0, n_views,
-                                                  nullptr, 0, nullptr, (int4*)d_seed_dump, dump_capacity,
-                                                  (unsigned long long*)d_counts));
+  const int kSM = sm_count();
+  EMU_CK(cudaMemsetAsync(d_counts, 0, 8 * sizeof(int64_t), st));
+  EMU_CK(cudaMemsetAsync(W.dump_cursor, 0, 256, st));
+  EMU_LAUNCH(EMU_STAGE_PREP, st, k_bbox_init<<<grid_for(n_views, 256, 1 << 20), 256, 0, st>>>(W.bbox, n_views));
+  EMU_LAUNCH(EMU_STAGE_PREP, st, k_bbox<<<grid_for(n, 256, kSM * 8), 256, 0, st>>>(sorted, d_view_off, n_views, n, W.bbox));
+  if (n_views > 0) {
+    rc = vote_chunk(P, T, W, sorted, d_cell_start, d_view_off, 0, n_views, choose_slices(T, n_views, kSM), kSM, counts, st);
+    if (rc != EMU_OK) return rc;
+    EMU_LAUNCH(EMU_STAGE_CANDS, st, k_seed_dump<<<dim3(64, n_views), 256, 0, st>>>(
+        0, W.ctl, sorted, W.view_seed_off, W.seed_cnt, W.ab, (int4*)d_seed_dump, dump_capacity));
+    EMU_LAUNCH(EMU_STAGE_VOTE, st, k_vote_generic<true><<<kSM * 16, kVoteThreads, 0, st>>>(
+        P, sorted, d_cell_start, d_view_off, W.bbox, 0, n_views, nullptr, 0, W.ctl, (int4*)d_seed_dump, dump_capacity,
+        W.dump_cursor, counts));
+  }
   return cudaGetLastError() == cudaSuccess ? EMU_OK : EMU_ERR_CUDA;
 }

@@ -35,12 +35,13 @@ int emu_bin_launch(const EmuDev& P, const int32_t* d_grains, const int32_t* d_vi
 
 // emu_find.cu
 size_t emu_find_ws_min_bytes(const EmuDev& P, int64_t n_grains, int32_t n_views);
-size_t emu_find_ws_recommended_bytes(const EmuDev& P, int64_t n_grains, int32_t n_views, int cand_per_grain);
-int emu_find_launch(const EmuDev& P, int cand_per_grain, const int32_t* d_sorted, const int32_t* d_cell_start,
+size_t emu_find_ws_recommended_bytes(const EmuDev& P, int64_t n_grains, int32_t n_views, int seeds_per_grain,
+                                     int cand_per_grain);
+int emu_find_launch(const EmuDev& P, int seeds_per_grain, int cand_per_grain, const int32_t* d_sorted, const int32_t* d_cell_start,
                     const int32_t* d_view_off, int64_t n_grains, int32_t n_views, emu_track* d_tracks,
                     int32_t* d_track_off, int32_t* d_members, int64_t members_capacity, int64_t* d_counts,
                     void* d_ws, size_t ws_bytes, cudaStream_t st);
-int emu_count_seeds_launch(const EmuDev& P, const int32_t* d_sorted, const int32_t* d_cell_start,
+int emu_count_seeds_launch(const EmuDev& P, int seeds_per_grain, int cand_per_grain, const int32_t* d_sorted, const int32_t* d_cell_start,
                            const int32_t* d_view_off, int64_t n_grains, int32_t n_views, int32_t* d_seed_dump,
                            int64_t dump_capacity, int64_t* d_counts, void* d_ws, size_t ws_bytes,
                            cudaStream_t st);
