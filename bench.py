@@ -27,7 +27,7 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 CFG = 4                          # BASELINE.json configs[4] "throughput batch"
-CELL_UM = (8.0, 8.0, 8.0)        # cell size of the 3D hash (a pure speed knob: no effect on the track list)
+CELL_UM = (4.0, 4.0, 4.0)        # cell size of the 3D hash (a pure speed knob: no effect on the track list)
 VIEW_AREA_CM2 = 350e-4 * 300e-4  # 350 x 300 um = 1.05e-3 cm^2 per view
 # Algorithmic work of the voting kernel: lane-instructions per seed
 #   = tests/seed * 18 + pair-tests/seed * 9, with tests/seed and pair-tests/seed the ORACLE's own counters

@@ -39,6 +39,14 @@ EmuDev make_dev(const emu_params* p) {
   d.r2 = p->tube_r2_q;
   int r = 0; while ((int64_t)r * r < p->tube_r2_q) ++r;
   d.Rw = (float)(r + 2);
+  d.Rup = (float)r;
+  for (int i = 0; i < 3; ++i) {
+    d.csf[i] = (float)d.cs[i];
+    d.klo[i] = -(d.Rw * d.inv_cs[i] + 0.5f);
+    d.khi[i] = d.Rw * d.inv_cs[i] - 0.5f;
+  }
+  // 4-byte grains: x in 16 bits, y and z relative to their cell in 8 bits each (emu_find.cu)
+  d.packed_ok = ((int64_t)d.n[0] * d.cs[0] <= 65536 && d.cs[1] <= 256 && d.cs[2] <= 256) ? 1 : 0;
   d.min_grains = p->min_grains;
   d.max_tracks = p->max_tracks_per_view;
   return d;

@@ -21,6 +21,12 @@ struct EmuDev {           // passed by value to every kernel
   float Rw;               // walk radius: ceil(sqrt(r2)) + 2 q of slack for the float bounds
   int min_grains;
   int max_tracks;
+  // brick kernels (emu_find.cu): cell index of a dilated bound without a float->int conversion,
+  //   lo = rn(x * inv_cs + klo), hi = rn(x * inv_cs + khi), klo = -(Rw * inv_cs + 0.5), khi = Rw * inv_cs - 0.5
+  float klo[3], khi[3];
+  float csf[3];           // cell size as float
+  float Rup;              // ceil(sqrt(r2)) as float (error band of the float tube test)
+  int packed_ok;          // 1: the 4-byte grain format of the brick kernels can hold a view of this grid
 };
 
 // floor(c / cs) clamped to [0, n-1] (reading Q13: out-of-box grains land in the boundary cells).

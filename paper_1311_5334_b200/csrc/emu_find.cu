@@ -32,12 +32,16 @@ constexpr unsigned kCiMask = (1u << kCiBits) - 1u;
 constexpr unsigned kNone = 0xffffffffu;
 constexpr int kMaxTube = 8191;                    // n_tube field of the packed priority: 13 bits
 
-constexpr int kBrickThreads = 512;                // one persistent block per SM
-constexpr int kCapG = 11776;                      // grains a brick may hold   (16 B each)
-constexpr int kCapC = 16384;                      // cells a brick may hold    (2 B each)
+constexpr int kBrickThreads = 1024;               // one persistent block per SM
+constexpr int kPoolBytes = 222 * 1024;            // dynamic shared memory of a brick: grains | row table | cell table
 constexpr int kGrab = 128;                        // seeds a warp takes from the block's stream at a time
-constexpr size_t kBrickSmem = (size_t)kCapG * 16 + (size_t)(kCapC + 2) * 2;
 constexpr int kTieBits = 1 << 16;                 // bitmap of tied priorities
+
+// shared-memory bytes of a brick with n grains in `rows` rows of cells, each w cells wide:
+// 4 B per grain, 4 B per row (sorted position of the row's first grain), 2 B per cell (+ the end mark)
+__host__ __device__ inline long long brick_bytes(long long n, long long rows, long long w) {
+  return 4 * n + 4 * rows + 2 * (rows * w + 2);
+}
 
 struct Cand {            // 16 B
   int a, b;              // sorted positions of the seed grains, a < b
@@ -95,20 +99,30 @@ __device__ bool cand_better(const int4* __restrict__ sorted, const Cand& c, cons
   return cand_kless(sorted, c, e);
 }
 
-// Packed seed geometry, 16 B: the line A + t*d and (for candidates) its n_tube.
-//   x = n_tube << 19 | Ax (19 bits, signed)      y = Ay
-//   z = Az << 12 | dz (12 bits, signed)          w = dx (12 bits, signed) << 12 | dy (12 bits, signed)
-// |A| < 2^17 and |d| < 2^11 (D2 < sep_max^2 <= 2^22), so every field fits.
+// Packed seed geometry, 16 B: the line A + t*d and (for candidates) its n_tube.  Only views whose grains
+// all lie inside the box take the brick path (k_plan), so A fits 16 bits per axis; |d| < 2^11.
+//   x = Ax | Ay << 16      y = Az | n_tube << 16 (13 bits)
+//   z = (dx + 2048) | (dy + 2048) << 16      w = dz + 2048
 __device__ __forceinline__ int4 geo_pack(int ax, int ay, int az, int dx, int dy, int dz) {
   int4 g;
-  g.x = ax & 0x7ffff; g.y = ay; g.z = (az << 12) | (dz & 0xfff); g.w = ((dx & 0xfff) << 12) | (dy & 0xfff);
+  g.x = (ax & 0xffff) | (ay << 16); g.y = az & 0xffff;
+  g.z = ((dx + 2048) & 0xffff) | ((dy + 2048) << 16); g.w = (dz + 2048) & 0xffff;
   return g;
 }
-__device__ __forceinline__ int sbfe(int v, int pos, int len) {
-  int r;
-  asm("bfe.s32 %0, %1, %2, %3;" : "=r"(r) : "r"(v), "r"(pos), "r"(len));
-  return r;
+__device__ __forceinline__ void geo_d(const int4& g, int& dx, int& dy, int& dz) {
+  dx = (g.z & 0xffff) - 2048; dy = (int)((unsigned)g.z >> 16) - 2048; dz = (g.w & 0xffff) - 2048;
 }
+// 16 bits of a word as a float WITHOUT a conversion instruction: the bytes are dropped into the mantissa
+// of 2^23, so the result is 2^23 + value exactly ("magic" float).  sel picks the bytes (PRMT).
+constexpr unsigned kMagic = 0x4B000000u;           // 2^23
+constexpr float kMagicF = 8388608.0f;
+__device__ __forceinline__ float magic_lo16(unsigned w) { return __uint_as_float(__byte_perm(w, kMagic, 0x7410)); }
+__device__ __forceinline__ float magic_hi16(unsigned w) { return __uint_as_float(__byte_perm(w, kMagic, 0x7432)); }
+__device__ __forceinline__ float magic_b2(unsigned w) { return __uint_as_float(__byte_perm(w, kMagic, 0x7442)); }
+__device__ __forceinline__ float magic_b3(unsigned w) { return __uint_as_float(__byte_perm(w, kMagic, 0x7443)); }
+// round-to-nearest float -> int and small int -> float through the 1.5 * 2^23 trick (|value| < 2^22)
+__device__ __forceinline__ int rn_int(float y) { return __float_as_int(__fadd_rn(y, 12582912.0f)) - 0x4B400000; }
+__device__ __forceinline__ float int_f(int i) { return __fadd_rn(__int_as_float(i + 0x4B400000), -12582912.0f); }
 
 // ---------------------------------------------------------------------------------------------
 // per-view bounding boxes
@@ -309,21 +323,31 @@ k_chunk_offsets(int nv, const unsigned* __restrict__ tot, unsigned* __restrict__
 
 // ---------------------------------------------------------------------------------------------
 // Brick plan: one warp per view.  Every tile (tx, ty) of cell columns is cut into runs of z layers
-// that hold at most kCapG grains and kCapC cells; empty bricks are dropped.
+// whose grains, row table and cell table fit the shared-memory pool; empty bricks are dropped.
+// The brick kernels keep a grain in 4 bytes (x in 16 bits, y and z relative to the cell in 8 bits),
+// which needs every grain of the view inside the box: a view with out-of-box grains (legal, reading
+// Q13), or a grid the format cannot hold, sends the chunk to the generic kernels.
 __global__ void __launch_bounds__(128)
-k_plan(EmuDev P, Tiling T, const int* __restrict__ cell_start, int v0, int v1, Brick* __restrict__ bricks,
-       unsigned brick_cap, FindCtl* __restrict__ ctl) {
+k_plan(EmuDev P, Tiling T, const int* __restrict__ cell_start, const EmuBox* __restrict__ bbox, int v0, int v1,
+       Brick* __restrict__ bricks, unsigned brick_cap, FindCtl* __restrict__ ctl) {
   const int lane = threadIdx.x & 31;
   const int v = v0 + blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
   if (v >= v1 || ctl->skip) return;
   const int nx = P.n[0], ny = P.n[1], nz = P.n[2];
   const int vbase = v * P.ncell;
+  if (cell_start[vbase + P.ncell] == cell_start[vbase]) return;          // empty view: no bricks
+  {
+    const EmuBox bb = bbox[v];
+    bool in_box = P.packed_ok != 0;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) in_box = in_box && bb.lo[a] >= 0 && bb.hi[a] < P.n[a] * P.cs[a];
+    if (!in_box) { if (lane == 0) ctl->generic = 1; return; }
+  }
   for (int t = 0; t < T.tx * T.ty; ++t) {
     const int cx0 = (t % T.tx) * T.w, cy0 = (t / T.tx) * T.h;
     const int cx1 = min(nx, cx0 + T.w) - 1, cy1 = min(ny, cy0 + T.h) - 1;
     if (cx0 > cx1 || cy0 > cy1) continue;
-    const int layer_cells = (cx1 - cx0 + 1) * (cy1 - cy0 + 1);
-    if (layer_cells > kCapC) { if (lane == 0) ctl->generic = 1; return; }
+    const int W = cx1 - cx0 + 1, H = cy1 - cy0 + 1;
     int z_first = 0, acc = 0;
     for (int cz = 0; cz <= nz; ++cz) {
       int cnt = 0;
@@ -333,9 +357,9 @@ k_plan(EmuDev P, Tiling T, const int* __restrict__ cell_start, int v0, int v1, B
           cnt += __ldg(cell_start + rb + cx1 + 1) - __ldg(cell_start + rb + cx0);
         }
         cnt = __reduce_add_sync(EMU_FULL, cnt);
-        if (cnt > kCapG) { if (lane == 0) ctl->generic = 1; return; }
+        if (brick_bytes(cnt, H, W) > kPoolBytes) { if (lane == 0) ctl->generic = 1; return; }
       }
-      const bool flush = (cz == nz) || (acc + cnt > kCapG) || ((cz - z_first + 1) * layer_cells > kCapC);
+      const bool flush = (cz == nz) || brick_bytes(acc + cnt, (long long)(cz - z_first + 1) * H, W) > kPoolBytes;
       if (flush) {
         if (acc > 0 && lane == 0) {
           const unsigned slot = atomicAdd(&ctl->n_bricks, 1u);
@@ -359,26 +383,33 @@ __global__ void k_plan_finish(FindCtl* ctl, unsigned brick_cap) {
 // ---------------------------------------------------------------------------------------------
 // A3 / A5 on shared-memory bricks.
 //
-// A persistent block takes work items (brick, slice of the view's seed list).  It stages the brick
-// - the grains of its cells in (cz, cy, cx) order and a 16-bit local cell table - in shared memory
-// and streams the seeds of the slice past it.  Each LANE owns one seed at a time and is in one of
-// three states; the warp repeatedly executes the phase most of its lanes wait for (persistent-thread
-// ray traversal):
+// A persistent block takes work items (brick, slice of the view's seed list).  It stages the brick in
+// shared memory - every grain in 4 bytes (x | y-in-cell << 16 | z-in-cell << 24) in (cz, cy, cx) order,
+// a 16-bit cell table, and per row of cells the sorted position of its first grain - and streams the
+// seeds of the slice past it.  Each LANE owns one seed at a time and is in one of three states; the
+// warp repeatedly executes the phase most of its lanes wait for (persistent-thread ray traversal):
 //   SEED  fetch the next seed of the warp's range, unpack it, clip the line against the brick
-//   ROW   advance the traversal: next z layer of the brick, next row of cells (cy) in it, giving a run
-//         [j, e) of consecutive grains of the cells cx0..cx1 the tube can touch in that row
-//   TEST  one exact integer point-line test of grain j (emu_in_tube); VOTE counts, ASSOC takes part in
-//         the priority maximum of the grain
-// The traversal bounds are conservative float intervals (a grain in the tube is within R of its foot
-// on the line in every coordinate), widened by Rw = R + 2 q against rounding; only the integer test
-// decides, so the bounds only have to be a superset.  Boundary cells of the VIEW are open-ended
-// because out-of-box grains are clamped into them (reading Q13): they reach to the view's bounding box.
+//   ROW   advance the traversal: next row of cells (cy) of the current z layer, else the next layer,
+//         giving a run [j, e) of consecutive grains of the cells cx0..cx1 the tube can touch in the row
+//   TEST  one point-line test of grain j; VOTE counts, ASSOC joins the priority maximum of the grain
+//
+// Traversal: the line is X(t) = A + t d.  A grain in the tube is within R of its foot on the line in
+// every coordinate, so a grain in row (cy, cz) has its foot parameter in the intersection of the two
+// slab intervals widened by Rw = R + 2 q, and its x within Rw of x over that interval.  The bounds are
+// float (errors far below the 2 q of slack) and only have to be a superset: the test decides.
+//
+// Test: v = P - A and d are exact in float (|v| < 2^16, |d| < 2^11).  c = v x d is formed as
+// fma(v1, d2, -rn(v2 d1)): the products stay below 2^27, so |c_f - c| <= 4 + 2^-24 |c| per component, and
+// s_f = |c_f|^2 carries a relative error below 2^-22.  With m_up = R_up (|dx| + |dy| + |dz|) >= sqrt(T),
+// T = r2 D2, delta = 16 + 2^-21 m_up and band = 1.01 (2 m_up delta + delta^2) + 2^-20 T:
+//   s_f <= T - band  =>  in the tube;   s_f > T + band  =>  outside;   otherwise the exact 64-bit
+// integer predicate (emu_in_tube) decides.  The result is therefore the exact one in every case
+// (DESIGN.md section 6 has the derivation).
 enum { kVote = 0, kAssoc = 1 };
 enum { S_NEED = 0, S_ROW = 1, S_TEST = 2 };
 
 struct BrickShared {
   int row_gs[kBrickThreads];
-  int row_off[kBrickThreads];
   unsigned warp_sum[kBrickThreads / 32];
   unsigned work;
   unsigned next, end;
@@ -388,26 +419,28 @@ struct BrickShared {
 template <int kMode>
 __global__ void __launch_bounds__(kBrickThreads, 1)
 k_brick(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ cell_start,
-        const EmuBox* __restrict__ bbox, int v0, const Brick* __restrict__ bricks, FindCtl* __restrict__ ctl,
+        int v0, const Brick* __restrict__ bricks, FindCtl* __restrict__ ctl,
         int slices, const int4* __restrict__ geo, const unsigned* __restrict__ view_item_off,
         unsigned* __restrict__ seed_cnt, unsigned long long* __restrict__ keyA,
         unsigned long long* __restrict__ keyB, unsigned long long* __restrict__ counts) {
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  int4* sg = reinterpret_cast<int4*>(smem_raw);
-  unsigned short* lcs = reinterpret_cast<unsigned short*>(smem_raw + (size_t)kCapG * 16);
+  extern __shared__ __align__(16) unsigned char pool[];
   __shared__ BrickShared sh;
 
   if (ctl->skip || ctl->generic) return;
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   const unsigned n_items = ctl->n_bricks * (unsigned)slices;
   const float R = P.Rw;
+  const float r2f = (float)P.r2;
+  const float BIG = 1.0e9f;
   unsigned long long n_tests = 0;
   int cur_brick = -1;
   Brick B;
   B.view = 0; B.cx0 = B.cx1 = B.cy0 = B.cy1 = B.cz0 = B.cz1 = B.n = 0;
   int W = 1, H = 1;
   float blo[3] = {0.f, 0.f, 0.f}, bhi[3] = {0.f, 0.f, 0.f};   // brick extent widened by R
-  int elo[3] = {0, 0, 0}, ehi[3] = {0, 0, 0};                 // open-ended extent of the view's boundary cells
+  const unsigned* sg = reinterpret_cast<const unsigned*>(pool);
+  const int* rdelta = reinterpret_cast<const int*>(pool);
+  const unsigned short* lcs = reinterpret_cast<const unsigned short*>(pool);
 
   for (;;) {
     __syncthreads();                                  // everyone is done with the previous item
@@ -424,19 +457,15 @@ k_brick(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ cell_
       W = B.cx1 - B.cx0 + 1; H = B.cy1 - B.cy0 + 1;
       const int rows = H * (B.cz1 - B.cz0 + 1);
       const int vbase = B.view * P.ncell;
-      const EmuBox bb = bbox[B.view];
-#pragma unroll
-      for (int a = 0; a < 3; ++a) {
-        elo[a] = min(bb.lo[a], 0);
-        ehi[a] = max(bb.hi[a], P.n[a] * P.cs[a] - 1);
-      }
+      unsigned* sgw = reinterpret_cast<unsigned*>(pool);
+      int* rdw = reinterpret_cast<int*>(pool + 4 * (size_t)B.n);
+      unsigned short* lcw = reinterpret_cast<unsigned short*>(pool + 4 * (size_t)B.n + 4 * (size_t)rows);
+      sg = sgw; rdelta = rdw; lcs = lcw;
       {
         const int c0[3] = {B.cx0, B.cy0, B.cz0}, c1[3] = {B.cx1, B.cy1, B.cz1};
 #pragma unroll
         for (int a = 0; a < 3; ++a) {
-          const int lo = (c0[a] == 0) ? elo[a] : c0[a] * P.cs[a];
-          const int hi = (c1[a] == P.n[a] - 1) ? ehi[a] : (c1[a] + 1) * P.cs[a] - 1;
-          blo[a] = (float)lo - R; bhi[a] = (float)hi + R;
+          blo[a] = (float)(c0[a] * P.cs[a]) - R; bhi[a] = (float)((c1[a] + 1) * P.cs[a] - 1) + R;
         }
       }
       if (tid == 0) sh.carry = 0;
@@ -463,27 +492,28 @@ k_brick(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ cell_
         }
         __syncthreads();
         const int carry = sh.carry;
+        const int off = carry + (int)sh.warp_sum[wid] + incl - len;     // first slot of row r in the brick
         sh.row_gs[tid] = gs;
-        sh.row_off[tid] = carry + (int)sh.warp_sum[wid] + incl - len;
+        if (r < rows) rdw[r] = gs - off;
         __syncthreads();
-        if (tid == kBrickThreads - 1) sh.carry = carry + (int)sh.warp_sum[wid] + incl;
+        if (tid == kBrickThreads - 1) sh.carry = off + len;
         const int nr = min(kBrickThreads, rows - r0);
         for (int k = wid; k < nr; k += kBrickThreads / 32) {
-          const int rgs = sh.row_gs[k], roff = sh.row_off[k];
           const int rr = r0 + k;
+          const int rgs = sh.row_gs[k], roff = rgs - rdw[rr];
           const int cz = B.cz0 + rr / H, cy = B.cy0 + rr % H;
           const int rb = vbase + (cz * P.n[1] + cy) * P.n[0] + B.cx0;
-          for (int i = lane; i < W; i += 32) lcs[rr * W + i] = (unsigned short)(roff + (__ldg(cell_start + rb + i) - rgs));
+          for (int i = lane; i < W; i += 32) lcw[rr * W + i] = (unsigned short)(roff + (__ldg(cell_start + rb + i) - rgs));
           const int rlen = __ldg(cell_start + rb + W) - rgs;
+          const int y0 = cy * P.cs[1], z0 = cz * P.cs[2];
           for (int i = lane; i < rlen; i += 32) {
-            int4 g = __ldg(sorted + rgs + i);
-            g.w = rgs + i;                               // the grain's sorted position (ASSOC needs it)
-            sg[roff + i] = g;
+            const int4 g = __ldg(sorted + rgs + i);
+            sgw[roff + i] = (unsigned)g.x | ((unsigned)(g.y - y0) << 16) | ((unsigned)(g.z - z0) << 24);
           }
         }
         __syncthreads();
       }
-      if (tid == 0) lcs[rows * W] = (unsigned short)sh.carry;
+      if (tid == 0) lcw[rows * W] = (unsigned short)sh.carry;
     }
     // ---- the slice of the view's items ----
     {
@@ -498,11 +528,13 @@ k_brick(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ cell_
 
     // ---- per-lane traversal state ----
     int st = S_NEED;
-    int ax = 0, ay = 0, az = 0, dx = 0, dy = 0, dz = 0;
-    long long r2D2 = 0;
-    float fax = 0.f, fay = 0.f, faz = 0.f, fdx = 0.f, fdy = 0.f, inv_dy = 0.f, inv_dz = 0.f;
+    float ax = 0.f, ay = 0.f, az = 0.f, dx = 0.f, dy = 0.f, dz = 0.f;
+    float oxm = 0.f, oym = 0.f, ozm = 0.f;           // magic-biased origin of v = P - A for the current row
+    float Tlo = 0.f, Thi = 0.f;
     float t0 = 0.f, t1 = 0.f, tl0 = 0.f, tl1 = 0.f;
-    int cz = 0, cz_hi = -1, cy = 1, cy_hi = 0, j = 0, e = 0;
+    float dty = 0.f, tyl = 0.f, tyh = 0.f, dtz = 0.f, tzl = 0.f, tzh = 0.f;
+    float cyf = 0.f;
+    int cz = 0, cz_hi = -1, cy = 1, cy_hi = 0, rowoff = 0, j = 0, e = 0;
     unsigned sidx = 0;
     int count = 0;
     unsigned long long ka = 0, kb = 0;
@@ -523,10 +555,23 @@ k_brick(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ cell_
         const int keep = (3 * nT + 3) >> 2;
         do {
           if (st == S_TEST) {
-            const int4 p = sg[j];
-            if (emu_in_tube(p.x, p.y, p.z, ax, ay, az, dx, dy, dz, r2D2)) {
-              if (kMode == kVote) ++count;
-              else { atomicMax(keyA + p.w, ka); atomicMax(keyB + p.w, kb); }
+            const unsigned g = sg[j];
+            const float vx = __fsub_rn(magic_lo16(g), oxm), vy = __fsub_rn(magic_b2(g), oym), vz = __fsub_rn(magic_b3(g), ozm);
+            const float cx = __fmaf_rn(vy, dz, -__fmul_rn(vz, dy));
+            const float cyy = __fmaf_rn(vz, dx, -__fmul_rn(vx, dz));
+            const float czz = __fmaf_rn(vx, dy, -__fmul_rn(vy, dx));
+            const float s = __fmaf_rn(cx, cx, __fmaf_rn(cyy, cyy, __fmul_rn(czz, czz)));
+            bool in = s <= Tlo;
+            if (s > Tlo && s <= Thi) {                      // inside the error band: the exact predicate
+              const int idx = __float2int_rn(dx), idy = __float2int_rn(dy), idz = __float2int_rn(dz);
+              in = emu_in_tube(__float2int_rn(vx), __float2int_rn(vy), __float2int_rn(vz), 0, 0, 0, idx, idy, idz,
+                               (long long)P.r2 * (long long)(idx * idx + idy * idy + idz * idz));
+            }
+            if (kMode == kVote) count += in ? 1 : 0;
+            else if (in) {
+              // row of the grain -> its sorted position
+              const int pos = j + rdelta[(cz - B.cz0) * H + (cy - B.cy0)];
+              atomicMax(keyA + pos, ka); atomicMax(keyB + pos, kb);
             }
             ++j; ++item_tests;
             if (j >= e) st = S_ROW;
@@ -537,45 +582,39 @@ k_brick(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ cell_
         const int keep = (3 * nR + 3) >> 2;
         do {
           if (st == S_ROW) {
+            // advance to the next row of the layer (cy names the row a TEST phase is working on)
+            ++cy; cyf += 1.0f; rowoff += W; oym -= P.csf[1];
             if (cy > cy_hi) {                               // next z layer of the brick
               ++cz;
               if (cz > cz_hi) {                             // the seed is finished
                 if (kMode == kVote && count) atomicAdd(seed_cnt + sidx, (unsigned)count);
                 st = S_NEED;
               } else {
-                tl0 = t0; tl1 = t1;
-                if (dz != 0) {
-                  const int lo = (cz == 0) ? elo[2] : cz * P.cs[2];
-                  const int hi = (cz == P.n[2] - 1) ? ehi[2] : (cz + 1) * P.cs[2] - 1;
-                  const float a = ((float)lo - R - faz) * inv_dz, bq = ((float)hi + R - faz) * inv_dz;
-                  tl0 = fmaxf(t0, fminf(a, bq)); tl1 = fminf(t1, fmaxf(a, bq));
-                }
+                const float czf = int_f(cz);
+                tl0 = fmaxf(t0, __fmaf_rn(czf, dtz, tzl)); tl1 = fminf(t1, __fmaf_rn(czf, dtz, tzh));
+                cy = 1; cy_hi = 0;
                 if (tl0 <= tl1) {
-                  const float ya = fmaf(tl0, fdy, fay), yb = fmaf(tl1, fdy, fay);
-                  cy = max(B.cy0, emu_clampcell_f(fminf(ya, yb) - R, P.inv_cs[1], P.n[1]));
-                  cy_hi = min(B.cy1, emu_clampcell_f(fmaxf(ya, yb) + R, P.inv_cs[1], P.n[1]));
-                }                                           // else: cy > cy_hi stays, the next step moves on
+                  const float ya = __fmaf_rn(tl0, dy, ay), yb = __fmaf_rn(tl1, dy, ay);
+                  cy = max(B.cy0, rn_int(__fmaf_rn(fminf(ya, yb), P.inv_cs[1], P.klo[1])));
+                  cy_hi = min(B.cy1, rn_int(__fmaf_rn(fmaxf(ya, yb), P.inv_cs[1], P.khi[1])));
+                  cyf = int_f(cy);
+                  rowoff = ((cz - B.cz0) * H + (cy - B.cy0)) * W - B.cx0;
+                  ozm = __fmaf_rn(-czf, P.csf[2], az + kMagicF);
+                  oym = __fmaf_rn(-cyf, P.csf[1], ay + kMagicF);
+                }
               }
             }
             if (st == S_ROW && cy <= cy_hi) {               // row cy of layer cz
-              float tr0 = tl0, tr1 = tl1;
-              if (dy != 0) {
-                const int lo = (cy == 0) ? elo[1] : cy * P.cs[1];
-                const int hi = (cy == P.n[1] - 1) ? ehi[1] : (cy + 1) * P.cs[1] - 1;
-                const float a = ((float)lo - R - fay) * inv_dy, bq = ((float)hi + R - fay) * inv_dy;
-                tr0 = fmaxf(tl0, fminf(a, bq)); tr1 = fminf(tl1, fmaxf(a, bq));
-              }
-              if (tr0 <= tr1) {
-                const float xa = fmaf(tr0, fdx, fax), xb = fmaf(tr1, fdx, fax);
-                const int cx0 = max(B.cx0, emu_clampcell_f(fminf(xa, xb) - R, P.inv_cs[0], P.n[0]));
-                const int cx1 = min(B.cx1, emu_clampcell_f(fmaxf(xa, xb) + R, P.inv_cs[0], P.n[0]));
-                if (cx0 <= cx1) {
-                  const int rl = ((cz - B.cz0) * H + (cy - B.cy0)) * W - B.cx0;
-                  j = lcs[rl + cx0]; e = lcs[rl + cx1 + 1];
+              const float ta = fmaxf(tl0, __fmaf_rn(cyf, dty, tyl)), tb = fminf(tl1, __fmaf_rn(cyf, dty, tyh));
+              if (ta <= tb) {
+                const float xa = __fmaf_rn(ta, dx, ax), xb = __fmaf_rn(tb, dx, ax);
+                const int c0 = max(B.cx0, rn_int(__fmaf_rn(fminf(xa, xb), P.inv_cs[0], P.klo[0])));
+                const int c1 = min(B.cx1, rn_int(__fmaf_rn(fmaxf(xa, xb), P.inv_cs[0], P.khi[0])));
+                if (c0 <= c1) {
+                  j = lcs[rowoff + c0]; e = lcs[rowoff + c1 + 1];
                   if (j < e) st = S_TEST;
                 }
               }
-              ++cy;
             }
           }
         } while (__popc(__ballot_sync(EMU_FULL, st == S_ROW)) >= keep);
@@ -595,34 +634,45 @@ k_brick(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ cell_
           wcur = min(wend, wcur + (unsigned)__popc(mS));
           if (take) {
             const int4 q = __ldg(geo + idx);
-            ax = sbfe(q.x, 0, 19); ay = q.y; az = q.z >> 12;
-            dz = sbfe(q.z, 0, 12); dx = sbfe(q.w, 12, 12); dy = sbfe(q.w, 0, 12);
-            const int d2 = dx * dx + dy * dy + dz * dz;
-            r2D2 = (long long)P.r2 * d2;
+            oxm = magic_lo16((unsigned)q.x);
+            ax = oxm - kMagicF; ay = magic_hi16((unsigned)q.x) - kMagicF; az = magic_lo16((unsigned)q.y) - kMagicF;
+            dx = magic_lo16((unsigned)q.z) - (kMagicF + 2048.0f); dy = magic_hi16((unsigned)q.z) - (kMagicF + 2048.0f);
+            dz = magic_lo16((unsigned)q.w) - (kMagicF + 2048.0f);
+            const float D2 = __fmaf_rn(dx, dx, __fmaf_rn(dy, dy, dz * dz));          // exact: < 2^22
+            {
+              const float T = r2f * D2;
+              const float m_up = P.Rup * (fabsf(dx) + fabsf(dy) + fabsf(dz));
+              const float delta = __fmaf_rn(m_up, 4.76837158203125e-7f, 16.0f);     // 16 + 2^-21 m_up
+              const float band = __fmaf_rn(1.01f * delta, __fmaf_rn(2.0f, m_up, delta), T * 9.5367431640625e-7f);
+              Tlo = T - band; Thi = T + band;
+            }
             sidx = idx; count = 0;
             if (kMode == kAssoc) {
-              const unsigned long long k1 = cand_k1((int)((unsigned)q.x >> 19), d2);
+              const unsigned long long k1 = cand_k1((int)((unsigned)q.y >> 16), __float2int_rn(D2));
               ka = (k1 << kCiBits) | (unsigned long long)(kCiMask - idx);
               kb = (k1 << kCiBits) | (unsigned long long)idx;
             }
-            fax = (float)ax; fay = (float)ay; faz = (float)az; fdx = (float)dx; fdy = (float)dy;
-            const float fdz = (float)dz;
-            const float inv_dx = dx ? 1.0f / fdx : 0.0f;
-            inv_dy = dy ? 1.0f / fdy : 0.0f;
-            inv_dz = dz ? 1.0f / fdz : 0.0f;
+            const float inv_dx = dx != 0.f ? __fdividef(1.0f, dx) : 0.0f;
+            const float inv_dy = dy != 0.f ? __fdividef(1.0f, dy) : 0.0f;
+            const float inv_dz = dz != 0.f ? __fdividef(1.0f, dz) : 0.0f;
             // clip the line against the brick's extent (already widened by R)
-            t0 = -1.0e9f; t1 = 1.0e9f;
+            t0 = -BIG; t1 = BIG;
             bool hit = true;
-            if (dx != 0) { const float a = (blo[0] - fax) * inv_dx, bq = (bhi[0] - fax) * inv_dx; t0 = fmaxf(t0, fminf(a, bq)); t1 = fminf(t1, fmaxf(a, bq)); }
-            else hit = hit && (fax >= blo[0]) && (fax <= bhi[0]);
-            if (dy != 0) { const float a = (blo[1] - fay) * inv_dy, bq = (bhi[1] - fay) * inv_dy; t0 = fmaxf(t0, fminf(a, bq)); t1 = fminf(t1, fmaxf(a, bq)); }
-            else hit = hit && (fay >= blo[1]) && (fay <= bhi[1]);
-            if (dz != 0) { const float a = (blo[2] - faz) * inv_dz, bq = (bhi[2] - faz) * inv_dz; t0 = fmaxf(t0, fminf(a, bq)); t1 = fminf(t1, fmaxf(a, bq)); }
-            else hit = hit && (faz >= blo[2]) && (faz <= bhi[2]);
+            if (dx != 0.f) { const float a = (blo[0] - ax) * inv_dx, bq = (bhi[0] - ax) * inv_dx; t0 = fmaxf(t0, fminf(a, bq)); t1 = fminf(t1, fmaxf(a, bq)); }
+            else hit = hit && (ax >= blo[0]) && (ax <= bhi[0]);
+            if (dy != 0.f) { const float a = (blo[1] - ay) * inv_dy, bq = (bhi[1] - ay) * inv_dy; t0 = fmaxf(t0, fminf(a, bq)); t1 = fminf(t1, fmaxf(a, bq)); }
+            else hit = hit && (ay >= blo[1]) && (ay <= bhi[1]);
+            if (dz != 0.f) { const float a = (blo[2] - az) * inv_dz, bq = (bhi[2] - az) * inv_dz; t0 = fmaxf(t0, fminf(a, bq)); t1 = fminf(t1, fmaxf(a, bq)); }
+            else hit = hit && (az >= blo[2]) && (az <= bhi[2]);
             if (hit && t0 <= t1) {
-              const float za = fmaf(t0, fdz, faz), zb = fmaf(t1, fdz, faz);
-              cz = max(B.cz0, emu_clampcell_f(fminf(za, zb) - R, P.inv_cs[2], P.n[2])) - 1;
-              cz_hi = min(B.cz1, emu_clampcell_f(fmaxf(za, zb) + R, P.inv_cs[2], P.n[2]));
+              // slab k of an axis covers [k cs - R, (k+1) cs - 1 + R]: its t interval is the one of slab 0 moved by k cs / d
+              dty = P.csf[1] * inv_dy; dtz = P.csf[2] * inv_dz;
+              tyl = -BIG; tyh = BIG; tzl = -BIG; tzh = BIG;
+              if (dy != 0.f) { const float a = (-R - ay) * inv_dy, bq = (P.csf[1] - 1.0f + R - ay) * inv_dy; tyl = fminf(a, bq); tyh = fmaxf(a, bq); }
+              if (dz != 0.f) { const float a = (-R - az) * inv_dz, bq = (P.csf[2] - 1.0f + R - az) * inv_dz; tzl = fminf(a, bq); tzh = fmaxf(a, bq); }
+              const float za = __fmaf_rn(t0, dz, az), zb = __fmaf_rn(t1, dz, az);
+              cz = max(B.cz0, rn_int(__fmaf_rn(fminf(za, zb), P.inv_cs[2], P.klo[2]))) - 1;
+              cz_hi = min(B.cz1, rn_int(__fmaf_rn(fmaxf(za, zb), P.inv_cs[2], P.khi[2])));
               cy = 1; cy_hi = 0;                            // forces a layer step first
               st = S_ROW;
             }
@@ -666,11 +716,12 @@ k_cands(EmuDev P, int v0, const FindCtl* __restrict__ ctl, const unsigned* __res
       const unsigned ci = view_cand_off[vl] + base + (unsigned)__popc(m & ((1u << lane) - 1u));
       int4 g = geo[i];
       const int2 p = ab[i];
-      const int dz = sbfe(g.z, 0, 12), dx = sbfe(g.w, 12, 12), dy = sbfe(g.w, 0, 12);
+      int dx, dy, dz;
+      geo_d(g, dx, dy, dz);
       if (n > (unsigned)kMaxTube) status |= EMU_ST_RANGE;
       Cand c; c.a = p.x; c.b = p.y; c.n_tube_view = (int)min(n, 0xffffu) | (vl << 16); c.d2 = dx * dx + dy * dy + dz * dz;
       cands[ci] = c;
-      g.x = (int)(((unsigned)g.x & 0x7ffffu) | (min(n, (unsigned)kMaxTube) << 19));
+      g.y = (int)(((unsigned)g.y & 0xffffu) | (min(n, (unsigned)kMaxTube) << 16));
       cand_geo[ci] = g;
     }
   }
@@ -1115,17 +1166,15 @@ size_t fixed_bytes(const EmuDev& P, const Tiling& T, int64_t n_grains, int32_t n
   return b + 256;
 }
 
-// Tiles per view: enough that an average tile holds about 70 % of kCapG grains and one layer of it fits
-// the cell table; among the factorisations of that count the one whose whole z extent fits the cell
-// table, then the squarest in physical size.
+// Tiles per view: the fewest tiles (every seed is streamed past every brick of its view) for which an
+// average tile - 1.35 x its share of the grains, its rows and its cells over the whole z extent - fits the
+// shared-memory pool; among the factorisations of that count the squarest in physical size.  k_plan cuts
+// a tile that turns out too full into runs of z layers.
 Tiling choose_tiling(const EmuDev& P, int64_t n_grains, int32_t n_views) {
   const double avg = n_views > 0 ? (double)n_grains / n_views : 0.0;
-  int need = (int)ceil(avg / (0.70 * kCapG));
-  if (need < 1) need = 1;
   Tiling fallback; fallback.tx = P.n[0]; fallback.ty = P.n[1]; fallback.w = 1; fallback.h = 1;   // one column per tile
-  bool have_fallback = false;
-  const int64_t max_t = (int64_t)P.n[0] * P.n[1];
-  for (int64_t t = need; t <= emu_min64(max_t, (int64_t)need + 4096); ++t) {
+  const int64_t max_t = emu_min64((int64_t)P.n[0] * P.n[1], 8192);
+  for (int64_t t = 1; t <= max_t; ++t) {
     Tiling best; best.tx = best.ty = best.w = best.h = 0;
     double best_score = -1.0;
     for (int64_t tx = 1; tx <= t; ++tx) {
@@ -1133,14 +1182,13 @@ Tiling choose_tiling(const EmuDev& P, int64_t n_grains, int32_t n_views) {
       const int64_t ty = t / tx;
       if (tx > P.n[0] || ty > P.n[1]) continue;
       const int w = (int)((P.n[0] + tx - 1) / tx), h = (int)((P.n[1] + ty - 1) / ty);
-      if ((int64_t)w * h > kCapC) continue;
+      const double grains = 1.35 * avg * ((double)w * h) / ((double)P.n[0] * P.n[1]) + 64.0;
+      if (brick_bytes((long long)grains, (long long)h * P.n[2], w) > kPoolBytes) continue;
       const double sx = (double)w * P.cs[0], sy = (double)h * P.cs[1];
-      const double score = (sx < sy ? sx / sy : sy / sx) + (((int64_t)w * h * P.n[2] <= kCapC) ? 1.0 : 0.0);
+      const double score = sx < sy ? sx / sy : sy / sx;
       if (score > best_score) { best_score = score; best.tx = (int)tx; best.ty = (int)ty; best.w = w; best.h = h; }
     }
-    if (best_score >= 1.0) return best;                       // every z layer of a tile fits the cell table
-    if (best_score >= 0.0 && !have_fallback) { fallback = best; have_fallback = true; }
-    if (have_fallback && t >= (int64_t)need + 64) break;
+    if (best_score >= 0.0) return best;
   }
   return fallback;
 }
@@ -1263,11 +1311,11 @@ static int vote_chunk(const EmuDev& P, const Tiling& T, FindWs& W, const int4* s
       P, sorted, d_cell_start, d_view_off, v0, v1, W.seed_off, W.view_seed_off, W.ctl, W.geo, W.ab, counts));
   EMU_CK(cudaMemsetAsync(W.seed_cnt, 0, W.seed_cap * sizeof(unsigned), st));
   EMU_LAUNCH(EMU_STAGE_PREP, st, k_plan<<<grid_for(nv, 4, 1 << 20), 128, 0, st>>>(
-      P, T, d_cell_start, v0, v1, W.bricks, (unsigned)W.brick_cap, W.ctl));
+      P, T, d_cell_start, W.bbox, v0, v1, W.bricks, (unsigned)W.brick_cap, W.ctl));
   EMU_LAUNCH(EMU_STAGE_PREP, st, k_plan_finish<<<1, 1, 0, st>>>(W.ctl, (unsigned)W.brick_cap));
-  EMU_CK(cudaFuncSetAttribute(k_brick<kVote>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kBrickSmem));
-  EMU_LAUNCH(EMU_STAGE_VOTE, st, k_brick<kVote><<<kSM, kBrickThreads, kBrickSmem, st>>>(
-      P, sorted, d_cell_start, W.bbox, v0, W.bricks, W.ctl, slices, W.geo, W.view_seed_off, W.seed_cnt, nullptr, nullptr,
+  EMU_CK(cudaFuncSetAttribute(k_brick<kVote>, cudaFuncAttributeMaxDynamicSharedMemorySize, kPoolBytes));
+  EMU_LAUNCH(EMU_STAGE_VOTE, st, k_brick<kVote><<<kSM, kBrickThreads, kPoolBytes, st>>>(
+      P, sorted, d_cell_start, v0, W.bricks, W.ctl, slices, W.geo, W.view_seed_off, W.seed_cnt, nullptr, nullptr,
       counts));
   return EMU_OK;
 }
@@ -1318,9 +1366,9 @@ int emu_find_launch(const EmuDev& P, int seeds_per_grain, int cand_per_grain, co
     EMU_LAUNCH(EMU_STAGE_PREP, st, k_cands_finish<<<1, 1, 0, st>>>(W.ctl, (unsigned)W.cand_cap, counts));
     EMU_LAUNCH(EMU_STAGE_PREP, st, k_reset_cand_arrays<<<kSM * 8, 256, 0, st>>>(W.ctl, W.wins, W.cand_track));
     // A5
-    EMU_CK(cudaFuncSetAttribute(k_brick<kAssoc>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kBrickSmem));
-    EMU_LAUNCH(EMU_STAGE_ASSOC, st, k_brick<kAssoc><<<kSM, kBrickThreads, kBrickSmem, st>>>(
-        P, sorted, d_cell_start, W.bbox, v0, W.bricks, W.ctl, slices, W.cand_geo, W.view_cand_off, nullptr, W.keyA, W.keyB,
+    EMU_CK(cudaFuncSetAttribute(k_brick<kAssoc>, cudaFuncAttributeMaxDynamicSharedMemorySize, kPoolBytes));
+    EMU_LAUNCH(EMU_STAGE_ASSOC, st, k_brick<kAssoc><<<kSM, kBrickThreads, kPoolBytes, st>>>(
+        P, sorted, d_cell_start, v0, W.bricks, W.ctl, slices, W.cand_geo, W.view_cand_off, nullptr, W.keyA, W.keyB,
         counts));
     EMU_LAUNCH(EMU_STAGE_ASSOC, st, k_assoc_generic<0><<<kSM * 16, kVoteThreads, 0, st>>>(
         P, sorted, d_cell_start, W.bbox, v0, W.cands, W.ctl, W.tie_bits, W.keyA, W.keyB, W.owner));

@@ -52,9 +52,16 @@ def test_binning_bit_exact(E, oracle_mod, cfg, cell_um, messy):
     assert np.array_equal(B.sorted.cpu().numpy(), srt)
 
 
+# cells of 4 um and finer in y, z take the shared-memory brick kernels (4-byte grains, float test with the
+# exact fallback); 8 um cells take the generic global-memory kernels.  The result may not depend on it.
+CELLS = [(8.0, 8.0, 8.0), (4.0, 4.0, 4.0), (6.5, 3.0, 2.5)]
+
+
+@pytest.mark.parametrize("cell_um", CELLS)
 @pytest.mark.parametrize("cfg", [0, 1, 2, 3])
-def test_per_seed_counts_bit_exact(E, config_oracle, cfg):
+def test_per_seed_counts_bit_exact(E, config_oracle, cfg, cell_um):
     b, p, ref = config_oracle(cfg)
+    p = dict(p, cell_size_q=default_params(cfg, cell_um=cell_um)["cell_size_q"])
     dump, counts = seed_dump_gpu(E, p, b.grains, b.view_off, ref.counters["seeds"] + 16)
     assert int(counts[E.EMU_CNT["seeds"]]) == ref.counters["seeds"]
     a = dump[np.lexsort((dump[:, 2], dump[:, 1], dump[:, 0]))]
@@ -62,9 +69,11 @@ def test_per_seed_counts_bit_exact(E, config_oracle, cfg):
     assert np.array_equal(a, r)
 
 
+@pytest.mark.parametrize("cell_um", CELLS)
 @pytest.mark.parametrize("cfg", [0, 1, 2, 3])
-def test_track_list_bit_exact(E, config_oracle, cfg):
+def test_track_list_bit_exact(E, config_oracle, cfg, cell_um):
     b, p, ref = config_oracle(cfg)
+    p = dict(p, cell_size_q=default_params(cfg, cell_um=cell_um)["cell_size_q"])
     got = run_gpu(E, p, b.grains, b.view_off)
     assert_same_tracks(E, got, ref)
     assert len(got["tracks"]) > 0
