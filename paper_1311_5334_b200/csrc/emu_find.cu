@@ -406,7 +406,20 @@ __global__ void k_plan_finish(FindCtl* ctl, unsigned brick_cap) {
 // integer predicate (emu_in_tube) decides.  The result is therefore the exact one in every case
 // (DESIGN.md section 6 has the derivation).
 enum { kVote = 0, kAssoc = 1 };
-enum { S_NEED = 0, S_ROW = 1, S_TEST = 2 };
+enum { S_NEED = 0, S_ROW = 1 };
+constexpr int kRefill = 8;                        // idle lanes of a warp that trigger a refill from the seed stream
+constexpr int kRefillStop = 4;                    // the refill goes on while at least this many lanes are still idle
+
+__device__ __forceinline__ unsigned lds_u32(unsigned addr) {
+  unsigned v;
+  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr));
+  return v;
+}
+__device__ __forceinline__ unsigned lds_u16(unsigned addr) {
+  unsigned short v;
+  asm volatile("ld.shared.u16 %0, [%1];" : "=h"(v) : "r"(addr));
+  return (unsigned)v;
+}
 
 struct BrickShared {
   int row_gs[kBrickThreads];
@@ -527,100 +540,28 @@ k_brick(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ cell_
     const unsigned s_end = sh.end;
 
     // ---- per-lane traversal state ----
-    int st = S_NEED;
+    int st = S_NEED;                                 // S_NEED: no seed; S_ROW: walking a seed (j < e: a run is pending)
     float ax = 0.f, ay = 0.f, az = 0.f, dx = 0.f, dy = 0.f, dz = 0.f;
     float oxm = 0.f, oym = 0.f, ozm = 0.f;           // magic-biased origin of v = P - A for the current row
     float Tlo = 0.f, Thi = 0.f;
     float t0 = 0.f, t1 = 0.f, tl0 = 0.f, tl1 = 0.f;
     float dty = 0.f, tyl = 0.f, tyh = 0.f, dtz = 0.f, tzl = 0.f, tzh = 0.f;
     float cyf = 0.f;
-    int cz = 0, cz_hi = -1, cy = 1, cy_hi = 0, rowoff = 0, j = 0, e = 0;
+    int cz = 0, cz_hi = -1, cy = 1, cy_hi = 0, rowoff = 0;
+    unsigned j = 0, e = 0;                           // shared-memory byte addresses of the pending run of grains
     unsigned sidx = 0;
     int count = 0;
     unsigned long long ka = 0, kb = 0;
     unsigned wcur = 0, wend = 0;
     bool exhausted = false;
+    const unsigned sg_a = (unsigned)__cvta_generic_to_shared(sg);
+    const unsigned lcs_a = (unsigned)__cvta_generic_to_shared(lcs);
 
     unsigned item_tests = 0;
     for (;;) {
+      // ---------------- SEED: refill the idle lanes once enough of them wait ----------------
       unsigned mS = __ballot_sync(EMU_FULL, st == S_NEED);
-      const unsigned mR = __ballot_sync(EMU_FULL, st == S_ROW);
-      const unsigned mT = __ballot_sync(EMU_FULL, st == S_TEST);
-      if (exhausted) mS = 0;
-      if (!(mS | mR | mT)) break;
-      const int nS = __popc(mS), nR = __popc(mR), nT = __popc(mT);
-      // the phase most lanes wait for; it is repeated while at least 3/4 of them still want it
-      if (nT >= nR && nT >= nS) {
-        // ---------------- TEST ----------------
-        const int keep = (3 * nT + 3) >> 2;
-        do {
-          if (st == S_TEST) {
-            const unsigned g = sg[j];
-            const float vx = __fsub_rn(magic_lo16(g), oxm), vy = __fsub_rn(magic_b2(g), oym), vz = __fsub_rn(magic_b3(g), ozm);
-            const float cx = __fmaf_rn(vy, dz, -__fmul_rn(vz, dy));
-            const float cyy = __fmaf_rn(vz, dx, -__fmul_rn(vx, dz));
-            const float czz = __fmaf_rn(vx, dy, -__fmul_rn(vy, dx));
-            const float s = __fmaf_rn(cx, cx, __fmaf_rn(cyy, cyy, __fmul_rn(czz, czz)));
-            bool in = s <= Tlo;
-            if (s > Tlo && s <= Thi) {                      // inside the error band: the exact predicate
-              const int idx = __float2int_rn(dx), idy = __float2int_rn(dy), idz = __float2int_rn(dz);
-              in = emu_in_tube(__float2int_rn(vx), __float2int_rn(vy), __float2int_rn(vz), 0, 0, 0, idx, idy, idz,
-                               (long long)P.r2 * (long long)(idx * idx + idy * idy + idz * idz));
-            }
-            if (kMode == kVote) count += in ? 1 : 0;
-            else if (in) {
-              // row of the grain -> its sorted position
-              const int pos = j + rdelta[(cz - B.cz0) * H + (cy - B.cy0)];
-              atomicMax(keyA + pos, ka); atomicMax(keyB + pos, kb);
-            }
-            ++j; ++item_tests;
-            if (j >= e) st = S_ROW;
-          }
-        } while (__popc(__ballot_sync(EMU_FULL, st == S_TEST)) >= keep);
-      } else if (nR >= nS) {
-        // ---------------- ROW ----------------
-        const int keep = (3 * nR + 3) >> 2;
-        do {
-          if (st == S_ROW) {
-            // advance to the next row of the layer (cy names the row a TEST phase is working on)
-            ++cy; cyf += 1.0f; rowoff += W; oym -= P.csf[1];
-            if (cy > cy_hi) {                               // next z layer of the brick
-              ++cz;
-              if (cz > cz_hi) {                             // the seed is finished
-                if (kMode == kVote && count) atomicAdd(seed_cnt + sidx, (unsigned)count);
-                st = S_NEED;
-              } else {
-                const float czf = int_f(cz);
-                tl0 = fmaxf(t0, __fmaf_rn(czf, dtz, tzl)); tl1 = fminf(t1, __fmaf_rn(czf, dtz, tzh));
-                cy = 1; cy_hi = 0;
-                if (tl0 <= tl1) {
-                  const float ya = __fmaf_rn(tl0, dy, ay), yb = __fmaf_rn(tl1, dy, ay);
-                  cy = max(B.cy0, rn_int(__fmaf_rn(fminf(ya, yb), P.inv_cs[1], P.klo[1])));
-                  cy_hi = min(B.cy1, rn_int(__fmaf_rn(fmaxf(ya, yb), P.inv_cs[1], P.khi[1])));
-                  cyf = int_f(cy);
-                  rowoff = ((cz - B.cz0) * H + (cy - B.cy0)) * W - B.cx0;
-                  ozm = __fmaf_rn(-czf, P.csf[2], az + kMagicF);
-                  oym = __fmaf_rn(-cyf, P.csf[1], ay + kMagicF);
-                }
-              }
-            }
-            if (st == S_ROW && cy <= cy_hi) {               // row cy of layer cz
-              const float ta = fmaxf(tl0, __fmaf_rn(cyf, dty, tyl)), tb = fminf(tl1, __fmaf_rn(cyf, dty, tyh));
-              if (ta <= tb) {
-                const float xa = __fmaf_rn(ta, dx, ax), xb = __fmaf_rn(tb, dx, ax);
-                const int c0 = max(B.cx0, rn_int(__fmaf_rn(fminf(xa, xb), P.inv_cs[0], P.klo[0])));
-                const int c1 = min(B.cx1, rn_int(__fmaf_rn(fmaxf(xa, xb), P.inv_cs[0], P.khi[0])));
-                if (c0 <= c1) {
-                  j = lcs[rowoff + c0]; e = lcs[rowoff + c1 + 1];
-                  if (j < e) st = S_TEST;
-                }
-              }
-            }
-          }
-        } while (__popc(__ballot_sync(EMU_FULL, st == S_ROW)) >= keep);
-      } else {
-        // ---------------- SEED ----------------
-        const int keep = (3 * nS + 3) >> 2;
+      if (!exhausted && __popc(mS) >= kRefill) {
         for (;;) {
           if (wcur == wend) {
             unsigned base = 0;
@@ -674,12 +615,75 @@ k_brick(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ cell_
               cz = max(B.cz0, rn_int(__fmaf_rn(fminf(za, zb), P.inv_cs[2], P.klo[2]))) - 1;
               cz_hi = min(B.cz1, rn_int(__fmaf_rn(fmaxf(za, zb), P.inv_cs[2], P.khi[2])));
               cy = 1; cy_hi = 0;                            // forces a layer step first
+              j = 0; e = 0;
               st = S_ROW;
             }
           }
           mS = __ballot_sync(EMU_FULL, st == S_NEED);
-          if (__popc(mS) < keep) break;
+          if (__popc(mS) < kRefillStop) break;
         }
+      } else if (mS == EMU_FULL) {
+        break;                                              // the slice is exhausted and every lane is done
+      }
+
+      // ---------------- ROW: lanes whose run is used up move to the next row of cells ----------------
+      if (st == S_ROW && j >= e) {
+        ++cy; cyf += 1.0f; rowoff += W; oym -= P.csf[1];
+        if (cy > cy_hi) {                                   // next z layer of the brick
+          ++cz;
+          if (cz > cz_hi) {                                 // the seed is finished
+            if (kMode == kVote && count) atomicAdd(seed_cnt + sidx, (unsigned)count);
+            st = S_NEED;
+          } else {
+            const float czf = int_f(cz);
+            tl0 = fmaxf(t0, __fmaf_rn(czf, dtz, tzl)); tl1 = fminf(t1, __fmaf_rn(czf, dtz, tzh));
+            cy = 1; cy_hi = 0;
+            if (tl0 <= tl1) {
+              const float ya = __fmaf_rn(tl0, dy, ay), yb = __fmaf_rn(tl1, dy, ay);
+              cy = max(B.cy0, rn_int(__fmaf_rn(fminf(ya, yb), P.inv_cs[1], P.klo[1])));
+              cy_hi = min(B.cy1, rn_int(__fmaf_rn(fmaxf(ya, yb), P.inv_cs[1], P.khi[1])));
+              cyf = int_f(cy);
+              rowoff = ((cz - B.cz0) * H + (cy - B.cy0)) * W - B.cx0;
+              ozm = __fmaf_rn(-czf, P.csf[2], az + kMagicF);
+              oym = __fmaf_rn(-cyf, P.csf[1], ay + kMagicF);
+            }
+          }
+        }
+        if (st == S_ROW && cy <= cy_hi) {                   // row cy of layer cz
+          const float ta = fmaxf(tl0, __fmaf_rn(cyf, dty, tyl)), tb = fminf(tl1, __fmaf_rn(cyf, dty, tyh));
+          if (ta <= tb) {
+            const float xa = __fmaf_rn(ta, dx, ax), xb = __fmaf_rn(tb, dx, ax);
+            const int c0 = max(B.cx0, rn_int(__fmaf_rn(fminf(xa, xb), P.inv_cs[0], P.klo[0])));
+            const int c1 = min(B.cx1, rn_int(__fmaf_rn(fmaxf(xa, xb), P.inv_cs[0], P.khi[0])));
+            if (c0 <= c1) {
+              j = sg_a + 4u * lds_u16(lcs_a + 2u * (unsigned)(rowoff + c0));
+              e = sg_a + 4u * lds_u16(lcs_a + 2u * (unsigned)(rowoff + c1 + 1));
+            }
+          }
+        }
+      }
+
+      // ---------------- TEST: one grain of the pending run ----------------
+      if (j < e) {
+        const unsigned g = lds_u32(j);
+        const float vx = __fsub_rn(magic_lo16(g), oxm), vy = __fsub_rn(magic_b2(g), oym), vz = __fsub_rn(magic_b3(g), ozm);
+        const float cx = __fmaf_rn(vy, dz, -__fmul_rn(vz, dy));
+        const float cyy = __fmaf_rn(vz, dx, -__fmul_rn(vx, dz));
+        const float czz = __fmaf_rn(vx, dy, -__fmul_rn(vy, dx));
+        const float s = __fmaf_rn(cx, cx, __fmaf_rn(cyy, cyy, __fmul_rn(czz, czz)));
+        bool in = s <= Tlo;
+        if (s > Tlo && s <= Thi) {                          // inside the error band: the exact predicate
+          const int idx = __float2int_rn(dx), idy = __float2int_rn(dy), idz = __float2int_rn(dz);
+          in = emu_in_tube(__float2int_rn(vx), __float2int_rn(vy), __float2int_rn(vz), 0, 0, 0, idx, idy, idz,
+                           (long long)P.r2 * (long long)(idx * idx + idy * idy + idz * idz));
+        }
+        if (kMode == kVote) count += in ? 1 : 0;
+        else if (in) {
+          // slot of the grain in the brick + first sorted position of its row - first slot of its row
+          const int pos = (int)((j - sg_a) >> 2) + rdelta[(cz - B.cz0) * H + (cy - B.cy0)];
+          atomicMax(keyA + pos, ka); atomicMax(keyB + pos, kb);
+        }
+        j += 4u; ++item_tests;
       }
     }
     n_tests += item_tests;
