@@ -37,10 +37,12 @@ constexpr int kPoolBytes = 222 * 1024;            // dynamic shared memory of a 
 constexpr int kGrab = 128;                        // seeds a warp takes from the block's stream at a time
 constexpr int kTieBits = 1 << 16;                 // bitmap of tied priorities
 
-// shared-memory bytes of a brick with n grains in `rows` rows of cells, each w cells wide:
-// 4 B per grain, 4 B per row (sorted position of the row's first grain), 2 B per cell (+ the end mark)
+// shared-memory layout of a brick: n grains of 4 B, then one table row per row of cells: the brick slot
+// of the first grain of each of its w cells, the end of the row, and (last two entries, as one 32-bit
+// word) the sorted position of the row's first grain minus its slot.  Row stride in 16-bit entries:
+__host__ __device__ inline int brick_row_stride(int w) { return (w + 4) & ~1; }
 __host__ __device__ inline long long brick_bytes(long long n, long long rows, long long w) {
-  return 4 * n + 4 * rows + 2 * (rows * w + 2);
+  return 4 * n + 2 * rows * (long long)brick_row_stride((int)w);
 }
 
 struct Cand {            // 16 B
@@ -123,6 +125,10 @@ __device__ __forceinline__ float magic_b3(unsigned w) { return __uint_as_float(_
 // round-to-nearest float -> int and small int -> float through the 1.5 * 2^23 trick (|value| < 2^22)
 __device__ __forceinline__ int rn_int(float y) { return __float_as_int(__fadd_rn(y, 12582912.0f)) - 0x4B400000; }
 __device__ __forceinline__ float int_f(int i) { return __fadd_rn(__int_as_float(i + 0x4B400000), -12582912.0f); }
+// round a float to the nearest integer, staying in float (|value| < 2^22)
+__device__ __forceinline__ float rn_flt(float y) { return __fadd_rn(__fadd_rn(y, 12582912.0f), -12582912.0f); }
+// a float that holds a small non-negative integer -> that integer
+__device__ __forceinline__ int __float2int_rn_magic(float y) { return __float_as_int(__fadd_rn(y, 12582912.0f)) - 0x4B400000; }
 
 // ---------------------------------------------------------------------------------------------
 // per-view bounding boxes
@@ -406,7 +412,6 @@ __global__ void k_plan_finish(FindCtl* ctl, unsigned brick_cap) {
 // integer predicate (emu_in_tube) decides.  The result is therefore the exact one in every case
 // (DESIGN.md section 6 has the derivation).
 enum { kVote = 0, kAssoc = 1 };
-enum { S_NEED = 0, S_ROW = 1 };
 constexpr int kRefill = 8;                        // idle lanes of a warp that trigger a refill from the seed stream
 constexpr int kRefillStop = 4;                    // the refill goes on while at least this many lanes are still idle
 
@@ -445,15 +450,14 @@ k_brick(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ cell_
   const float R = P.Rw;
   const float r2f = (float)P.r2;
   const float BIG = 1.0e9f;
+  unsigned pool_a;                                  // shared-window address of the pool (volatile: computed once)
+  asm volatile("mov.u32 %0, %1;" : "=r"(pool_a) : "r"((unsigned)__cvta_generic_to_shared(pool)));
   unsigned long long n_tests = 0;
   int cur_brick = -1;
   Brick B;
   B.view = 0; B.cx0 = B.cx1 = B.cy0 = B.cy1 = B.cz0 = B.cz1 = B.n = 0;
-  int W = 1, H = 1;
+  int W = 1, H = 1, S = 4;
   float blo[3] = {0.f, 0.f, 0.f}, bhi[3] = {0.f, 0.f, 0.f};   // brick extent widened by R
-  const unsigned* sg = reinterpret_cast<const unsigned*>(pool);
-  const int* rdelta = reinterpret_cast<const int*>(pool);
-  const unsigned short* lcs = reinterpret_cast<const unsigned short*>(pool);
 
   for (;;) {
     __syncthreads();                                  // everyone is done with the previous item
@@ -467,13 +471,11 @@ k_brick(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ cell_
       // ---- stage brick b ----
       cur_brick = b;
       B = bricks[b];
-      W = B.cx1 - B.cx0 + 1; H = B.cy1 - B.cy0 + 1;
+      W = B.cx1 - B.cx0 + 1; H = B.cy1 - B.cy0 + 1; S = brick_row_stride(W);
       const int rows = H * (B.cz1 - B.cz0 + 1);
       const int vbase = B.view * P.ncell;
       unsigned* sgw = reinterpret_cast<unsigned*>(pool);
-      int* rdw = reinterpret_cast<int*>(pool + 4 * (size_t)B.n);
-      unsigned short* lcw = reinterpret_cast<unsigned short*>(pool + 4 * (size_t)B.n + 4 * (size_t)rows);
-      sg = sgw; rdelta = rdw; lcs = lcw;
+      unsigned short* tab = reinterpret_cast<unsigned short*>(pool + 4 * (size_t)B.n);
       {
         const int c0[3] = {B.cx0, B.cy0, B.cz0}, c1[3] = {B.cx1, B.cy1, B.cz1};
 #pragma unroll
@@ -505,18 +507,18 @@ k_brick(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ cell_
         }
         __syncthreads();
         const int carry = sh.carry;
-        const int off = carry + (int)sh.warp_sum[wid] + incl - len;     // first slot of row r in the brick
+        const int off = carry + (int)sh.warp_sum[wid] + incl - len;     // slot of the first grain of row r
         sh.row_gs[tid] = gs;
-        if (r < rows) rdw[r] = gs - off;
+        if (r < rows) *reinterpret_cast<int*>(tab + (size_t)r * S + (S - 2)) = gs - off;
         __syncthreads();
         if (tid == kBrickThreads - 1) sh.carry = off + len;
         const int nr = min(kBrickThreads, rows - r0);
         for (int k = wid; k < nr; k += kBrickThreads / 32) {
           const int rr = r0 + k;
-          const int rgs = sh.row_gs[k], roff = rgs - rdw[rr];
+          const int rgs = sh.row_gs[k], roff = rgs - *reinterpret_cast<const int*>(tab + (size_t)rr * S + (S - 2));
           const int cz = B.cz0 + rr / H, cy = B.cy0 + rr % H;
           const int rb = vbase + (cz * P.n[1] + cy) * P.n[0] + B.cx0;
-          for (int i = lane; i < W; i += 32) lcw[rr * W + i] = (unsigned short)(roff + (__ldg(cell_start + rb + i) - rgs));
+          for (int i = lane; i <= W; i += 32) tab[(size_t)rr * S + i] = (unsigned short)(roff + (__ldg(cell_start + rb + i) - rgs));
           const int rlen = __ldg(cell_start + rb + W) - rgs;
           const int y0 = cy * P.cs[1], z0 = cz * P.cs[2];
           for (int i = lane; i < rlen; i += 32) {
@@ -526,7 +528,6 @@ k_brick(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ cell_
         }
         __syncthreads();
       }
-      if (tid == 0) lcw[rows * W] = (unsigned short)sh.carry;
     }
     // ---- the slice of the view's items ----
     {
@@ -538,29 +539,55 @@ k_brick(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ cell_
     }
     __syncthreads();
     const unsigned s_end = sh.end;
+    // table address of row (cy = 0, cz = cz0 - 1) of the brick's numbering moved back by cx0 cells, so that
+    // cell cx of row cy of the current layer sits at layp + cy * row_b + 2 cx
+    const unsigned row_b = 2u * (unsigned)S, lay_b = row_b * (unsigned)H;   // table bytes per row / per z layer
+    const unsigned tab0 = pool_a + 4u * (unsigned)B.n - 2u * (unsigned)B.cx0 - (unsigned)B.cy0 * row_b - lay_b;
+    const unsigned delta_o = 2u * (unsigned)(B.cx0 + S - 2);               // from a row address to its position word
+    const float cz0f = (float)B.cz0, cz1f = (float)B.cz1, cy1f = (float)B.cy1;
 
-    // ---- per-lane traversal state ----
-    int st = S_NEED;                                 // S_NEED: no seed; S_ROW: walking a seed (j < e: a run is pending)
-    float ax = 0.f, ay = 0.f, az = 0.f, dx = 0.f, dy = 0.f, dz = 0.f;
+    // ---- per-lane state: one seed per lane ----
+    bool idle = true;                                // no seed (waiting for the next refill)
+    float ax = 0.f, ay = 0.f, dx = 0.f, dy = 0.f, dz = 0.f;
     float oxm = 0.f, oym = 0.f, ozm = 0.f;           // magic-biased origin of v = P - A for the current row
     float Tlo = 0.f, Thi = 0.f;
     float t0 = 0.f, t1 = 0.f, tl0 = 0.f, tl1 = 0.f;
     float dty = 0.f, tyl = 0.f, tyh = 0.f, dtz = 0.f, tzl = 0.f, tzh = 0.f;
-    float cyf = 0.f;
-    int cz = 0, cz_hi = -1, cy = 1, cy_hi = 0, rowoff = 0;
-    unsigned j = 0, e = 0;                           // shared-memory byte addresses of the pending run of grains
+    float cyf = 1.f, cyhf = 0.f, czf = 0.f, czhf = -1.f;   // current / last row of the layer, current / last layer
+    unsigned rowp = 0, layp = 0;                     // table address of the current row / of row 0 of the current layer
+    unsigned j = 0, e = 0;                           // shared-memory addresses of the pending run of grains
     unsigned sidx = 0;
     int count = 0;
     unsigned long long ka = 0, kb = 0;
     unsigned wcur = 0, wend = 0;
     bool exhausted = false;
-    const unsigned sg_a = (unsigned)__cvta_generic_to_shared(sg);
-    const unsigned lcs_a = (unsigned)__cvta_generic_to_shared(lcs);
-
     unsigned item_tests = 0;
+
+    // one point-line test of the grain at shared address `ga` (see the header comment for the error band)
+    auto test_grain = [&](unsigned ga) {
+      const unsigned g = lds_u32(ga);
+      const float vx = __fsub_rn(magic_lo16(g), oxm), vy = __fsub_rn(magic_b2(g), oym), vz = __fsub_rn(magic_b3(g), ozm);
+      const float cx = __fmaf_rn(vy, dz, -__fmul_rn(vz, dy));
+      const float cyy = __fmaf_rn(vz, dx, -__fmul_rn(vx, dz));
+      const float czz = __fmaf_rn(vx, dy, -__fmul_rn(vy, dx));
+      const float s = __fmaf_rn(cx, cx, __fmaf_rn(cyy, cyy, __fmul_rn(czz, czz)));
+      bool in = s <= Tlo;
+      if (s > Tlo && s <= Thi) {                            // inside the error band: the exact predicate
+        const int idx = __float2int_rn(dx), idy = __float2int_rn(dy), idz = __float2int_rn(dz);
+        in = emu_in_tube(__float2int_rn(vx), __float2int_rn(vy), __float2int_rn(vz), 0, 0, 0, idx, idy, idz,
+                         (long long)P.r2 * (long long)(idx * idx + idy * idy + idz * idz));
+      }
+      if (kMode == kVote) { if (in) ++count; }
+      else if (in) {
+        // slot of the grain in the brick + (sorted position - slot) of the first grain of its row
+        const int pos = (int)((ga - pool_a) >> 2) + (int)lds_u32(rowp + delta_o);
+        atomicMax(keyA + pos, ka); atomicMax(keyB + pos, kb);
+      }
+    };
+
     for (;;) {
       // ---------------- SEED: refill the idle lanes once enough of them wait ----------------
-      unsigned mS = __ballot_sync(EMU_FULL, st == S_NEED);
+      unsigned mS = __ballot_sync(EMU_FULL, idle);
       if (!exhausted && __popc(mS) >= kRefill) {
         for (;;) {
           if (wcur == wend) {
@@ -571,28 +598,15 @@ k_brick(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ cell_
             wcur = base; wend = min(base + (unsigned)kGrab, s_end);
           }
           const unsigned idx = wcur + (unsigned)__popc(mS & ((1u << lane) - 1u));
-          const bool take = (st == S_NEED) && (idx < wend);
+          const bool take = idle && (idx < wend);
           wcur = min(wend, wcur + (unsigned)__popc(mS));
           if (take) {
             const int4 q = __ldg(geo + idx);
             oxm = magic_lo16((unsigned)q.x);
-            ax = oxm - kMagicF; ay = magic_hi16((unsigned)q.x) - kMagicF; az = magic_lo16((unsigned)q.y) - kMagicF;
+            ax = oxm - kMagicF; ay = magic_hi16((unsigned)q.x) - kMagicF;
+            const float az = magic_lo16((unsigned)q.y) - kMagicF;
             dx = magic_lo16((unsigned)q.z) - (kMagicF + 2048.0f); dy = magic_hi16((unsigned)q.z) - (kMagicF + 2048.0f);
             dz = magic_lo16((unsigned)q.w) - (kMagicF + 2048.0f);
-            const float D2 = __fmaf_rn(dx, dx, __fmaf_rn(dy, dy, dz * dz));          // exact: < 2^22
-            {
-              const float T = r2f * D2;
-              const float m_up = P.Rup * (fabsf(dx) + fabsf(dy) + fabsf(dz));
-              const float delta = __fmaf_rn(m_up, 4.76837158203125e-7f, 16.0f);     // 16 + 2^-21 m_up
-              const float band = __fmaf_rn(1.01f * delta, __fmaf_rn(2.0f, m_up, delta), T * 9.5367431640625e-7f);
-              Tlo = T - band; Thi = T + band;
-            }
-            sidx = idx; count = 0;
-            if (kMode == kAssoc) {
-              const unsigned long long k1 = cand_k1((int)((unsigned)q.y >> 16), __float2int_rn(D2));
-              ka = (k1 << kCiBits) | (unsigned long long)(kCiMask - idx);
-              kb = (k1 << kCiBits) | (unsigned long long)idx;
-            }
             const float inv_dx = dx != 0.f ? __fdividef(1.0f, dx) : 0.0f;
             const float inv_dy = dy != 0.f ? __fdividef(1.0f, dy) : 0.0f;
             const float inv_dz = dz != 0.f ? __fdividef(1.0f, dz) : 0.0f;
@@ -606,20 +620,37 @@ k_brick(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ cell_
             if (dz != 0.f) { const float a = (blo[2] - az) * inv_dz, bq = (bhi[2] - az) * inv_dz; t0 = fmaxf(t0, fminf(a, bq)); t1 = fminf(t1, fmaxf(a, bq)); }
             else hit = hit && (az >= blo[2]) && (az <= bhi[2]);
             if (hit && t0 <= t1) {
+              const float D2 = __fmaf_rn(dx, dx, __fmaf_rn(dy, dy, dz * dz));        // exact: < 2^22
+              {
+                const float T = r2f * D2;
+                const float m_up = P.Rup * (fabsf(dx) + fabsf(dy) + fabsf(dz));
+                const float delta = __fmaf_rn(m_up, 4.76837158203125e-7f, 16.0f);   // 16 + 2^-21 m_up
+                const float band = __fmaf_rn(1.01f * delta, __fmaf_rn(2.0f, m_up, delta), T * 9.5367431640625e-7f);
+                Tlo = T - band; Thi = T + band;
+              }
+              sidx = idx; count = 0;
+              if (kMode == kAssoc) {
+                const unsigned long long k1 = cand_k1((int)((unsigned)q.y >> 16), __float2int_rn(D2));
+                ka = (k1 << kCiBits) | (unsigned long long)(kCiMask - idx);
+                kb = (k1 << kCiBits) | (unsigned long long)idx;
+              }
               // slab k of an axis covers [k cs - R, (k+1) cs - 1 + R]: its t interval is the one of slab 0 moved by k cs / d
               dty = P.csf[1] * inv_dy; dtz = P.csf[2] * inv_dz;
               tyl = -BIG; tyh = BIG; tzl = -BIG; tzh = BIG;
               if (dy != 0.f) { const float a = (-R - ay) * inv_dy, bq = (P.csf[1] - 1.0f + R - ay) * inv_dy; tyl = fminf(a, bq); tyh = fmaxf(a, bq); }
               if (dz != 0.f) { const float a = (-R - az) * inv_dz, bq = (P.csf[2] - 1.0f + R - az) * inv_dz; tzl = fminf(a, bq); tzh = fmaxf(a, bq); }
               const float za = __fmaf_rn(t0, dz, az), zb = __fmaf_rn(t1, dz, az);
-              cz = max(B.cz0, rn_int(__fmaf_rn(fminf(za, zb), P.inv_cs[2], P.klo[2]))) - 1;
-              cz_hi = min(B.cz1, rn_int(__fmaf_rn(fmaxf(za, zb), P.inv_cs[2], P.khi[2])));
-              cy = 1; cy_hi = 0;                            // forces a layer step first
+              const int czi = max(B.cz0, rn_int(__fmaf_rn(fminf(za, zb), P.inv_cs[2], P.klo[2]))) - 1;   // the layer before the first
+              czf = int_f(czi);
+              czhf = fminf(cz1f, rn_flt(__fmaf_rn(fmaxf(za, zb), P.inv_cs[2], P.khi[2])));
+              ozm = __fmaf_rn(-czf, P.csf[2], az + kMagicF);
+              layp = tab0 + (unsigned)(czi - B.cz0 + 1) * lay_b;
+              cyf = 1.f; cyhf = 0.f;                        // forces a layer step first
               j = 0; e = 0;
-              st = S_ROW;
+              idle = false;
             }
           }
-          mS = __ballot_sync(EMU_FULL, st == S_NEED);
+          mS = __ballot_sync(EMU_FULL, idle);
           if (__popc(mS) < kRefillStop) break;
         }
       } else if (mS == EMU_FULL) {
@@ -627,66 +658,49 @@ k_brick(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ cell_
       }
 
       // ---------------- ROW: lanes whose run is used up move to the next row of cells ----------------
-      if (st == S_ROW && j >= e) {
-        ++cy; cyf += 1.0f; rowoff += W; oym -= P.csf[1];
-        if (cy > cy_hi) {                                   // next z layer of the brick
-          ++cz;
-          if (cz > cz_hi) {                                 // the seed is finished
+      if (!idle && j >= e) {
+        cyf += 1.0f; rowp += row_b; oym -= P.csf[1];
+        if (cyf > cyhf) {                                   // next z layer of the brick
+          czf += 1.0f; ozm -= P.csf[2]; layp += lay_b;
+          if (czf > czhf) {                                 // the seed is finished
             if (kMode == kVote && count) atomicAdd(seed_cnt + sidx, (unsigned)count);
-            st = S_NEED;
+            idle = true;
           } else {
-            const float czf = int_f(cz);
             tl0 = fmaxf(t0, __fmaf_rn(czf, dtz, tzl)); tl1 = fminf(t1, __fmaf_rn(czf, dtz, tzh));
-            cy = 1; cy_hi = 0;
+            cyf = 1.f; cyhf = 0.f;
             if (tl0 <= tl1) {
               const float ya = __fmaf_rn(tl0, dy, ay), yb = __fmaf_rn(tl1, dy, ay);
-              cy = max(B.cy0, rn_int(__fmaf_rn(fminf(ya, yb), P.inv_cs[1], P.klo[1])));
-              cy_hi = min(B.cy1, rn_int(__fmaf_rn(fmaxf(ya, yb), P.inv_cs[1], P.khi[1])));
-              cyf = int_f(cy);
-              rowoff = ((cz - B.cz0) * H + (cy - B.cy0)) * W - B.cx0;
-              ozm = __fmaf_rn(-czf, P.csf[2], az + kMagicF);
+              const int cyi = max(B.cy0, rn_int(__fmaf_rn(fminf(ya, yb), P.inv_cs[1], P.klo[1])));
+              cyhf = fminf(cy1f, rn_flt(__fmaf_rn(fmaxf(ya, yb), P.inv_cs[1], P.khi[1])));
+              cyf = int_f(cyi);
+              rowp = layp + (unsigned)cyi * row_b;
               oym = __fmaf_rn(-cyf, P.csf[1], ay + kMagicF);
             }
           }
         }
-        if (st == S_ROW && cy <= cy_hi) {                   // row cy of layer cz
+        if (!idle && cyf <= cyhf) {                         // row cyf of layer czf
           const float ta = fmaxf(tl0, __fmaf_rn(cyf, dty, tyl)), tb = fminf(tl1, __fmaf_rn(cyf, dty, tyh));
           if (ta <= tb) {
             const float xa = __fmaf_rn(ta, dx, ax), xb = __fmaf_rn(tb, dx, ax);
             const int c0 = max(B.cx0, rn_int(__fmaf_rn(fminf(xa, xb), P.inv_cs[0], P.klo[0])));
             const int c1 = min(B.cx1, rn_int(__fmaf_rn(fmaxf(xa, xb), P.inv_cs[0], P.khi[0])));
             if (c0 <= c1) {
-              j = sg_a + 4u * lds_u16(lcs_a + 2u * (unsigned)(rowoff + c0));
-              e = sg_a + 4u * lds_u16(lcs_a + 2u * (unsigned)(rowoff + c1 + 1));
+              j = pool_a + 4u * lds_u16(rowp + 2u * (unsigned)c0);
+              e = pool_a + 4u * lds_u16(rowp + 2u * (unsigned)c1 + 2u);
+              item_tests += e - j;
             }
           }
         }
       }
 
-      // ---------------- TEST: one grain of the pending run ----------------
+      // ---------------- TEST: up to two grains of the pending run ----------------
       if (j < e) {
-        const unsigned g = lds_u32(j);
-        const float vx = __fsub_rn(magic_lo16(g), oxm), vy = __fsub_rn(magic_b2(g), oym), vz = __fsub_rn(magic_b3(g), ozm);
-        const float cx = __fmaf_rn(vy, dz, -__fmul_rn(vz, dy));
-        const float cyy = __fmaf_rn(vz, dx, -__fmul_rn(vx, dz));
-        const float czz = __fmaf_rn(vx, dy, -__fmul_rn(vy, dx));
-        const float s = __fmaf_rn(cx, cx, __fmaf_rn(cyy, cyy, __fmul_rn(czz, czz)));
-        bool in = s <= Tlo;
-        if (s > Tlo && s <= Thi) {                          // inside the error band: the exact predicate
-          const int idx = __float2int_rn(dx), idy = __float2int_rn(dy), idz = __float2int_rn(dz);
-          in = emu_in_tube(__float2int_rn(vx), __float2int_rn(vy), __float2int_rn(vz), 0, 0, 0, idx, idy, idz,
-                           (long long)P.r2 * (long long)(idx * idx + idy * idy + idz * idz));
-        }
-        if (kMode == kVote) count += in ? 1 : 0;
-        else if (in) {
-          // slot of the grain in the brick + first sorted position of its row - first slot of its row
-          const int pos = (int)((j - sg_a) >> 2) + rdelta[(cz - B.cz0) * H + (cy - B.cy0)];
-          atomicMax(keyA + pos, ka); atomicMax(keyB + pos, kb);
-        }
-        j += 4u; ++item_tests;
+        test_grain(j);
+        j += 4u;
+        if (j < e) { test_grain(j); j += 4u; }
       }
     }
-    n_tests += item_tests;
+    n_tests += item_tests >> 2;
   }
 
   for (int o = 16; o; o >>= 1) n_tests += __shfl_xor_sync(EMU_FULL, n_tests, o);
