@@ -27,13 +27,13 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 CFG = 4                          # BASELINE.json configs[4] "throughput batch"
-CELL_UM = (4.0, 4.0, 4.0)        # cell size of the 3D hash (a pure speed knob: no effect on the track list)
+CELL_UM = (3.0, 4.0, 4.0)        # cell size of the 3D hash (a pure speed knob: no effect on the track list)
 VIEW_AREA_CM2 = 350e-4 * 300e-4  # 350 x 300 um = 1.05e-3 cm^2 per view
 # Algorithmic work of the voting kernel: lane-instructions per seed
 #   = tests/seed * 18 + pair-tests/seed * 9, with tests/seed and pair-tests/seed the ORACLE's own counters
 # (oracle mode "cells", same cell size) on views 0..7 of this workload.  The cpu_baseline leg re-measures
 # them live; the constants serve the runs that have no such leg (N > 1).
-ALG_PER_SEED = {(8.0, 8.0, 8.0): (317.7, 2.88)}
+ALG_PER_SEED = {(8.0, 8.0, 8.0): (317.7, 2.88), (3.0, 4.0, 4.0): (102.1, 2.26)}
 INSTR_PER_TEST, INSTR_PER_PAIR = 18, 9
 BIN_BYTES_PER_GRAIN = 32.7       # 16 B read + 16 B written + 4 B per cell
 
@@ -207,9 +207,11 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     assert world == args.gpus, f"--gpus {args.gpus} but WORLD_SIZE={world}: launch with torchrun"
 
+    from paper_1311_5334_b200 import shard
     p = params_dict()
     V = args.views
-    grains, off = make_workload(rank * V, V)
+    first_view, _ = shard.view_range(rank, world, V)          # weak scaling: every rank owns V views of its own
+    grains, off = make_workload(first_view, V)
     n = int(off[-1])
     prm = E.make_params(**{k: p[k] for k in ("view_size_q", "cell_size_q", "sep_min_q", "sep_max_q", "tube_r2_q",
                                              "min_grains", "max_tracks_per_view")})
@@ -245,14 +247,7 @@ def main():
     ms_total = ev0.elapsed_time(ev1)
     clocks = sampler.stop() if rank == 0 else None
     stage_ms, stage_launches = prof.read()
-    t_ms = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t_ms, op=dist.ReduceOp.MAX)
-    ms_total = float(t_ms.item())
-    n_all = torch.tensor([n], dtype=torch.int64, device="cuda")
-    if world > 1:
-        dist.all_reduce(n_all, op=dist.ReduceOp.SUM)
-    n_total = int(n_all.item())
+    ms_total, (n_total,) = shard.reduce_step(ms_total, [n], device="cuda")    # max over ranks / sum over ranks
     ms_step = ms_total / args.steps
     counts = B.counts.cpu().numpy().copy()
 
@@ -269,12 +264,10 @@ def main():
             nt, nm = H.call()                               # synchronous: returns with the outputs on the host
         barrier()
         dt = time.perf_counter() - t0
-        t_e = torch.tensor([dt], dtype=torch.float64, device="cuda")
-        if world > 1:
-            dist.all_reduce(t_e, op=dist.ReduceOp.MAX)
-        e2e = {"value": n_total * args.steps / float(t_e.item()), "unit": "grains/s",
+        dt_max, _ = shard.reduce_step(dt, [0], device="cuda")
+        e2e = {"value": n_total * args.steps / dt_max, "unit": "grains/s",
                "h2d_bytes_per_step": H.h2d_bytes(), "d2h_bytes_per_step": H.d2h_bytes(nt, nm),
-               "ms_per_step": float(t_e.item()) / args.steps * 1e3,
+               "ms_per_step": dt_max / args.steps * 1e3,
                "call": "emu_track_views_host (pinned host buffers; copies inside the timed call)"}
         assert int(H.h_counts[E.EMU_CNT["status"]]) == 0
         assert nt == int(counts[E.EMU_CNT["tracks"]]), "host path and device path disagree"
@@ -306,7 +299,7 @@ def main():
     if alg is not None and stage_launches["vote"]:
         alg_instr = seeds * (alg[0] * INSTR_PER_TEST + alg[1] * INSTR_PER_PAIR)   # per step, all vote launches
         achieved = alg_instr / (stage_ms["vote"] / args.steps * 1e-3) / 1e12
-        roofline = {"kernel": "k_vote", "bound": "alu", "achieved": achieved, "peak": alu_peak,
+        roofline = {"kernel": "k_brick<kVote> (A2 seeds are streamed in, A3 tube count, shared-memory bricks)", "bound": "alu", "achieved": achieved, "peak": alu_peak,
                     "unit": "Tlane-instr/s", "frac": achieved / alu_peak, "traffic": None,
                     "peak_source": f"148 SM x 4 schedulers x 32 lanes x {sm_max:.0f} MHz ({peaks['_source']} max SM clock)",
                     "algorithmic": f"{seeds} seeds x ({alg[0]:.1f} tests x {INSTR_PER_TEST} + {alg[1]:.2f} pair tests x "
