@@ -45,8 +45,18 @@ EmuDev make_dev(const emu_params* p) {
     d.klo[i] = -(d.Rw * d.inv_cs[i] + 0.5f);
     d.khi[i] = d.Rw * d.inv_cs[i] - 0.5f;
   }
-  // 4-byte grains: x in 16 bits, y and z relative to their cell in 8 bits each (emu_find.cu)
-  d.packed_ok = ((int64_t)d.n[0] * d.cs[0] <= 65536 && d.cs[1] <= 256 && d.cs[2] <= 256) ? 1 : 0;
+  // frames: cyclic permutations of the axes, the same cell size triple applied to (u,v,w)
+  // 4-byte grains: u in 16 bits, v and w relative to their cell in 8 bits each (emu_find.cu)
+  d.packed_ok = (d.cs[1] <= 256 && d.cs[2] <= 256) ? 1 : 0;
+  for (int f = 0; f < 3; ++f) {
+    int64_t fc = 1;
+    for (int i = 0; i < 3; ++i) {
+      d.fr[f].n[i] = (p->view_size_q[(f + i) % 3] + d.cs[i] - 1) / d.cs[i];
+      fc *= d.fr[f].n[i];
+    }
+    d.fr[f].ncell = fc > 0x7fffffff ? -1 : (int)fc;
+    if ((int64_t)d.fr[f].n[0] * d.cs[0] > 65536) d.packed_ok = 0;
+  }
   d.min_grains = p->min_grains;
   d.max_tracks = p->max_tracks_per_view;
   return d;
@@ -54,7 +64,8 @@ EmuDev make_dev(const emu_params* p) {
 
 bool shape_ok(const EmuDev& d, int64_t n_grains, int32_t n_views) {
   if (d.ncell < 1 || n_views < 0 || n_grains < 0 || n_grains >= ((int64_t)1 << 31) - 64) return false;
-  if ((int64_t)n_views * d.ncell >= ((int64_t)1 << 31) - 64) return false;
+  for (int f = 0; f < 3; ++f)
+    if (d.fr[f].ncell < 1 || (int64_t)n_views * d.fr[f].ncell >= ((int64_t)1 << 31) - 64) return false;
   return true;
 }
 
@@ -148,7 +159,7 @@ int emu_bin_grains(const emu_params* params, const int32_t* d_grains, const int3
   if (!d_view_off || !d_cell_start || !d_status || !d_ws) return EMU_ERR_INVALID;
   if (n_grains > 0 && (!d_grains || !d_sorted)) return EMU_ERR_INVALID;
   if (!aligned16(d_grains) || !aligned16(d_sorted)) return EMU_ERR_INVALID;
-  return emu_bin_launch(d, d_grains, d_view_off, n_grains, n_views, d_sorted, d_cell_start, d_status, d_ws, ws_bytes,
+  return emu_bin_launch(d, 0, d_grains, d_view_off, n_grains, n_views, d_sorted, d_cell_start, d_status, d_ws, ws_bytes,
                         (cudaStream_t)stream);
 }
 
@@ -234,7 +245,7 @@ int emu_track_views_host(const emu_params* params, const int32_t* h_grains, cons
   if (n_grains > 0 && cudaMemcpyAsync(A.grains, h_grains, (size_t)n_grains * 16, cudaMemcpyHostToDevice, st) != cudaSuccess) return EMU_ERR_CUDA;
   if (cudaMemcpyAsync(A.view_off, h_view_off, ((size_t)n_views + 1) * 4, cudaMemcpyHostToDevice, st) != cudaSuccess) return EMU_ERR_CUDA;
   if (cudaMemsetAsync(A.status, 0, 8, st) != cudaSuccess) return EMU_ERR_CUDA;
-  int rc = emu_bin_launch(d, A.grains, A.view_off, n_grains, n_views, A.sorted, A.cell_start, A.status, A.ws, A.ws_bytes, st);
+  int rc = emu_bin_launch(d, 0, A.grains, A.view_off, n_grains, n_views, A.sorted, A.cell_start, A.status, A.ws, A.ws_bytes, st);
   if (rc != EMU_OK) return rc;
   rc = emu_find_launch(d, seeds_per_grain(params), cand_per_grain(params), A.sorted, A.cell_start, A.view_off, n_grains, n_views, A.tracks,
                        A.track_off, A.members, n_grains, A.counts, A.ws, A.ws_bytes, st);

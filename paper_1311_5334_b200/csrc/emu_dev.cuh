@@ -10,7 +10,14 @@
 
 #define EMU_FULL 0xffffffffu
 
+// Frames.  The tube walk of emu_find.cu wants the line's dominant axis to be the axis the rows of cells
+// run along, so every view is binned three times, once per cyclic permutation of the axes:
+//   frame 0: (u,v,w) = (x,y,z)   frame 1: (u,v,w) = (y,z,x)   frame 2: (u,v,w) = (z,x,y)
+// The cell size triple cs[] applies to (u,v,w) in every frame; frame 0 is the binning the C ABI defines.
+struct EmuFrame { int n[3]; int ncell; };
+
 struct EmuDev {           // passed by value to every kernel
+  EmuFrame fr[3];         // grid of every frame: n = ceil(view_size[perm] / cs); fr[0] = {n, ncell}
   int n[3];               // cells per axis = ceil(view_size / cell_size)
   int cs[3];              // cell size, q
   float inv_cs[3];
@@ -29,6 +36,13 @@ struct EmuDev {           // passed by value to every kernel
   int packed_ok;          // 1: the 4-byte grain format of the brick kernels can hold a view of this grid
 };
 
+// lab coordinates -> frame coordinates (w is carried along)
+__host__ __device__ __forceinline__ int4 emu_to_frame(int f, int4 g) {
+  if (f == 1) return make_int4(g.y, g.z, g.x, g.w);
+  if (f == 2) return make_int4(g.z, g.x, g.y, g.w);
+  return g;
+}
+
 // floor(c / cs) clamped to [0, n-1] (reading Q13: out-of-box grains land in the boundary cells).
 // |c| < 2^18 here, so the float quotient is within 1 of the truth and one correction step is exact.
 __device__ __forceinline__ int emu_cell_axis(int c, int cs, float inv_cs, int n) {
@@ -43,6 +57,15 @@ __device__ __forceinline__ int emu_cell_of(const EmuDev& P, int x, int y, int z)
   int cy = emu_cell_axis(y, P.cs[1], P.inv_cs[1], P.n[1]);
   int cz = emu_cell_axis(z, P.cs[2], P.inv_cs[2], P.n[2]);
   return cx + P.n[0] * (cy + P.n[1] * cz);
+}
+
+// cell of a grain given in the coordinates of frame f
+__device__ __forceinline__ int emu_cell_of_frame(const EmuDev& P, int f, int u, int v, int w) {
+  const EmuFrame& F = P.fr[f];
+  int cu = emu_cell_axis(u, P.cs[0], P.inv_cs[0], F.n[0]);
+  int cv = emu_cell_axis(v, P.cs[1], P.inv_cs[1], F.n[1]);
+  int cw = emu_cell_axis(w, P.cs[2], P.inv_cs[2], F.n[2]);
+  return cu + F.n[0] * (cv + F.n[1] * cw);
 }
 
 // view that owns sorted position / row g: largest v in [v0, v1) with view_off[v] <= g

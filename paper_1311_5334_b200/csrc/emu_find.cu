@@ -1,16 +1,24 @@
 // emu_find.cu - A2..A5 + A7: seeds, tube vote, threshold, exclusive association, threshold, order.
 // (P:72 and Fig. 4; readings Q1-Q8, Q15 in DESIGN.md section 3.)
 //
+// FRAMES.  A seed line is walked in the frame whose first axis u is the line's dominant axis (emu_dev.cuh):
+// rows of cells run along u, so a line with |dv|, |dw| <= |du| stays long in every row it enters and enters
+// few of them.  Every view is therefore binned three times (frame 0 is the caller's A1 output, frames 1
+// and 2 are binned here from it), the seeds of a view are split into three lists by dominant axis, and
+// the brick kernels see three "virtual views" per view.  Grain-indexed state (priority keys, owners) is
+// indexed by ROW (the caller's grain index), which every frame carries in w.
+//
 // Views are processed in chunks sized by the workspace.  Per chunk:
-//   k_seed_pairs<0>   every grain A: number of seeds {A,B}, B behind A in cell order          (A2)
-//   k_view_scan, k_chunk_offsets   per-grain / per-view seed offsets (deterministic seed layout)
-//   k_seed_pairs<1>   the seeds themselves: packed geometry (A, d) + the two sorted positions
-//   k_plan            cut every view into BRICKS (a tile of cell columns x a run of z layers) that fit
-//                     shared memory
+//   k_seed_pairs<0>   every grain A: number of seeds {A,B}, B behind A in cell order, per frame  (A2)
+//   k_view_scan, k_chunk_offsets   per-grain / per-(view, frame) seed offsets
+//   k_seed_pairs<1>   the seeds themselves: packed geometry (A, d) in frame coordinates, oriented so that
+//                     du > 0, + the two sorted positions (frame 0)
+//   k_plan            cut every (view, frame) into BRICKS (a tile of cell columns x a run of w layers) that
+//                     fit shared memory
 //   k_brick<VOTE>     persistent blocks: stage one brick's grains + cell table in shared memory, stream
-//                     all seeds of the view past it; every lane walks its own seed's tube through the
-//                     brick (uniform-grid ray traversal) and counts with the exact integer test   (A3)
-//   k_cands<0/1>      n_tube >= min_grains -> candidate list grouped by view                     (A4)
+//                     all seeds of the (view, frame) past it; every lane walks its own seed's tube through
+//                     the brick (uniform-grid ray traversal) and counts with the exact integer test (A3)
+//   k_cands<0/1>      n_tube >= min_grains -> candidate list grouped by (view, frame)            (A4)
 //   k_brick<ASSOC>    the candidates again: atomicMax of a packed priority into each member grain (A5)
 //   k_tie_detect, k_assoc_generic<1>   exact settlement of priority ties by (kmin, kmax)
 //   k_wins, k_select  members won per candidate, threshold again
@@ -51,11 +59,18 @@ struct Cand {            // 16 B
   int d2;
 };
 
-struct Brick {           // 32 B: cells [cx0..cx1] x [cy0..cy1] x [cz0..cz1] of one view, n grains
-  int view, cx0, cx1, cy0, cy1, cz0, cz1, n;
+struct Brick {           // 48 B: cells [cx0..cx1] x [cy0..cy1] x [cz0..cz1] (frame coordinates u, v, w) of one
+  int view, cx0, cx1, cy0, cy1, cz0, cz1, n;   // (view, frame), n grains
+  int frame, pad[3];
 };
 
-struct Tiling { int tx, ty, w, h; };   // tiles per view in x and y, tile width / height in cells
+struct Tiling { int tx, ty, w, h; };   // tiles per (view, frame) in u and v, tile width / height in cells
+struct Tilings { Tiling t[3]; };
+
+struct FramePtrs {       // the three binnings of the batch (frame 0 = the caller's arrays)
+  const int4* sorted[3];
+  const int* cell_start[3];
+};
 
 struct FindCtl {         // device scalars of one chunk
   unsigned cand_count;   // candidates of the chunk
@@ -174,23 +189,35 @@ k_bbox(const int4* __restrict__ sorted, const int* __restrict__ view_off, int n_
 }
 
 // ---------------------------------------------------------------------------------------------
-// A2.  One warp per grain A: the lanes scan the cells around A for partners B behind A in sorted
-// order (each unordered pair once, reading Q2) inside the separation window (reading Q1).
-//   kFill = 0: seed_off[a] = number of seeds of A
-//   kFill = 1: the seeds are written at view_seed_off[v - v0] + seed_off[a] + rank (seed_off now holds
-//              the exclusive prefix inside the view): a deterministic layout, grouped by A.
+// A2.  One warp per grain A.  The rows of cells (cy, cz) within sep_max of A are dealt to the lanes; a lane
+// runs along its row and tests the partners B BEHIND A in sorted order (each unordered pair once, reading
+// Q2) against the separation window (reading Q1).  A seed belongs to the frame of its dominant axis
+// (largest |d| component, the lowest axis on a tie).
+//   kFill = 0: seed_off[f * plane + a] = number of seeds of A in frame f
+//   kFill = 1: the seeds are written at view_seed_off[(v - v0) * 3 + f] + seed_off[f * plane + a] + slot
+//              (seed_off now holds the exclusive prefix inside the (view, frame)); the slot inside A's
+//              group comes from a warp-private counter, so the order inside a group is arbitrary - nothing
+//              downstream depends on the order of the seeds (every reduction is over a total order).
+constexpr int kPairWarps = kVoteThreads / 32;
+
+__device__ __forceinline__ int dominant_axis(int dx, int dy, int dz) {
+  const int ax = abs(dx), ay = abs(dy), az = abs(dz);
+  return (ax >= ay && ax >= az) ? 0 : (ay >= az ? 1 : 2);
+}
+
 template <int kFill>
 __global__ void __launch_bounds__(kVoteThreads)
 k_seed_pairs(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ cell_start,
-             const int* __restrict__ view_off, int v0, int v1, unsigned* __restrict__ seed_off,
+             const int* __restrict__ view_off, int v0, int v1, unsigned* __restrict__ seed_off, size_t plane,
              const unsigned* __restrict__ view_seed_off, const FindCtl* __restrict__ ctl,
              int4* __restrict__ geo, int2* __restrict__ ab, unsigned long long* __restrict__ counts) {
+  __shared__ unsigned cur_s[kPairWarps][4];
   if (kFill && ctl->skip) return;
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
-  const int nwarps = gridDim.x * (kVoteThreads / 32);
+  const int nwarps = gridDim.x * kPairWarps;
   const int g0 = __ldg(view_off + v0), g1 = __ldg(view_off + v1);
   unsigned long long n_pairs = 0;
-  for (int a = g0 + blockIdx.x * (kVoteThreads / 32) + wib; a < g1; a += nwarps) {
+  for (int a = g0 + blockIdx.x * kPairWarps + wib; a < g1; a += nwarps) {
     const int v = emu_find_view(view_off, v0, v1, a);
     const int4 A = __ldg(sorted + a);
     const int vbase = v * P.ncell;
@@ -200,38 +227,53 @@ k_seed_pairs(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ 
     const int cyb = emu_cell_axis(A.y + P.sep_max, P.cs[1], P.inv_cs[1], P.n[1]);
     const int czA = emu_cell_axis(A.z, P.cs[2], P.inv_cs[2], P.n[2]);   // partners behind A: cell >= cell(A)
     const int czb = emu_cell_axis(A.z + P.sep_max, P.cs[2], P.inv_cs[2], P.n[2]);
-    unsigned n = 0;
-    unsigned base = 0;
-    if (kFill) base = view_seed_off[v - v0] + seed_off[a];
-    for (int cz = czA; cz <= czb; ++cz) {
-      for (int cy = cya; cy <= cyb; ++cy) {
-        const int rb = vbase + (cz * P.n[1] + cy) * P.n[0];
-        int s = __ldg(cell_start + rb + cxa);
-        const int e = __ldg(cell_start + rb + cxb + 1);
-        s = max(s, a + 1);
-        for (int j0 = s; j0 < e; j0 += 32) {
-          const int j = j0 + lane;
-          bool ok = false;
-          int dx = 0, dy = 0, dz = 0;
-          if (j < e) {
-            int4 B = __ldg(sorted + j);
-            dx = B.x - A.x; dy = B.y - A.y; dz = B.z - A.z;
-            // |d| can exceed 2^15 for far out-of-box grains: compare in 64 bits
-            long long d2 = (long long)dx * dx + (long long)dy * dy + (long long)dz * dz;
-            ok = (d2 >= P.sep_min2) && (d2 < P.sep_max2);
-            ++n_pairs;
-          }
-          const unsigned m = __ballot_sync(EMU_FULL, ok);
-          if (kFill && ok) {
-            const unsigned idx = base + n + __popc(m & ((1u << lane) - 1u));
-            geo[idx] = geo_pack(A.x, A.y, A.z, dx, dy, dz);
+    const int ny = cyb - cya + 1, n_rows = ny * (czb - czA + 1);
+    const float inv_ny = 1.0f / (float)ny;
+    unsigned n[3] = {0u, 0u, 0u};
+    unsigned base[3] = {0u, 0u, 0u};
+    if (kFill) {
+#pragma unroll
+      for (int f = 0; f < 3; ++f) base[f] = view_seed_off[(v - v0) * 3 + f] + seed_off[(size_t)f * plane + a];
+      if (lane < 3) cur_s[wib][lane] = 0u;
+      __syncwarp();
+    }
+    for (int r = lane; r < n_rows; r += 32) {
+      const int lz = (int)(((float)r + 0.5f) * inv_ny);              // r / ny (small integers: exact)
+      const int cz = czA + lz, cy = cya + (r - lz * ny);
+      const int rb = vbase + (cz * P.n[1] + cy) * P.n[0];
+      int s = __ldg(cell_start + rb + cxa);
+      const int e = __ldg(cell_start + rb + cxb + 1);
+      s = max(s, a + 1);
+      for (int j = s; j < e; ++j) {
+        const int4 B = __ldg(sorted + j);
+        const int dx = B.x - A.x, dy = B.y - A.y, dz = B.z - A.z;
+        // |d| can exceed 2^15 for far out-of-box grains: compare in 64 bits
+        const long long d2 = (long long)dx * dx + (long long)dy * dy + (long long)dz * dz;
+        ++n_pairs;
+        if (d2 >= P.sep_min2 && d2 < P.sep_max2) {
+          const int f = dominant_axis(dx, dy, dz);
+          if (!kFill) {
+            n[0] += (f == 0); n[1] += (f == 1); n[2] += (f == 2);
+          } else {
+            const unsigned idx = (f == 0 ? base[0] : (f == 1 ? base[1] : base[2])) + atomicAdd(&cur_s[wib][f], 1u);
+            int4 Af = emu_to_frame(f, A);
+            int4 df = emu_to_frame(f, make_int4(dx, dy, dz, 0));
+            if (df.x < 0) { Af = emu_to_frame(f, B); df.x = -df.x; df.y = -df.y; df.z = -df.z; }   // du > 0
+            geo[idx] = geo_pack(Af.x, Af.y, Af.z, df.x, df.y, df.z);
             ab[idx] = make_int2(a, j);
           }
-          n += __popc(m);
         }
       }
     }
-    if (!kFill && lane == 0) seed_off[a] = n;
+    if (!kFill) {
+#pragma unroll
+      for (int f = 0; f < 3; ++f) {
+        const unsigned t = __reduce_add_sync(EMU_FULL, n[f]);
+        if (lane == 0) seed_off[(size_t)f * plane + a] = t;
+      }
+    } else {
+      __syncwarp();
+    }
   }
   if (!kFill) {
     for (int o = 16; o; o >>= 1) n_pairs += __shfl_xor_sync(EMU_FULL, n_pairs, o);
@@ -239,14 +281,17 @@ k_seed_pairs(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ 
   }
 }
 
-// per-view exclusive scan (in place) of the per-grain seed counts; view_tot[v - v0] = seeds of the view
+// per-(view, frame) exclusive scan (in place) of the per-grain seed counts;
+// view_tot[(v - v0) * 3 + f] = seeds of the view in frame f
 __global__ void __launch_bounds__(1024)
-k_view_scan(const int* __restrict__ view_off, int v0, int v1, unsigned* __restrict__ seed_off,
+k_view_scan(const int* __restrict__ view_off, int v0, int v1, unsigned* __restrict__ seed_off_all, size_t plane,
             unsigned* __restrict__ view_tot, unsigned long long* __restrict__ counts) {
   __shared__ unsigned warp_sum[32];
   __shared__ unsigned carry_s;
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-  for (int v = v0 + blockIdx.x; v < v1; v += gridDim.x) {
+  for (int vf = blockIdx.x; vf < (v1 - v0) * 3; vf += gridDim.x) {
+    const int v = v0 + vf / 3;
+    unsigned* seed_off = seed_off_all + (size_t)(vf % 3) * plane;
     const int g0 = __ldg(view_off + v), g1 = __ldg(view_off + v + 1);
     if (threadIdx.x == 0) carry_s = 0;
     __syncthreads();
@@ -275,7 +320,7 @@ k_view_scan(const int* __restrict__ view_off, int v0, int v1, unsigned* __restri
       if (threadIdx.x == blockDim.x - 1) carry_s = mine;
       __syncthreads();
     }
-    if (threadIdx.x == 0) view_tot[v - v0] = carry_s;
+    if (threadIdx.x == 0) view_tot[vf] = carry_s;
     __syncthreads();
   }
 }
@@ -328,25 +373,33 @@ k_chunk_offsets(int nv, const unsigned* __restrict__ tot, unsigned* __restrict__
 }
 
 // ---------------------------------------------------------------------------------------------
-// Brick plan: one warp per view.  Every tile (tx, ty) of cell columns is cut into runs of z layers
+// Brick plan: one warp per (view, frame).  Every tile (tx, ty) of cell columns is cut into runs of w layers
 // whose grains, row table and cell table fit the shared-memory pool; empty bricks are dropped.
-// The brick kernels keep a grain in 4 bytes (x in 16 bits, y and z relative to the cell in 8 bits),
+// The brick kernels keep a grain in 4 bytes (u in 16 bits, v and w relative to the cell in 8 bits),
 // which needs every grain of the view inside the box: a view with out-of-box grains (legal, reading
 // Q13), or a grid the format cannot hold, sends the chunk to the generic kernels.
 __global__ void __launch_bounds__(128)
-k_plan(EmuDev P, Tiling T, const int* __restrict__ cell_start, const EmuBox* __restrict__ bbox, int v0, int v1,
+k_plan(EmuDev P, Tilings TT, FramePtrs F, const EmuBox* __restrict__ bbox, int v0, int v1,
        Brick* __restrict__ bricks, unsigned brick_cap, FindCtl* __restrict__ ctl) {
   const int lane = threadIdx.x & 31;
-  const int v = v0 + blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-  if (v >= v1 || ctl->skip) return;
-  const int nx = P.n[0], ny = P.n[1], nz = P.n[2];
-  const int vbase = v * P.ncell;
-  if (cell_start[vbase + P.ncell] == cell_start[vbase]) return;          // empty view: no bricks
+  const int vf = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+  if (vf >= (v1 - v0) * 3 || ctl->skip) return;
+  const int v = v0 + vf / 3, f = vf % 3;
+  const Tiling T = TT.t[f];
+  const int* __restrict__ cell_start = F.cell_start[f];
+  const int nx = P.fr[f].n[0], ny = P.fr[f].n[1], nz = P.fr[f].n[2];
+  const int vbase = v * P.fr[f].ncell;
+  if (cell_start[vbase + P.fr[f].ncell] == cell_start[vbase]) return;          // empty view: no bricks
   {
-    const EmuBox bb = bbox[v];
+    const EmuBox bb = bbox[v];                                               // lab coordinates
     bool in_box = P.packed_ok != 0;
 #pragma unroll
     for (int a = 0; a < 3; ++a) in_box = in_box && bb.lo[a] >= 0 && bb.hi[a] < P.n[a] * P.cs[a];
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {                                            // ... and inside every frame's grid
+      const int a = (f + i) % 3;
+      in_box = in_box && bb.hi[a] < P.fr[f].n[i] * P.cs[i];
+    }
     if (!in_box) { if (lane == 0) ctl->generic = 1; return; }
   }
   for (int t = 0; t < T.tx * T.ty; ++t) {
@@ -371,6 +424,7 @@ k_plan(EmuDev P, Tiling T, const int* __restrict__ cell_start, const EmuBox* __r
           const unsigned slot = atomicAdd(&ctl->n_bricks, 1u);
           if (slot < brick_cap) {
             Brick b; b.view = v; b.cx0 = cx0; b.cx1 = cx1; b.cy0 = cy0; b.cy1 = cy1; b.cz0 = z_first; b.cz1 = cz - 1; b.n = acc;
+            b.frame = f; b.pad[0] = b.pad[1] = b.pad[2] = 0;
             bricks[slot] = b;
           }
         }
@@ -389,20 +443,22 @@ __global__ void k_plan_finish(FindCtl* ctl, unsigned brick_cap) {
 // ---------------------------------------------------------------------------------------------
 // A3 / A5 on shared-memory bricks.
 //
-// A persistent block takes work items (brick, slice of the view's seed list).  It stages the brick in
-// shared memory - every grain in 4 bytes (x | y-in-cell << 16 | z-in-cell << 24) in (cz, cy, cx) order,
-// a 16-bit cell table, and per row of cells the sorted position of its first grain - and streams the
-// seeds of the slice past it.  Each LANE owns one seed at a time and is in one of three states; the
-// warp repeatedly executes the phase most of its lanes wait for (persistent-thread ray traversal):
-//   SEED  fetch the next seed of the warp's range, unpack it, clip the line against the brick
-//   ROW   advance the traversal: next row of cells (cy) of the current z layer, else the next layer,
-//         giving a run [j, e) of consecutive grains of the cells cx0..cx1 the tube can touch in the row
-//   TEST  one point-line test of grain j; VOTE counts, ASSOC joins the priority maximum of the grain
+// A persistent block takes work items (brick, slice of the seed list of the brick's (view, frame)).  It
+// stages the brick in shared memory - every grain in 4 bytes (u | v-in-cell << 16 | w-in-cell << 24) in
+// (cw, cv, cu) order, a 16-bit cell table, and per row of cells the sorted position of its first grain - and
+// streams the seeds of the slice past it.  Each LANE owns one seed at a time; the loop body is fused:
+//   SEED  idle lanes are refilled in batches from the block's seed stream: unpack, clip against the brick
+//   ROW   lanes whose run of grains is used up advance: next row of cells (cv) of the current w layer, else
+//         the next layer, giving a run [j, e) of consecutive grains of the cells cu0..cu1 the tube can touch
+//   TEST  up to two point-line tests of the grains j, j+1; VOTE counts, ASSOC joins the priority maximum
 //
-// Traversal: the line is X(t) = A + t d.  A grain in the tube is within R of its foot on the line in
-// every coordinate, so a grain in row (cy, cz) has its foot parameter in the intersection of the two
-// slab intervals widened by Rw = R + 2 q, and its x within Rw of x over that interval.  The bounds are
-// float (errors far below the 2 q of slack) and only have to be a superset: the test decides.
+// Traversal.  In its frame the line has du > 0 and |dv|, |dw| <= du, so it is a function of u:
+//   v(u) = v0 + a u,  w(u) = w0 + b u,  a = dv/du, b = dw/du, |a|, |b| <= 1.
+// A grain in the tube is within R of its foot on the line in every coordinate, so a grain in row (cv, cw)
+// has its foot's u inside the intersection of the two slab intervals {u : v(u) in [cv cs - Rw, (cv+1) cs - 1 + Rw]}
+// and likewise for w, Rw = R + 2 q, and its own u within Rw of that interval.  The bounds are float (errors
+// far below the 2 q of slack, measured in v / w: an error in an interval end is the error of v(u) there divided
+// by a, so it does not grow in v) and only have to be a superset: the test decides.
 //
 // Test: v = P - A and d are exact in float (|v| < 2^16, |d| < 2^11).  c = v x d is formed as
 // fma(v1, d2, -rn(v2 d1)): the products stay below 2^27, so |c_f - c| <= 4 + 2^-24 |c| per component, and
@@ -418,6 +474,11 @@ constexpr int kRefillStop = 4;                    // the refill goes on while at
 __device__ __forceinline__ unsigned lds_u32(unsigned addr) {
   unsigned v;
   asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr));
+  return v;
+}
+__device__ __forceinline__ unsigned lds_u32_off4(unsigned addr) {
+  unsigned v;
+  asm volatile("ld.shared.u32 %0, [%1+4];" : "=r"(v) : "r"(addr));
   return v;
 }
 __device__ __forceinline__ unsigned lds_u16(unsigned addr) {
@@ -436,8 +497,7 @@ struct BrickShared {
 
 template <int kMode>
 __global__ void __launch_bounds__(kBrickThreads, 1)
-k_brick(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ cell_start,
-        int v0, const Brick* __restrict__ bricks, FindCtl* __restrict__ ctl,
+k_brick(EmuDev P, FramePtrs F, int v0, const Brick* __restrict__ bricks, FindCtl* __restrict__ ctl,
         int slices, const int4* __restrict__ geo, const unsigned* __restrict__ view_item_off,
         unsigned* __restrict__ seed_cnt, unsigned long long* __restrict__ keyA,
         unsigned long long* __restrict__ keyB, unsigned long long* __restrict__ counts) {
@@ -455,9 +515,10 @@ k_brick(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ cell_
   unsigned long long n_tests = 0;
   int cur_brick = -1;
   Brick B;
-  B.view = 0; B.cx0 = B.cx1 = B.cy0 = B.cy1 = B.cz0 = B.cz1 = B.n = 0;
+  B.view = 0; B.cx0 = B.cx1 = B.cy0 = B.cy1 = B.cz0 = B.cz1 = B.n = 0; B.frame = 0;
   int W = 1, H = 1, S = 4;
   float blo[3] = {0.f, 0.f, 0.f}, bhi[3] = {0.f, 0.f, 0.f};   // brick extent widened by R
+  const int4* __restrict__ sorted = F.sorted[0];
 
   for (;;) {
     __syncthreads();                                  // everyone is done with the previous item
@@ -471,9 +532,12 @@ k_brick(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ cell_
       // ---- stage brick b ----
       cur_brick = b;
       B = bricks[b];
+      sorted = F.sorted[B.frame];
+      const int* __restrict__ cell_start = F.cell_start[B.frame];
+      const int gnx = P.fr[B.frame].n[0], gny = P.fr[B.frame].n[1];
       W = B.cx1 - B.cx0 + 1; H = B.cy1 - B.cy0 + 1; S = brick_row_stride(W);
       const int rows = H * (B.cz1 - B.cz0 + 1);
-      const int vbase = B.view * P.ncell;
+      const int vbase = B.view * P.fr[B.frame].ncell;
       unsigned* sgw = reinterpret_cast<unsigned*>(pool);
       unsigned short* tab = reinterpret_cast<unsigned short*>(pool + 4 * (size_t)B.n);
       {
@@ -490,7 +554,7 @@ k_brick(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ cell_
         int gs = 0, len = 0;
         if (r < rows) {
           const int cz = B.cz0 + r / H, cy = B.cy0 + r % H;
-          const int rb = vbase + (cz * P.n[1] + cy) * P.n[0];
+          const int rb = vbase + (cz * gny + cy) * gnx;
           gs = __ldg(cell_start + rb + B.cx0);
           len = __ldg(cell_start + rb + B.cx1 + 1) - gs;
         }
@@ -517,7 +581,7 @@ k_brick(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ cell_
           const int rr = r0 + k;
           const int rgs = sh.row_gs[k], roff = rgs - *reinterpret_cast<const int*>(tab + (size_t)rr * S + (S - 2));
           const int cz = B.cz0 + rr / H, cy = B.cy0 + rr % H;
-          const int rb = vbase + (cz * P.n[1] + cy) * P.n[0] + B.cx0;
+          const int rb = vbase + (cz * gny + cy) * gnx + B.cx0;
           for (int i = lane; i <= W; i += 32) tab[(size_t)rr * S + i] = (unsigned short)(roff + (__ldg(cell_start + rb + i) - rgs));
           const int rlen = __ldg(cell_start + rb + W) - rgs;
           const int y0 = cy * P.cs[1], z0 = cz * P.cs[2];
@@ -529,10 +593,10 @@ k_brick(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ cell_
         __syncthreads();
       }
     }
-    // ---- the slice of the view's items ----
+    // ---- the slice of the (view, frame)'s items ----
     {
-      const int vl = B.view - v0;
-      const unsigned lo = view_item_off[vl], hi = view_item_off[vl + 1];
+      const int vf = (B.view - v0) * 3 + B.frame;
+      const unsigned lo = view_item_off[vf], hi = view_item_off[vf + 1];
       const unsigned per = (hi - lo + (unsigned)slices - 1u) / (unsigned)slices;
       const unsigned s0 = min(hi, lo + per * (unsigned)sl), s1 = min(hi, s0 + per);
       if (tid == 0) { sh.next = s0; sh.end = s1; }
@@ -541,17 +605,18 @@ k_brick(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ cell_
     const unsigned s_end = sh.end;
     // table address of row (cy = 0, cz = cz0 - 1) of the brick's numbering moved back by cx0 cells, so that
     // cell cx of row cy of the current layer sits at layp + cy * row_b + 2 cx
-    const unsigned row_b = 2u * (unsigned)S, lay_b = row_b * (unsigned)H;   // table bytes per row / per z layer
+    const unsigned row_b = 2u * (unsigned)S, lay_b = row_b * (unsigned)H;   // table bytes per row / per w layer
     const unsigned tab0 = pool_a + 4u * (unsigned)B.n - 2u * (unsigned)B.cx0 - (unsigned)B.cy0 * row_b - lay_b;
     const unsigned delta_o = 2u * (unsigned)(B.cx0 + S - 2);               // from a row address to its position word
-    const float cz0f = (float)B.cz0, cz1f = (float)B.cz1, cy1f = (float)B.cy1;
+    const float cz1f = (float)B.cz1, cy1f = (float)B.cy1;
 
     // ---- per-lane state: one seed per lane ----
     bool idle = true;                                // no seed (waiting for the next refill)
-    float ax = 0.f, ay = 0.f, dx = 0.f, dy = 0.f, dz = 0.f;
+    float ay = 0.f, dx = 1.f, dy = 0.f, dz = 0.f;
+    float a = 0.f, y0 = 0.f;                         // v(u) = y0 + a u
     float oxm = 0.f, oym = 0.f, ozm = 0.f;           // magic-biased origin of v = P - A for the current row
     float Tlo = 0.f, Thi = 0.f;
-    float t0 = 0.f, t1 = 0.f, tl0 = 0.f, tl1 = 0.f;
+    float t0 = 0.f, t1 = 0.f, tl0 = 0.f, tl1 = 0.f;  // u interval of the line inside the brick / inside the layer
     float dty = 0.f, tyl = 0.f, tyh = 0.f, dtz = 0.f, tzl = 0.f, tzh = 0.f;
     float cyf = 1.f, cyhf = 0.f, czf = 0.f, czhf = -1.f;   // current / last row of the layer, current / last layer
     unsigned rowp = 0, layp = 0;                     // table address of the current row / of row 0 of the current layer
@@ -563,26 +628,18 @@ k_brick(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ cell_
     bool exhausted = false;
     unsigned item_tests = 0;
 
-    // one point-line test of the grain at shared address `ga` (see the header comment for the error band)
-    auto test_grain = [&](unsigned ga) {
-      const unsigned g = lds_u32(ga);
-      const float vx = __fsub_rn(magic_lo16(g), oxm), vy = __fsub_rn(magic_b2(g), oym), vz = __fsub_rn(magic_b3(g), ozm);
+    // |(P - A) x d|^2 in float for the grain word g (see the header comment for the error band)
+    auto tube_s = [&](unsigned g, float& vx, float& vy, float& vz) {
+      vx = __fsub_rn(magic_lo16(g), oxm); vy = __fsub_rn(magic_b2(g), oym); vz = __fsub_rn(magic_b3(g), ozm);
       const float cx = __fmaf_rn(vy, dz, -__fmul_rn(vz, dy));
       const float cyy = __fmaf_rn(vz, dx, -__fmul_rn(vx, dz));
       const float czz = __fmaf_rn(vx, dy, -__fmul_rn(vy, dx));
-      const float s = __fmaf_rn(cx, cx, __fmaf_rn(cyy, cyy, __fmul_rn(czz, czz)));
-      bool in = s <= Tlo;
-      if (s > Tlo && s <= Thi) {                            // inside the error band: the exact predicate
-        const int idx = __float2int_rn(dx), idy = __float2int_rn(dy), idz = __float2int_rn(dz);
-        in = emu_in_tube(__float2int_rn(vx), __float2int_rn(vy), __float2int_rn(vz), 0, 0, 0, idx, idy, idz,
+      return __fmaf_rn(cx, cx, __fmaf_rn(cyy, cyy, __fmul_rn(czz, czz)));
+    };
+    auto exact_in = [&](float vx, float vy, float vz) {
+      const int idx = __float2int_rn(dx), idy = __float2int_rn(dy), idz = __float2int_rn(dz);
+      return emu_in_tube(__float2int_rn(vx), __float2int_rn(vy), __float2int_rn(vz), 0, 0, 0, idx, idy, idz,
                          (long long)P.r2 * (long long)(idx * idx + idy * idy + idz * idz));
-      }
-      if (kMode == kVote) { if (in) ++count; }
-      else if (in) {
-        // slot of the grain in the brick + (sorted position - slot) of the first grain of its row
-        const int pos = (int)((ga - pool_a) >> 2) + (int)lds_u32(rowp + delta_o);
-        atomicMax(keyA + pos, ka); atomicMax(keyB + pos, kb);
-      }
     };
 
     for (;;) {
@@ -603,27 +660,31 @@ k_brick(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ cell_
           if (take) {
             const int4 q = __ldg(geo + idx);
             oxm = magic_lo16((unsigned)q.x);
-            ax = oxm - kMagicF; ay = magic_hi16((unsigned)q.x) - kMagicF;
+            const float ax = oxm - kMagicF;
+            ay = magic_hi16((unsigned)q.x) - kMagicF;
             const float az = magic_lo16((unsigned)q.y) - kMagicF;
             dx = magic_lo16((unsigned)q.z) - (kMagicF + 2048.0f); dy = magic_hi16((unsigned)q.z) - (kMagicF + 2048.0f);
             dz = magic_lo16((unsigned)q.w) - (kMagicF + 2048.0f);
-            const float inv_dx = dx != 0.f ? __fdividef(1.0f, dx) : 0.0f;
-            const float inv_dy = dy != 0.f ? __fdividef(1.0f, dy) : 0.0f;
-            const float inv_dz = dz != 0.f ? __fdividef(1.0f, dz) : 0.0f;
-            // clip the line against the brick's extent (already widened by R)
-            t0 = -BIG; t1 = BIG;
+            // du >= 1 (the seed is oriented along +u and u is its dominant axis)
+            const float inv_dx = __fdividef(1.0f, dx);
+            a = dy * inv_dx;
+            const float bz = dz * inv_dx;
+            y0 = __fmaf_rn(-a, ax, ay);
+            const float z0 = __fmaf_rn(-bz, ax, az);
+            const float inv_a = dy != 0.f ? __fdividef(dx, dy) : 0.0f;
+            const float inv_b = dz != 0.f ? __fdividef(dx, dz) : 0.0f;
+            // clip the line against the brick's extent (already widened by R): an interval of u
+            t0 = blo[0]; t1 = bhi[0];
             bool hit = true;
-            if (dx != 0.f) { const float a = (blo[0] - ax) * inv_dx, bq = (bhi[0] - ax) * inv_dx; t0 = fmaxf(t0, fminf(a, bq)); t1 = fminf(t1, fmaxf(a, bq)); }
-            else hit = hit && (ax >= blo[0]) && (ax <= bhi[0]);
-            if (dy != 0.f) { const float a = (blo[1] - ay) * inv_dy, bq = (bhi[1] - ay) * inv_dy; t0 = fmaxf(t0, fminf(a, bq)); t1 = fminf(t1, fmaxf(a, bq)); }
+            if (dy != 0.f) { const float p = (blo[1] - y0) * inv_a, r = (bhi[1] - y0) * inv_a; t0 = fmaxf(t0, fminf(p, r)); t1 = fminf(t1, fmaxf(p, r)); }
             else hit = hit && (ay >= blo[1]) && (ay <= bhi[1]);
-            if (dz != 0.f) { const float a = (blo[2] - az) * inv_dz, bq = (bhi[2] - az) * inv_dz; t0 = fmaxf(t0, fminf(a, bq)); t1 = fminf(t1, fmaxf(a, bq)); }
+            if (dz != 0.f) { const float p = (blo[2] - z0) * inv_b, r = (bhi[2] - z0) * inv_b; t0 = fmaxf(t0, fminf(p, r)); t1 = fminf(t1, fmaxf(p, r)); }
             else hit = hit && (az >= blo[2]) && (az <= bhi[2]);
             if (hit && t0 <= t1) {
               const float D2 = __fmaf_rn(dx, dx, __fmaf_rn(dy, dy, dz * dz));        // exact: < 2^22
               {
                 const float T = r2f * D2;
-                const float m_up = P.Rup * (fabsf(dx) + fabsf(dy) + fabsf(dz));
+                const float m_up = P.Rup * (dx + fabsf(dy) + fabsf(dz));
                 const float delta = __fmaf_rn(m_up, 4.76837158203125e-7f, 16.0f);   // 16 + 2^-21 m_up
                 const float band = __fmaf_rn(1.01f * delta, __fmaf_rn(2.0f, m_up, delta), T * 9.5367431640625e-7f);
                 Tlo = T - band; Thi = T + band;
@@ -634,12 +695,12 @@ k_brick(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ cell_
                 ka = (k1 << kCiBits) | (unsigned long long)(kCiMask - idx);
                 kb = (k1 << kCiBits) | (unsigned long long)idx;
               }
-              // slab k of an axis covers [k cs - R, (k+1) cs - 1 + R]: its t interval is the one of slab 0 moved by k cs / d
-              dty = P.csf[1] * inv_dy; dtz = P.csf[2] * inv_dz;
+              // slab k of an axis covers [k cs - R, (k+1) cs - 1 + R]: its u interval is the one of slab 0 moved by k cs / slope
+              dty = P.csf[1] * inv_a; dtz = P.csf[2] * inv_b;
               tyl = -BIG; tyh = BIG; tzl = -BIG; tzh = BIG;
-              if (dy != 0.f) { const float a = (-R - ay) * inv_dy, bq = (P.csf[1] - 1.0f + R - ay) * inv_dy; tyl = fminf(a, bq); tyh = fmaxf(a, bq); }
-              if (dz != 0.f) { const float a = (-R - az) * inv_dz, bq = (P.csf[2] - 1.0f + R - az) * inv_dz; tzl = fminf(a, bq); tzh = fmaxf(a, bq); }
-              const float za = __fmaf_rn(t0, dz, az), zb = __fmaf_rn(t1, dz, az);
+              if (dy != 0.f) { const float p = (-R - y0) * inv_a, r = (P.csf[1] - 1.0f + R - y0) * inv_a; tyl = fminf(p, r); tyh = fmaxf(p, r); }
+              if (dz != 0.f) { const float p = (-R - z0) * inv_b, r = (P.csf[2] - 1.0f + R - z0) * inv_b; tzl = fminf(p, r); tzh = fmaxf(p, r); }
+              const float za = __fmaf_rn(bz, t0, z0), zb = __fmaf_rn(bz, t1, z0);
               const int czi = max(B.cz0, rn_int(__fmaf_rn(fminf(za, zb), P.inv_cs[2], P.klo[2]))) - 1;   // the layer before the first
               czf = int_f(czi);
               czhf = fminf(cz1f, rn_flt(__fmaf_rn(fmaxf(za, zb), P.inv_cs[2], P.khi[2])));
@@ -660,7 +721,7 @@ k_brick(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ cell_
       // ---------------- ROW: lanes whose run is used up move to the next row of cells ----------------
       if (!idle && j >= e) {
         cyf += 1.0f; rowp += row_b; oym -= P.csf[1];
-        if (cyf > cyhf) {                                   // next z layer of the brick
+        if (cyf > cyhf) {                                   // next w layer of the brick
           czf += 1.0f; ozm -= P.csf[2]; layp += lay_b;
           if (czf > czhf) {                                 // the seed is finished
             if (kMode == kVote && count) atomicAdd(seed_cnt + sidx, (unsigned)count);
@@ -669,7 +730,7 @@ k_brick(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ cell_
             tl0 = fmaxf(t0, __fmaf_rn(czf, dtz, tzl)); tl1 = fminf(t1, __fmaf_rn(czf, dtz, tzh));
             cyf = 1.f; cyhf = 0.f;
             if (tl0 <= tl1) {
-              const float ya = __fmaf_rn(tl0, dy, ay), yb = __fmaf_rn(tl1, dy, ay);
+              const float ya = __fmaf_rn(a, tl0, y0), yb = __fmaf_rn(a, tl1, y0);
               const int cyi = max(B.cy0, rn_int(__fmaf_rn(fminf(ya, yb), P.inv_cs[1], P.klo[1])));
               cyhf = fminf(cy1f, rn_flt(__fmaf_rn(fmaxf(ya, yb), P.inv_cs[1], P.khi[1])));
               cyf = int_f(cyi);
@@ -681,9 +742,8 @@ k_brick(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ cell_
         if (!idle && cyf <= cyhf) {                         // row cyf of layer czf
           const float ta = fmaxf(tl0, __fmaf_rn(cyf, dty, tyl)), tb = fminf(tl1, __fmaf_rn(cyf, dty, tyh));
           if (ta <= tb) {
-            const float xa = __fmaf_rn(ta, dx, ax), xb = __fmaf_rn(tb, dx, ax);
-            const int c0 = max(B.cx0, rn_int(__fmaf_rn(fminf(xa, xb), P.inv_cs[0], P.klo[0])));
-            const int c1 = min(B.cx1, rn_int(__fmaf_rn(fmaxf(xa, xb), P.inv_cs[0], P.khi[0])));
+            const int c0 = max(B.cx0, rn_int(__fmaf_rn(ta, P.inv_cs[0], P.klo[0])));
+            const int c1 = min(B.cx1, rn_int(__fmaf_rn(tb, P.inv_cs[0], P.khi[0])));
             if (c0 <= c1) {
               j = pool_a + 4u * lds_u16(rowp + 2u * (unsigned)c0);
               e = pool_a + 4u * lds_u16(rowp + 2u * (unsigned)c1 + 2u);
@@ -695,9 +755,25 @@ k_brick(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ cell_
 
       // ---------------- TEST: up to two grains of the pending run ----------------
       if (j < e) {
-        test_grain(j);
-        j += 4u;
-        if (j < e) { test_grain(j); j += 4u; }
+        const unsigned g0 = lds_u32(j), g1 = lds_u32_off4(j);   // g1 may lie beyond the run (still inside the pool)
+        const bool two = j + 4u < e;
+        float v0x, v0y, v0z, v1x, v1y, v1z;
+        const float s0 = tube_s(g0, v0x, v0y, v0z), s1 = tube_s(g1, v1x, v1y, v1z);
+        bool in0 = s0 <= Tlo, in1 = s1 <= Tlo;
+        if ((s0 > Tlo && s0 <= Thi) || (s1 > Tlo && s1 <= Thi)) {      // inside the error band: the exact predicate
+          if (s0 > Tlo && s0 <= Thi) in0 = exact_in(v0x, v0y, v0z);
+          if (s1 > Tlo && s1 <= Thi) in1 = exact_in(v1x, v1y, v1z);
+        }
+        in1 = in1 && two;
+        if (kMode == kVote) {
+          count += (int)in0 + (int)in1;
+        } else if (in0 || in1) {
+          // slot of the grain in the brick + (sorted position - slot) of the first grain of its row -> row of the grain
+          const int pos = (int)((j - pool_a) >> 2) + (int)lds_u32(rowp + delta_o);
+          if (in0) { const int row = __ldg(&sorted[pos].w); atomicMax(keyA + row, ka); atomicMax(keyB + row, kb); }
+          if (in1) { const int row = __ldg(&sorted[pos + 1].w); atomicMax(keyA + row, ka); atomicMax(keyB + row, kb); }
+        }
+        j += 8u;
       }
     }
     n_tests += item_tests >> 2;
@@ -708,7 +784,9 @@ k_brick(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ cell_
 }
 
 // ---------------------------------------------------------------------------------------------
-// A4: candidates = seeds with n_tube >= min_grains, grouped by view.  grid = (blocks, views of chunk).
+// A4: candidates = seeds with n_tube >= min_grains, grouped by (view, frame).  grid = (blocks, groups of
+// the chunk).  A warp takes 1024 consecutive seeds at a time, counts its candidates with ballots (keeping
+// every lane's 32 flags in a register) and makes ONE atomicAdd on the group's counter per 1024 seeds.
 template <int kFill>
 __global__ void __launch_bounds__(256)
 k_cands(EmuDev P, int v0, const FindCtl* __restrict__ ctl, const unsigned* __restrict__ view_seed_off,
@@ -716,31 +794,43 @@ k_cands(EmuDev P, int v0, const FindCtl* __restrict__ ctl, const unsigned* __res
         unsigned* __restrict__ view_cand_cnt, const unsigned* __restrict__ view_cand_off,
         Cand* __restrict__ cands, int4* __restrict__ cand_geo, unsigned long long* __restrict__ counts) {
   if (ctl->skip || ctl->generic) return;
-  const int vl = blockIdx.y, lane = threadIdx.x & 31;
-  const unsigned lo = view_seed_off[vl], hi = view_seed_off[vl + 1];
-  const unsigned span = gridDim.x * blockDim.x;
+  const int vf = blockIdx.y, lane = threadIdx.x & 31;
+  const unsigned lo = view_seed_off[vf], hi = view_seed_off[vf + 1];
+  const unsigned wpb = blockDim.x >> 5;
+  const unsigned span = gridDim.x * wpb * 1024u;
   unsigned status = 0;
-  for (unsigned i0 = lo + blockIdx.x * blockDim.x + (threadIdx.x & ~31u); i0 < hi; i0 += span) {
-    const unsigned i = i0 + lane;
-    const unsigned n = (i < hi) ? seed_cnt[i] : 0u;
-    const bool is = n >= (unsigned)P.min_grains;
-    const unsigned m = __ballot_sync(EMU_FULL, is);
-    if (!m) continue;
+  for (unsigned c0 = lo + (blockIdx.x * wpb + (threadIdx.x >> 5)) * 1024u; c0 < hi; c0 += span) {
+    unsigned flags = 0, total = 0;
+#pragma unroll 4
+    for (int it = 0; it < 32; ++it) {
+      const unsigned i = c0 + (unsigned)it * 32u + (unsigned)lane;
+      const bool is = (i < hi) && seed_cnt[i] >= (unsigned)P.min_grains;
+      flags |= (unsigned)is << it;
+      total += __popc(__ballot_sync(EMU_FULL, is));
+    }
+    if (!total) continue;
     unsigned base = 0;
-    if (lane == 0) base = atomicAdd(view_cand_cnt + vl, (unsigned)__popc(m));
+    if (lane == 0) base = atomicAdd(view_cand_cnt + vf, total);
     if (!kFill) continue;
-    base = __shfl_sync(EMU_FULL, base, 0);
-    if (is) {
-      const unsigned ci = view_cand_off[vl] + base + (unsigned)__popc(m & ((1u << lane) - 1u));
-      int4 g = geo[i];
-      const int2 p = ab[i];
-      int dx, dy, dz;
-      geo_d(g, dx, dy, dz);
-      if (n > (unsigned)kMaxTube) status |= EMU_ST_RANGE;
-      Cand c; c.a = p.x; c.b = p.y; c.n_tube_view = (int)min(n, 0xffffu) | (vl << 16); c.d2 = dx * dx + dy * dy + dz * dz;
-      cands[ci] = c;
-      g.y = (int)(((unsigned)g.y & 0xffffu) | (min(n, (unsigned)kMaxTube) << 16));
-      cand_geo[ci] = g;
+    base = __shfl_sync(EMU_FULL, base, 0) + view_cand_off[vf];
+    for (int it = 0; it < 32; ++it) {
+      const bool is = (flags >> it) & 1u;
+      const unsigned m = __ballot_sync(EMU_FULL, is);
+      if (is) {
+        const unsigned i = c0 + (unsigned)it * 32u + (unsigned)lane;
+        const unsigned ci = base + (unsigned)__popc(m & ((1u << lane) - 1u));
+        const unsigned n = seed_cnt[i];
+        int4 g = geo[i];
+        const int2 p = ab[i];
+        int dx, dy, dz;
+        geo_d(g, dx, dy, dz);
+        if (n > (unsigned)kMaxTube) status |= EMU_ST_RANGE;
+        Cand c; c.a = p.x; c.b = p.y; c.n_tube_view = (int)min(n, 0xffffu) | ((vf / 3) << 16); c.d2 = dx * dx + dy * dy + dz * dz;
+        cands[ci] = c;
+        g.y = (int)(((unsigned)g.y & 0xffffu) | (min(n, (unsigned)kMaxTube) << 16));
+        cand_geo[ci] = g;
+      }
+      base += __popc(m);
     }
   }
   if (kFill && __any_sync(EMU_FULL, status != 0) && lane == 0) atomicOr(counts + EMU_CNT_STATUS, (unsigned long long)EMU_ST_RANGE);
@@ -752,13 +842,13 @@ k_seed_dump(int v0, const FindCtl* __restrict__ ctl, const int4* __restrict__ so
             const unsigned* __restrict__ view_seed_off, const unsigned* __restrict__ seed_cnt,
             const int2* __restrict__ ab, int4* __restrict__ dump, long long dump_cap) {
   if (ctl->skip || ctl->generic) return;
-  const int vl = blockIdx.y;
-  const unsigned lo = view_seed_off[vl], hi = view_seed_off[vl + 1];
+  const int vf = blockIdx.y;
+  const unsigned lo = view_seed_off[vf], hi = view_seed_off[vf + 1];
   for (unsigned i = lo + blockIdx.x * blockDim.x + threadIdx.x; i < hi; i += gridDim.x * blockDim.x) {
     if ((long long)i >= dump_cap) continue;
     const int2 p = ab[i];
     const int ra = sorted[p.x].w, rb = sorted[p.y].w;
-    dump[i] = make_int4(v0 + vl, min(ra, rb), max(ra, rb), (int)seed_cnt[i]);
+    dump[i] = make_int4(v0 + vf / 3, min(ra, rb), max(ra, rb), (int)seed_cnt[i]);
   }
 }
 
@@ -878,7 +968,7 @@ __global__ void k_cands_finish(FindCtl* ctl, unsigned cand_cap, unsigned long lo
 // A5 with the generic walker.  kPass 0: priority maximum (only when the chunk runs generic).
 // kPass 1: settlement of ties - every candidate whose (n_tube, D2) is flagged in the tie bitmap walks
 // its tube again and competes for the tied grains by (kmin, kmax) with a CAS-min.
-//   keyA = K1 << 29 | (mask - ci)   keyB = K1 << 29 | ci,   K1 = n_tube << 22 | D2.
+//   keyA = K1 << 29 | (mask - ci)   keyB = K1 << 29 | ci,   K1 = n_tube << 22 | D2, both indexed by ROW.
 // The top K1 of a grain is unique; keyA and keyB then name the same candidate unless several
 // candidates tie on K1 for that grain.
 __device__ __forceinline__ unsigned tie_hash(unsigned long long k1, int vl) {
@@ -913,10 +1003,11 @@ k_assoc_generic(EmuDev P, const int4* __restrict__ sorted, const int* __restrict
       const unsigned long long ka = (k1 << kCiBits) | (unsigned long long)(kCiMask - ci);
       const unsigned long long kb = (k1 << kCiBits) | (unsigned long long)ci;
       emu_walk_tube(P, bb, sorted, cell_start, v * P.ncell, A.x, A.y, A.z, dx, dy, dz, (long long)P.r2 * c.d2,
-                    [&](int g) { atomicMax(keyA + g, ka); atomicMax(keyB + g, kb); });
+                    [&](int j) { const int g = sorted[j].w; atomicMax(keyA + g, ka); atomicMax(keyB + g, kb); });
     } else {
       emu_walk_tube(P, bb, sorted, cell_start, v * P.ncell, A.x, A.y, A.z, dx, dy, dz, (long long)P.r2 * c.d2,
-                    [&](int g) {
+                    [&](int j) {
+                      const int g = sorted[j].w;                 // keys and owners are indexed by row
                       if ((keyA[g] >> kCiBits) != k1) return;
                       unsigned cur = owner[g];
                       while (cur == kNone || (cur != ci && cand_kless(sorted, c, cands[cur]))) {
@@ -1107,7 +1198,7 @@ k_member_scatter(const int4* __restrict__ sorted, const int* __restrict__ view_o
     if (t == kNone) continue;
     int k = atomicAdd(cursor + (t - t0), 1);
     long long pos = (long long)tracks[t].member_off + k;
-    if (pos < members_capacity) members[pos] = sorted[g].w;
+    if (pos < members_capacity) members[pos] = g;                // g is a row
   }
 }
 
@@ -1160,6 +1251,7 @@ struct FindWs {
   FindCtl* ctl; unsigned* tie_bits; unsigned long long* dump_cursor;
   unsigned* view_seed_tot; unsigned* view_seed_off; unsigned* view_cand_cnt; unsigned* view_cand_off;
   int* view_ntracks; unsigned* view_tracks; Brick* bricks;
+  int4* sortedF[3]; int* cell_startF[3]; void* bin_ws; size_t bin_ws_bytes;     // frames 1, 2 (0 = the caller's)
   int4* geo; int2* ab; unsigned* seed_cnt;
   Cand* cands; int4* cand_geo; int* wins; unsigned* cand_track;
   size_t seed_cap, cand_cap, brick_cap; int views_per_chunk;
@@ -1169,39 +1261,50 @@ constexpr size_t kSeedBytes = sizeof(int4) + sizeof(int2) + sizeof(unsigned);   
 constexpr size_t kCandBytes = sizeof(Cand) + sizeof(int4) + sizeof(int) + sizeof(unsigned);      // 40
 constexpr size_t kMinSeedCap = 1u << 20, kMinCandCap = 1u << 16;
 
-size_t bricks_per_view(const EmuDev& P, const Tiling& T) { return (size_t)T.tx * T.ty * (size_t)P.n[2]; }
+size_t bricks_per_view(const EmuDev& P, const Tilings& TT) {
+  size_t n = 0;
+  for (int f = 0; f < 3; ++f) n += (size_t)TT.t[f].tx * TT.t[f].ty * (size_t)P.fr[f].n[2];
+  return n;
+}
 
-size_t fixed_bytes(const EmuDev& P, const Tiling& T, int64_t n_grains, int32_t n_views, int vpc) {
+size_t fixed_bytes(const EmuDev& P, const Tilings& TT, int64_t n_grains, int32_t n_views, int vpc) {
   size_t b = 0;
   b += emu_align256((size_t)n_views * sizeof(EmuBox));
   b += 2 * emu_align256((size_t)n_grains * sizeof(unsigned long long));
-  b += 2 * emu_align256((size_t)n_grains * sizeof(unsigned));
+  b += emu_align256((size_t)n_grains * sizeof(unsigned));                   // owner
+  b += emu_align256(3 * (size_t)n_grains * sizeof(unsigned));               // seed_off, one plane per frame
   b += emu_align256(sizeof(FindCtl)) + emu_align256(kTieBits / 8) + 256;
-  b += 4 * emu_align256(((size_t)vpc + 1) * sizeof(unsigned));
+  b += 4 * emu_align256((3 * (size_t)vpc + 1) * sizeof(unsigned));
   b += emu_align256((size_t)vpc * sizeof(int));
   b += emu_align256((size_t)vpc * P.max_tracks * sizeof(unsigned));
-  b += emu_align256((size_t)vpc * bricks_per_view(P, T) * sizeof(Brick));
+  b += emu_align256((size_t)vpc * bricks_per_view(P, TT) * sizeof(Brick));
+  for (int f = 1; f < 3; ++f) {                                             // the binnings of frames 1 and 2
+    b += emu_align256((size_t)n_grains * sizeof(int4));
+    b += emu_align256(((size_t)n_views * P.fr[f].ncell + 1) * sizeof(int));
+  }
+  b += emu_align256(emu_bin_ws_bytes(P, n_grains, n_views));
   return b + 256;
 }
 
-// Tiles per view: the fewest tiles (every seed is streamed past every brick of its view) for which an
-// average tile - 1.35 x its share of the grains, its rows and its cells over the whole z extent - fits the
-// shared-memory pool; among the factorisations of that count the squarest in physical size.  k_plan cuts
-// a tile that turns out too full into runs of z layers.
-Tiling choose_tiling(const EmuDev& P, int64_t n_grains, int32_t n_views) {
+// Tiles per (view, frame): the fewest tiles (every seed is streamed past every brick of its view and frame)
+// for which an average tile - 1.35 x its share of the grains, its rows and its cells over the whole w extent -
+// fits the shared-memory pool; among the factorisations of that count the squarest in physical size.
+// k_plan cuts a tile that turns out too full into runs of w layers.
+Tiling choose_tiling(const EmuDev& P, int f, int64_t n_grains, int32_t n_views) {
+  const int* n = P.fr[f].n;
   const double avg = n_views > 0 ? (double)n_grains / n_views : 0.0;
-  Tiling fallback; fallback.tx = P.n[0]; fallback.ty = P.n[1]; fallback.w = 1; fallback.h = 1;   // one column per tile
-  const int64_t max_t = emu_min64((int64_t)P.n[0] * P.n[1], 8192);
+  Tiling fallback; fallback.tx = n[0]; fallback.ty = n[1]; fallback.w = 1; fallback.h = 1;   // one column per tile
+  const int64_t max_t = emu_min64((int64_t)n[0] * n[1], 8192);
   for (int64_t t = 1; t <= max_t; ++t) {
     Tiling best; best.tx = best.ty = best.w = best.h = 0;
     double best_score = -1.0;
     for (int64_t tx = 1; tx <= t; ++tx) {
       if (t % tx) continue;
       const int64_t ty = t / tx;
-      if (tx > P.n[0] || ty > P.n[1]) continue;
-      const int w = (int)((P.n[0] + tx - 1) / tx), h = (int)((P.n[1] + ty - 1) / ty);
-      const double grains = 1.35 * avg * ((double)w * h) / ((double)P.n[0] * P.n[1]) + 64.0;
-      if (brick_bytes((long long)grains, (long long)h * P.n[2], w) > kPoolBytes) continue;
+      if (tx > n[0] || ty > n[1]) continue;
+      const int w = (int)((n[0] + tx - 1) / tx), h = (int)((n[1] + ty - 1) / ty);
+      const double grains = 1.35 * avg * ((double)w * h) / ((double)n[0] * n[1]) + 64.0;
+      if (brick_bytes((long long)grains, (long long)h * n[2], w) > kPoolBytes) continue;
       const double sx = (double)w * P.cs[0], sy = (double)h * P.cs[1];
       const double score = sx < sy ? sx / sy : sy / sx;
       if (score > best_score) { best_score = score; best.tx = (int)tx; best.ty = (int)ty; best.w = w; best.h = h; }
@@ -1211,39 +1314,46 @@ Tiling choose_tiling(const EmuDev& P, int64_t n_grains, int32_t n_views) {
   return fallback;
 }
 
+Tilings choose_tilings(const EmuDev& P, int64_t n_grains, int32_t n_views) {
+  Tilings TT;
+  for (int f = 0; f < 3; ++f) TT.t[f] = choose_tiling(P, f, n_grains, n_views);
+  return TT;
+}
+
 struct Hints { int seeds_per_grain, cand_per_grain; };
 
 }  // namespace
 
 size_t emu_find_ws_min_bytes(const EmuDev& P, int64_t n_grains, int32_t n_views) {
-  Tiling T = choose_tiling(P, n_grains, n_views);
-  return fixed_bytes(P, T, n_grains, n_views, 1) + kMinSeedCap * kSeedBytes + kMinCandCap * kCandBytes + 8 * 256;
+  Tilings TT = choose_tilings(P, n_grains, n_views);
+  return fixed_bytes(P, TT, n_grains, n_views, 1) + kMinSeedCap * kSeedBytes + kMinCandCap * kCandBytes + 8 * 256;
 }
 
 size_t emu_find_ws_recommended_bytes(const EmuDev& P, int64_t n_grains, int32_t n_views, int seeds_per_grain,
                                      int cand_per_grain) {
-  Tiling T = choose_tiling(P, n_grains, n_views);
+  Tilings TT = choose_tilings(P, n_grains, n_views);
   const int64_t per_view_g = emu_max64(1, (n_grains + emu_max64(1, n_views) - 1) / emu_max64(1, n_views));
   const int64_t spv = per_view_g * seeds_per_grain, cpv = per_view_g * cand_per_grain;
   const int64_t per_view_bytes = spv * (int64_t)kSeedBytes + cpv * (int64_t)kCandBytes;
   // as many views per chunk as fit 24 GiB of seed / candidate storage (at least one)
   int64_t vpc = emu_max64(1, emu_min64(emu_max64(1, n_views), ((int64_t)24 << 30) / emu_max64(1, per_view_bytes)));
-  vpc = emu_min64(vpc, 65535);
+  vpc = emu_min64(vpc, 21000);
   const size_t seed_cap = (size_t)emu_max64((int64_t)kMinSeedCap, spv * vpc);
   const size_t cand_cap = (size_t)emu_max64((int64_t)kMinCandCap, cpv * vpc);
-  return fixed_bytes(P, T, n_grains, n_views, (int)vpc) + seed_cap * kSeedBytes + cand_cap * kCandBytes + 16 * 256;
+  return fixed_bytes(P, TT, n_grains, n_views, (int)vpc) + seed_cap * kSeedBytes + cand_cap * kCandBytes + 16 * 256;
 }
 
-static int carve(const EmuDev& P, const Tiling& T, Hints hints, int64_t n_grains, int32_t n_views, void* d_ws,
+static int carve(const EmuDev& P, const Tilings& TT, Hints hints, int64_t n_grains, int32_t n_views, void* d_ws,
                  size_t ws_bytes, FindWs& W) {
   if (ws_bytes < emu_find_ws_min_bytes(P, n_grains, n_views)) return EMU_ERR_CAPACITY;
   const int64_t per_view_g = emu_max64(1, (n_grains + emu_max64(1, n_views) - 1) / emu_max64(1, n_views));
   const int64_t spv = per_view_g * hints.seeds_per_grain, cpv = per_view_g * hints.cand_per_grain;
   // views per chunk: the most whose expected seeds and candidates fit what is left after the fixed part
-  int vpc = n_views > 0 ? (int)emu_min64(n_views, 65535) : 1;
+  // (3 groups per view must fit the 65 535 blocks of grid.y)
+  int vpc = n_views > 0 ? (int)emu_min64(n_views, 21000) : 1;
   size_t seed_cap = 0, cand_cap = 0;
   for (;;) {
-    const size_t fx = fixed_bytes(P, T, n_grains, n_views, vpc) + 16 * 256;
+    const size_t fx = fixed_bytes(P, TT, n_grains, n_views, vpc) + 16 * 256;
     if (fx + kMinSeedCap * kSeedBytes + kMinCandCap * kCandBytes <= ws_bytes) {
       const size_t avail = ws_bytes - fx;
       // what is available is split between seeds and candidates in the proportion of the hints
@@ -1264,18 +1374,25 @@ static int carve(const EmuDev& P, const Tiling& T, Hints hints, int64_t n_grains
   W.keyA = (unsigned long long*)take((size_t)n_grains * sizeof(unsigned long long));
   W.keyB = (unsigned long long*)take((size_t)n_grains * sizeof(unsigned long long));
   W.owner = (unsigned*)take((size_t)n_grains * sizeof(unsigned));
-  W.seed_off = (unsigned*)take((size_t)n_grains * sizeof(unsigned));
+  W.seed_off = (unsigned*)take(3 * (size_t)n_grains * sizeof(unsigned));
   W.ctl = (FindCtl*)take(sizeof(FindCtl));
   W.tie_bits = (unsigned*)take(kTieBits / 8);
   W.dump_cursor = (unsigned long long*)take(256);
-  W.view_seed_tot = (unsigned*)take(((size_t)vpc + 1) * sizeof(unsigned));
-  W.view_seed_off = (unsigned*)take(((size_t)vpc + 1) * sizeof(unsigned));
-  W.view_cand_cnt = (unsigned*)take(((size_t)vpc + 1) * sizeof(unsigned));
-  W.view_cand_off = (unsigned*)take(((size_t)vpc + 1) * sizeof(unsigned));
+  W.view_seed_tot = (unsigned*)take((3 * (size_t)vpc + 1) * sizeof(unsigned));
+  W.view_seed_off = (unsigned*)take((3 * (size_t)vpc + 1) * sizeof(unsigned));
+  W.view_cand_cnt = (unsigned*)take((3 * (size_t)vpc + 1) * sizeof(unsigned));
+  W.view_cand_off = (unsigned*)take((3 * (size_t)vpc + 1) * sizeof(unsigned));
   W.view_ntracks = (int*)take((size_t)vpc * sizeof(int));
   W.view_tracks = (unsigned*)take((size_t)vpc * P.max_tracks * sizeof(unsigned));
-  W.brick_cap = (size_t)vpc * bricks_per_view(P, T);
+  W.brick_cap = (size_t)vpc * bricks_per_view(P, TT);
   W.bricks = (Brick*)take(W.brick_cap * sizeof(Brick));
+  W.sortedF[0] = nullptr; W.cell_startF[0] = nullptr;
+  for (int f = 1; f < 3; ++f) {
+    W.sortedF[f] = (int4*)take((size_t)n_grains * sizeof(int4));
+    W.cell_startF[f] = (int*)take(((size_t)n_views * P.fr[f].ncell + 1) * sizeof(int));
+  }
+  W.bin_ws_bytes = emu_bin_ws_bytes(P, n_grains, n_views);
+  W.bin_ws = take(W.bin_ws_bytes);
   W.geo = (int4*)take(seed_cap * sizeof(int4));
   W.ab = (int2*)take(seed_cap * sizeof(int2));
   W.seed_cnt = (unsigned*)take(seed_cap * sizeof(unsigned));
@@ -1301,40 +1418,60 @@ static int sm_count() {
 
 #define EMU_CK(x) do { if ((x) != cudaSuccess) return EMU_ERR_CUDA; } while (0)
 
-static int choose_slices(const Tiling& T, int nv, int n_sm) {
+static int choose_slices(const Tilings& TT, int nv, int n_sm) {
   // enough work items that every SM gets several even when the chunk holds few views
-  const int64_t bricks = emu_max64(1, (int64_t)nv * T.tx * T.ty);
+  int64_t bricks = 0;
+  for (int f = 0; f < 3; ++f) bricks += (int64_t)nv * TT.t[f].tx * TT.t[f].ty;
+  bricks = emu_max64(1, bricks);
   int64_t s = (4 * (int64_t)n_sm + bricks - 1) / bricks;
   if (s < 1) s = 1;
   if (s > 256) s = 256;
   return (int)s;
 }
 
+// once per call: bounding boxes, and the binnings of frames 1 and 2 from frame 0's (the caller's) output
+static int prepare_frames(const EmuDev& P, FindWs& W, FramePtrs& F, const int32_t* d_sorted, const int32_t* d_cell_start,
+                          const int32_t* d_view_off, int64_t n_grains, int32_t n_views, int kSM, cudaStream_t st) {
+  const int n = (int)n_grains;
+  EMU_LAUNCH(EMU_STAGE_PREP, st, k_bbox_init<<<grid_for(n_views, 256, 1 << 20), 256, 0, st>>>(W.bbox, n_views));
+  EMU_LAUNCH(EMU_STAGE_PREP, st, k_bbox<<<grid_for(n, 256, kSM * 8), 256, 0, st>>>((const int4*)d_sorted, d_view_off, n_views, n, W.bbox));
+  F.sorted[0] = (const int4*)d_sorted; F.cell_start[0] = d_cell_start;
+  for (int f = 1; f < 3; ++f) {
+    F.sorted[f] = W.sortedF[f]; F.cell_start[f] = W.cell_startF[f];
+    if (!P.packed_ok) continue;                        // every chunk will take the generic kernels (frame 0 only)
+    int rc = emu_bin_launch(P, f, d_sorted, d_view_off, n_grains, n_views, (int32_t*)W.sortedF[f], W.cell_startF[f],
+                            nullptr, W.bin_ws, W.bin_ws_bytes, st);
+    if (rc != EMU_OK) return rc;
+  }
+  return EMU_OK;
+}
+
 // seeds + votes of the chunk [v0, v1): leaves geo / ab / seed_cnt / view_seed_off filled (brick path), or
 // ctl->generic set
-static int vote_chunk(const EmuDev& P, const Tiling& T, FindWs& W, const int4* sorted, const int32_t* d_cell_start,
-                      const int32_t* d_view_off, int v0, int v1, int slices, int kSM, unsigned long long* counts,
-                      cudaStream_t st) {
+static int vote_chunk(const EmuDev& P, const Tilings& TT, FindWs& W, const FramePtrs& F, const int32_t* d_view_off,
+                      int64_t n_grains, int v0, int v1, int slices, int kSM, unsigned long long* counts, cudaStream_t st) {
   const int nv = v1 - v0;
+  const int4* sorted = F.sorted[0];
+  const int* d_cell_start = F.cell_start[0];
+  const size_t plane = (size_t)n_grains;
   EMU_CK(cudaMemsetAsync(W.ctl, 0, sizeof(FindCtl), st));
-  EMU_CK(cudaMemsetAsync(W.view_cand_cnt, 0, ((size_t)nv + 1) * sizeof(unsigned), st));
+  EMU_CK(cudaMemsetAsync(W.view_cand_cnt, 0, (3 * (size_t)nv + 1) * sizeof(unsigned), st));
   EMU_LAUNCH(EMU_STAGE_SEEDS, st, k_seed_pairs<0><<<kSM * 16, kVoteThreads, 0, st>>>(
-      P, sorted, d_cell_start, d_view_off, v0, v1, W.seed_off, nullptr, W.ctl, nullptr, nullptr, counts));
-  EMU_LAUNCH(EMU_STAGE_SEEDS, st, k_view_scan<<<grid_for(nv, 1, kSM * 2), 1024, 0, st>>>(
-      d_view_off, v0, v1, W.seed_off, W.view_seed_tot, counts));
+      P, sorted, d_cell_start, d_view_off, v0, v1, W.seed_off, plane, nullptr, W.ctl, nullptr, nullptr, counts));
+  EMU_LAUNCH(EMU_STAGE_SEEDS, st, k_view_scan<<<grid_for(3 * nv, 1, kSM * 2), 1024, 0, st>>>(
+      d_view_off, v0, v1, W.seed_off, plane, W.view_seed_tot, counts));
   EMU_LAUNCH(EMU_STAGE_SEEDS, st, k_chunk_offsets<<<1, 1024, 0, st>>>(
-      nv, W.view_seed_tot, W.view_seed_off, &W.ctl->seed_count, (unsigned)W.seed_cap, (unsigned)EMU_ST_SEED_OVERFLOW,
+      3 * nv, W.view_seed_tot, W.view_seed_off, &W.ctl->seed_count, (unsigned)W.seed_cap, (unsigned)EMU_ST_SEED_OVERFLOW,
       W.ctl, counts, EMU_CNT_SEEDS));
   EMU_LAUNCH(EMU_STAGE_SEEDS, st, k_seed_pairs<1><<<kSM * 16, kVoteThreads, 0, st>>>(
-      P, sorted, d_cell_start, d_view_off, v0, v1, W.seed_off, W.view_seed_off, W.ctl, W.geo, W.ab, counts));
+      P, sorted, d_cell_start, d_view_off, v0, v1, W.seed_off, plane, W.view_seed_off, W.ctl, W.geo, W.ab, counts));
   EMU_CK(cudaMemsetAsync(W.seed_cnt, 0, W.seed_cap * sizeof(unsigned), st));
-  EMU_LAUNCH(EMU_STAGE_PREP, st, k_plan<<<grid_for(nv, 4, 1 << 20), 128, 0, st>>>(
-      P, T, d_cell_start, W.bbox, v0, v1, W.bricks, (unsigned)W.brick_cap, W.ctl));
+  EMU_LAUNCH(EMU_STAGE_PREP, st, k_plan<<<grid_for(3 * nv, 4, 1 << 20), 128, 0, st>>>(
+      P, TT, F, W.bbox, v0, v1, W.bricks, (unsigned)W.brick_cap, W.ctl));
   EMU_LAUNCH(EMU_STAGE_PREP, st, k_plan_finish<<<1, 1, 0, st>>>(W.ctl, (unsigned)W.brick_cap));
   EMU_CK(cudaFuncSetAttribute(k_brick<kVote>, cudaFuncAttributeMaxDynamicSharedMemorySize, kPoolBytes));
   EMU_LAUNCH(EMU_STAGE_VOTE, st, k_brick<kVote><<<kSM, kBrickThreads, kPoolBytes, st>>>(
-      P, sorted, d_cell_start, v0, W.bricks, W.ctl, slices, W.geo, W.view_seed_off, W.seed_cnt, nullptr, nullptr,
-      counts));
+      P, F, v0, W.bricks, W.ctl, slices, W.geo, W.view_seed_off, W.seed_cnt, nullptr, nullptr, counts));
   return EMU_OK;
 }
 
@@ -1343,38 +1480,38 @@ int emu_find_launch(const EmuDev& P, int seeds_per_grain, int cand_per_grain, co
                     emu_track* d_tracks, int32_t* d_track_off, int32_t* d_members, int64_t members_capacity,
                     int64_t* d_counts, void* d_ws, size_t ws_bytes, cudaStream_t st) {
   FindWs W;
-  const Tiling T = choose_tiling(P, n_grains, n_views);
+  const Tilings TT = choose_tilings(P, n_grains, n_views);
   Hints hints; hints.seeds_per_grain = seeds_per_grain; hints.cand_per_grain = cand_per_grain;
-  int rc = carve(P, T, hints, n_grains, n_views, d_ws, ws_bytes, W);
+  int rc = carve(P, TT, hints, n_grains, n_views, d_ws, ws_bytes, W);
   if (rc != EMU_OK) return rc;
   const int4* sorted = (const int4*)d_sorted;
   unsigned long long* counts = (unsigned long long*)d_counts;
-  const int n = (int)n_grains;
   const int kSM = sm_count();
   EMU_CK(cudaMemsetAsync(d_counts, 0, 8 * sizeof(int64_t), st));
   EMU_CK(cudaMemsetAsync(d_track_off, 0, ((size_t)n_views + 1) * sizeof(int32_t), st));
   EMU_CK(cudaMemsetAsync(W.keyA, 0, (size_t)n_grains * sizeof(unsigned long long), st));
   EMU_CK(cudaMemsetAsync(W.keyB, 0, (size_t)n_grains * sizeof(unsigned long long), st));
   EMU_CK(cudaMemsetAsync(W.owner, 0xff, (size_t)n_grains * sizeof(unsigned), st));
-  EMU_LAUNCH(EMU_STAGE_PREP, st, k_bbox_init<<<grid_for(n_views, 256, 1 << 20), 256, 0, st>>>(W.bbox, n_views));
-  EMU_LAUNCH(EMU_STAGE_PREP, st, k_bbox<<<grid_for(n, 256, kSM * 8), 256, 0, st>>>(sorted, d_view_off, n_views, n, W.bbox));
+  FramePtrs F;
+  rc = prepare_frames(P, W, F, d_sorted, d_cell_start, d_view_off, n_grains, n_views, kSM, st);
+  if (rc != EMU_OK) return rc;
 
   for (int v0 = 0; v0 < n_views; v0 += W.views_per_chunk) {
     const int v1 = (int)emu_min64(n_views, (int64_t)v0 + W.views_per_chunk);
     const int nv = v1 - v0;
-    const int slices = choose_slices(T, nv, kSM);
+    const int slices = choose_slices(TT, nv, kSM);
     EMU_CK(cudaMemsetAsync(W.view_ntracks, 0, (size_t)nv * sizeof(int), st));
     EMU_CK(cudaMemsetAsync(W.tie_bits, 0, kTieBits / 8, st));
-    rc = vote_chunk(P, T, W, sorted, d_cell_start, d_view_off, v0, v1, slices, kSM, counts, st);
+    rc = vote_chunk(P, TT, W, F, d_view_off, n_grains, v0, v1, slices, kSM, counts, st);
     if (rc != EMU_OK) return rc;
-    // A4: candidates grouped by view
-    EMU_LAUNCH(EMU_STAGE_CANDS, st, k_cands<0><<<dim3(64, nv), 256, 0, st>>>(
+    // A4: candidates grouped by (view, frame)
+    EMU_LAUNCH(EMU_STAGE_CANDS, st, k_cands<0><<<dim3(16, 3 * nv), 256, 0, st>>>(
         P, v0, W.ctl, W.view_seed_off, W.seed_cnt, W.geo, W.ab, W.view_cand_cnt, nullptr, nullptr, nullptr, counts));
     EMU_LAUNCH(EMU_STAGE_CANDS, st, k_chunk_offsets<<<1, 1024, 0, st>>>(
-        nv, W.view_cand_cnt, W.view_cand_off, &W.ctl->cand_count, (unsigned)W.cand_cap, (unsigned)EMU_ST_CAND_OVERFLOW,
+        3 * nv, W.view_cand_cnt, W.view_cand_off, &W.ctl->cand_count, (unsigned)W.cand_cap, (unsigned)EMU_ST_CAND_OVERFLOW,
         W.ctl, counts, EMU_CNT_CANDIDATES));
-    EMU_CK(cudaMemsetAsync(W.view_cand_cnt, 0, ((size_t)nv + 1) * sizeof(unsigned), st));
-    EMU_LAUNCH(EMU_STAGE_CANDS, st, k_cands<1><<<dim3(64, nv), 256, 0, st>>>(
+    EMU_CK(cudaMemsetAsync(W.view_cand_cnt, 0, (3 * (size_t)nv + 1) * sizeof(unsigned), st));
+    EMU_LAUNCH(EMU_STAGE_CANDS, st, k_cands<1><<<dim3(16, 3 * nv), 256, 0, st>>>(
         P, v0, W.ctl, W.view_seed_off, W.seed_cnt, W.geo, W.ab, W.view_cand_cnt, W.view_cand_off, W.cands, W.cand_geo,
         counts));
     // generic fallback for the whole chunk (returns at once unless the brick plan failed)
@@ -1386,8 +1523,7 @@ int emu_find_launch(const EmuDev& P, int seeds_per_grain, int cand_per_grain, co
     // A5
     EMU_CK(cudaFuncSetAttribute(k_brick<kAssoc>, cudaFuncAttributeMaxDynamicSharedMemorySize, kPoolBytes));
     EMU_LAUNCH(EMU_STAGE_ASSOC, st, k_brick<kAssoc><<<kSM, kBrickThreads, kPoolBytes, st>>>(
-        P, sorted, d_cell_start, v0, W.bricks, W.ctl, slices, W.cand_geo, W.view_cand_off, nullptr, W.keyA, W.keyB,
-        counts));
+        P, F, v0, W.bricks, W.ctl, slices, W.cand_geo, W.view_cand_off, nullptr, W.keyA, W.keyB, counts));
     EMU_LAUNCH(EMU_STAGE_ASSOC, st, k_assoc_generic<0><<<kSM * 16, kVoteThreads, 0, st>>>(
         P, sorted, d_cell_start, W.bbox, v0, W.cands, W.ctl, W.tie_bits, W.keyA, W.keyB, W.owner));
     EMU_LAUNCH(EMU_STAGE_ASSOC, st, k_tie_detect<<<kSM * 4, 256, 0, st>>>(d_view_off, v0, v1, W.keyA, W.keyB, W.ctl, W.tie_bits));
@@ -1413,23 +1549,23 @@ int emu_count_seeds_launch(const EmuDev& P, int seeds_per_grain, int cand_per_gr
                            int32_t* d_seed_dump, int64_t dump_capacity, int64_t* d_counts, void* d_ws, size_t ws_bytes,
                            cudaStream_t st) {
   FindWs W;
-  const Tiling T = choose_tiling(P, n_grains, n_views);
+  const Tilings TT = choose_tilings(P, n_grains, n_views);
   Hints hints; hints.seeds_per_grain = seeds_per_grain; hints.cand_per_grain = cand_per_grain;
-  int rc = carve(P, T, hints, n_grains, n_views, d_ws, ws_bytes, W);
+  int rc = carve(P, TT, hints, n_grains, n_views, d_ws, ws_bytes, W);
   if (rc != EMU_OK) return rc;
   if (W.views_per_chunk < n_views) return EMU_ERR_CAPACITY;      // the per-seed dump is a one-chunk test aid
   const int4* sorted = (const int4*)d_sorted;
   unsigned long long* counts = (unsigned long long*)d_counts;
-  const int n = (int)n_grains;
   const int kSM = sm_count();
   EMU_CK(cudaMemsetAsync(d_counts, 0, 8 * sizeof(int64_t), st));
   EMU_CK(cudaMemsetAsync(W.dump_cursor, 0, 256, st));
-  EMU_LAUNCH(EMU_STAGE_PREP, st, k_bbox_init<<<grid_for(n_views, 256, 1 << 20), 256, 0, st>>>(W.bbox, n_views));
-  EMU_LAUNCH(EMU_STAGE_PREP, st, k_bbox<<<grid_for(n, 256, kSM * 8), 256, 0, st>>>(sorted, d_view_off, n_views, n, W.bbox));
+  FramePtrs F;
+  rc = prepare_frames(P, W, F, d_sorted, d_cell_start, d_view_off, n_grains, n_views, kSM, st);
+  if (rc != EMU_OK) return rc;
   if (n_views > 0) {
-    rc = vote_chunk(P, T, W, sorted, d_cell_start, d_view_off, 0, n_views, choose_slices(T, n_views, kSM), kSM, counts, st);
+    rc = vote_chunk(P, TT, W, F, d_view_off, n_grains, 0, n_views, choose_slices(TT, n_views, kSM), kSM, counts, st);
     if (rc != EMU_OK) return rc;
-    EMU_LAUNCH(EMU_STAGE_CANDS, st, k_seed_dump<<<dim3(64, n_views), 256, 0, st>>>(
+    EMU_LAUNCH(EMU_STAGE_CANDS, st, k_seed_dump<<<dim3(64, 3 * n_views), 256, 0, st>>>(
         0, W.ctl, sorted, W.view_seed_off, W.seed_cnt, W.ab, (int4*)d_seed_dump, dump_capacity));
     EMU_LAUNCH(EMU_STAGE_VOTE, st, k_vote_generic<true><<<kSM * 16, kVoteThreads, 0, st>>>(
         P, sorted, d_cell_start, d_view_off, W.bbox, 0, n_views, nullptr, 0, W.ctl, (int4*)d_seed_dump, dump_capacity,

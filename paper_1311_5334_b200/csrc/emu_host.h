@@ -29,7 +29,9 @@ void emu_prof_after(emu_profile* p, int stage, cudaStream_t st);
 
 // emu_bin.cu
 size_t emu_bin_ws_bytes(const EmuDev& P, int64_t n_grains, int32_t n_views);
-int emu_bin_launch(const EmuDev& P, const int32_t* d_grains, const int32_t* d_view_off, int64_t n_grains,
+// frame 0: the C ABI's A1 (w := row).  frames 1, 2: d_grains is frame 0's output (w = row is kept), the output
+// holds the grains in the frame's coordinates (emu_dev.cuh "Frames").
+int emu_bin_launch(const EmuDev& P, int frame, const int32_t* d_grains, const int32_t* d_view_off, int64_t n_grains,
                    int32_t n_views, int32_t* d_sorted, int32_t* d_cell_start, int64_t* d_status, void* d_ws,
                    size_t ws_bytes, cudaStream_t st);
 
