@@ -322,6 +322,7 @@ def main():
         "cm2_per_hour": V * world / (ms_step * 1e-3) * 3600 * VIEW_AREA_CM2,
         "grains_per_gpu": n, "seeds": seeds, "candidates": int(counts[E.EMU_CNT["candidates"]]),
         "tracks": int(counts[E.EMU_CNT["tracks"]]),
+        "tests_per_seed_gpu": float(counts[E.EMU_CNT["tests"]]) / max(1, seeds),
         "gpu_launches": int(sum(stage_launches.values())),
         "stage_ms_per_step": {k: v / args.steps for k, v in stage_ms.items()},
         "roofline": roofline, "roofline_bin": roofline_bin, "cpu_baseline": cpu, "e2e": e2e, "clocks": clocks,

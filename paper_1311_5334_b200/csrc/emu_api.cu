@@ -45,13 +45,13 @@ EmuDev make_dev(const emu_params* p) {
     d.klo[i] = -(d.Rw * d.inv_cs[i] + 0.5f);
     d.khi[i] = d.Rw * d.inv_cs[i] - 0.5f;
   }
-  // frames: cyclic permutations of the axes, the same cell size triple applied to (u,v,w)
+  // frames: permutations of the axes (emu_dev.cuh), the same cell size triple applied to (u,v,w)
   // 4-byte grains: u in 16 bits, v and w relative to their cell in 8 bits each (emu_find.cu)
   d.packed_ok = (d.cs[1] <= 256 && d.cs[2] <= 256) ? 1 : 0;
   for (int f = 0; f < 3; ++f) {
     int64_t fc = 1;
     for (int i = 0; i < 3; ++i) {
-      d.fr[f].n[i] = (p->view_size_q[(f + i) % 3] + d.cs[i] - 1) / d.cs[i];
+      d.fr[f].n[i] = (p->view_size_q[emu_frame_axis(f, i)] + d.cs[i] - 1) / d.cs[i];
       fc *= d.fr[f].n[i];
     }
     d.fr[f].ncell = fc > 0x7fffffff ? -1 : (int)fc;

@@ -36,9 +36,14 @@ struct EmuDev {           // passed by value to every kernel
   int packed_ok;          // 1: the 4-byte grain format of the brick kernels can hold a view of this grid
 };
 
+// lab axis of coordinate i of frame f
+__host__ __device__ __forceinline__ int emu_frame_axis(int f, int i) {
+  return f == 0 ? i : (f == 1 ? (i == 0 ? 1 : (i == 1 ? 0 : 2)) : (i == 0 ? 2 : i - 1));
+}
+
 // lab coordinates -> frame coordinates (w is carried along)
 __host__ __device__ __forceinline__ int4 emu_to_frame(int f, int4 g) {
-  if (f == 1) return make_int4(g.y, g.z, g.x, g.w);
+  if (f == 1) return make_int4(g.y, g.x, g.z, g.w);
   if (f == 2) return make_int4(g.z, g.x, g.y, g.w);
   return g;
 }

@@ -61,8 +61,19 @@ struct Cand {            // 16 B
 
 struct Brick {           // 48 B: cells [cx0..cx1] x [cy0..cy1] x [cz0..cz1] (frame coordinates u, v, w) of one
   int view, cx0, cx1, cy0, cy1, cz0, cz1, n;   // (view, frame), n grains
-  int frame, pad[3];
+  int frame;
+  int ord;               // ordinal of the brick inside its (view, frame): selects the hit record of a seed
+  int base;              // first entry of the brick in slot_row (brick slot -> row of the grain)
+  int pad;
 };
+
+// Hit records.  While it counts, the voting pass also writes down WHICH grains it found: every (seed, brick)
+// pair owns a record of kRecSlots 16-bit brick slots, and the 64-bit counter of the seed holds one 16-bit
+// field per brick ordinal.  The association pass (k_assoc_hits) then reads the records of the candidates
+// instead of walking their tubes again; a candidate with more than kRecSlots grains in one brick, or a
+// (view, frame) cut into more than kRecBricks bricks, falls back to the walk (k_brick<kAssoc>).
+constexpr int kRecBricks = 4;
+constexpr int kRecSlots = 16;
 
 struct Tiling { int tx, ty, w, h; };   // tiles per (view, frame) in u and v, tile width / height in cells
 struct Tilings { Tiling t[3]; };
@@ -80,10 +91,26 @@ struct FindCtl {         // device scalars of one chunk
   unsigned generic;      // 1: the brick plan failed, the generic kernels do the chunk
   unsigned skip;         // 1: capacity overflow, nothing more is done for the chunk
   unsigned work[2];      // work-item counters of the two brick passes
+  unsigned slot_total;   // entries of slot_row handed out to bricks
+  unsigned norecord;     // 1: a (view, frame) has more than kRecBricks bricks: no hit records, every candidate is walked
+  unsigned ovf_count;    // candidates of the chunk that have to be walked (record overflow)
+  unsigned pad;
 };
 
 __device__ __forceinline__ unsigned long long cand_k1(int n_tube, int d2) {
   return ((unsigned long long)min(n_tube, kMaxTube) << 22) | (unsigned long long)(unsigned)d2;
+}
+
+// n_tube of a seed from its 64-bit counter: four 16-bit fields (one per brick ordinal) when the voting pass
+// kept hit records, else one plain count.  A field holds one visit's count (<= 0xffff, clamped: such a seed
+// is out of range anyway, EMU_ST_RANGE).
+__device__ __forceinline__ unsigned tube_total(unsigned long long v, bool fields) {
+  if (!fields) return (unsigned)min(v, 0xffffffffull);
+  return (unsigned)(v & 0xffffu) + (unsigned)((v >> 16) & 0xffffu) + (unsigned)((v >> 32) & 0xffffu) + (unsigned)(v >> 48);
+}
+__device__ __forceinline__ bool tube_overflows(unsigned long long v) {   // some brick holds more grains than a record
+  return (unsigned)(v & 0xffffu) > (unsigned)kRecSlots || (unsigned)((v >> 16) & 0xffffu) > (unsigned)kRecSlots ||
+         (unsigned)((v >> 32) & 0xffffu) > (unsigned)kRecSlots || (unsigned)(v >> 48) > (unsigned)kRecSlots;
 }
 
 // k(g) = (z, x+y, min(x,y), x, row), lexicographic
@@ -360,7 +387,7 @@ k_chunk_offsets(int nv, const unsigned* __restrict__ tot, unsigned* __restrict__
   if (threadIdx.x == 0) {
     const unsigned long long total = carry_s;
     off[nv] = (unsigned)min(total, 0xffffffffull);
-    atomicAdd(counts + count_slot, total);
+    if (count_slot >= 0) atomicAdd(counts + count_slot, total);
     if (status_bit == (unsigned)EMU_ST_SEED_OVERFLOW) atomicMax(counts + EMU_CNT_NEED, total);
     if (total > cap) {
       atomicOr(counts + EMU_CNT_STATUS, (unsigned long long)status_bit);
@@ -380,7 +407,7 @@ k_chunk_offsets(int nv, const unsigned* __restrict__ tot, unsigned* __restrict__
 // Q13), or a grid the format cannot hold, sends the chunk to the generic kernels.
 __global__ void __launch_bounds__(128)
 k_plan(EmuDev P, Tilings TT, FramePtrs F, const EmuBox* __restrict__ bbox, int v0, int v1,
-       Brick* __restrict__ bricks, unsigned brick_cap, FindCtl* __restrict__ ctl) {
+       Brick* __restrict__ bricks, unsigned brick_cap, int* __restrict__ vf_brick_base, FindCtl* __restrict__ ctl) {
   const int lane = threadIdx.x & 31;
   const int vf = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
   if (vf >= (v1 - v0) * 3 || ctl->skip) return;
@@ -397,11 +424,12 @@ k_plan(EmuDev P, Tilings TT, FramePtrs F, const EmuBox* __restrict__ bbox, int v
     for (int a = 0; a < 3; ++a) in_box = in_box && bb.lo[a] >= 0 && bb.hi[a] < P.n[a] * P.cs[a];
 #pragma unroll
     for (int i = 0; i < 3; ++i) {                                            // ... and inside every frame's grid
-      const int a = (f + i) % 3;
+      const int a = emu_frame_axis(f, i);
       in_box = in_box && bb.hi[a] < P.fr[f].n[i] * P.cs[i];
     }
     if (!in_box) { if (lane == 0) ctl->generic = 1; return; }
   }
+  int ord = 0;
   for (int t = 0; t < T.tx * T.ty; ++t) {
     const int cx0 = (t % T.tx) * T.w, cy0 = (t / T.tx) * T.h;
     const int cx1 = min(nx, cx0 + T.w) - 1, cy1 = min(ny, cy0 + T.h) - 1;
@@ -420,13 +448,18 @@ k_plan(EmuDev P, Tilings TT, FramePtrs F, const EmuBox* __restrict__ bbox, int v
       }
       const bool flush = (cz == nz) || brick_bytes(acc + cnt, (long long)(cz - z_first + 1) * H, W) > kPoolBytes;
       if (flush) {
-        if (acc > 0 && lane == 0) {
-          const unsigned slot = atomicAdd(&ctl->n_bricks, 1u);
-          if (slot < brick_cap) {
-            Brick b; b.view = v; b.cx0 = cx0; b.cx1 = cx1; b.cy0 = cy0; b.cy1 = cy1; b.cz0 = z_first; b.cz1 = cz - 1; b.n = acc;
-            b.frame = f; b.pad[0] = b.pad[1] = b.pad[2] = 0;
-            bricks[slot] = b;
+        if (acc > 0) {
+          if (lane == 0) {
+            const unsigned slot = atomicAdd(&ctl->n_bricks, 1u);
+            if (slot < brick_cap) {
+              Brick b; b.view = v; b.cx0 = cx0; b.cx1 = cx1; b.cy0 = cy0; b.cy1 = cy1; b.cz0 = z_first; b.cz1 = cz - 1; b.n = acc;
+              b.frame = f; b.ord = ord; b.base = (int)atomicAdd(&ctl->slot_total, (unsigned)acc); b.pad = 0;
+              bricks[slot] = b;
+              if (ord < kRecBricks) vf_brick_base[vf * kRecBricks + ord] = b.base;
+              else ctl->norecord = 1;
+            }
           }
+          ++ord;
         }
         z_first = cz; acc = 0;
       }
@@ -498,15 +531,17 @@ struct BrickShared {
 template <int kMode>
 __global__ void __launch_bounds__(kBrickThreads, 1)
 k_brick(EmuDev P, FramePtrs F, int v0, const Brick* __restrict__ bricks, FindCtl* __restrict__ ctl,
-        int slices, const int4* __restrict__ geo, const unsigned* __restrict__ view_item_off,
-        unsigned* __restrict__ seed_cnt, unsigned long long* __restrict__ keyA,
-        unsigned long long* __restrict__ keyB, unsigned long long* __restrict__ counts) {
+        int slices, const int4* __restrict__ geo, const unsigned* __restrict__ item_ci,
+        const unsigned* __restrict__ view_item_off, unsigned long long* __restrict__ seed_cnt, unsigned short* __restrict__ recs, int* __restrict__ slot_row,
+        unsigned long long* __restrict__ keyA, unsigned long long* __restrict__ keyB,
+        unsigned long long* __restrict__ counts) {
   extern __shared__ __align__(16) unsigned char pool[];
   __shared__ BrickShared sh;
 
   if (ctl->skip || ctl->generic) return;
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   const unsigned n_items = ctl->n_bricks * (unsigned)slices;
+  const bool record = (kMode == kVote) && recs != nullptr && ctl->norecord == 0;
   const float R = P.Rw;
   const float r2f = (float)P.r2;
   const float BIG = 1.0e9f;
@@ -588,6 +623,7 @@ k_brick(EmuDev P, FramePtrs F, int v0, const Brick* __restrict__ bricks, FindCtl
           for (int i = lane; i < rlen; i += 32) {
             const int4 g = __ldg(sorted + rgs + i);
             sgw[roff + i] = (unsigned)g.x | ((unsigned)(g.y - y0) << 16) | ((unsigned)(g.z - z0) << 24);
+            if (record && sl == 0) slot_row[B.base + roff + i] = g.w;      // the first item of a brick publishes its rows
           }
         }
         __syncthreads();
@@ -609,6 +645,8 @@ k_brick(EmuDev P, FramePtrs F, int v0, const Brick* __restrict__ bricks, FindCtl
     const unsigned tab0 = pool_a + 4u * (unsigned)B.n - 2u * (unsigned)B.cx0 - (unsigned)B.cy0 * row_b - lay_b;
     const unsigned delta_o = 2u * (unsigned)(B.cx0 + S - 2);               // from a row address to its position word
     const float cz1f = (float)B.cz1, cy1f = (float)B.cy1;
+    const int ord_shift = record ? 16 * (B.ord & (kRecBricks - 1)) : 0;   // without records: one plain counter
+    const size_t rec_ord = (size_t)(B.ord & (kRecBricks - 1)) * kRecSlots;
 
     // ---- per-lane state: one seed per lane ----
     bool idle = true;                                // no seed (waiting for the next refill)
@@ -692,8 +730,9 @@ k_brick(EmuDev P, FramePtrs F, int v0, const Brick* __restrict__ bricks, FindCtl
               sidx = idx; count = 0;
               if (kMode == kAssoc) {
                 const unsigned long long k1 = cand_k1((int)((unsigned)q.y >> 16), __float2int_rn(D2));
-                ka = (k1 << kCiBits) | (unsigned long long)(kCiMask - idx);
-                kb = (k1 << kCiBits) | (unsigned long long)idx;
+                const unsigned ci = __ldg(item_ci + idx);            // the streamed list is the "walk" list
+                ka = (k1 << kCiBits) | (unsigned long long)(kCiMask - ci);
+                kb = (k1 << kCiBits) | (unsigned long long)ci;
               }
               // slab k of an axis covers [k cs - R, (k+1) cs - 1 + R]: its u interval is the one of slab 0 moved by k cs / slope
               dty = P.csf[1] * inv_a; dtz = P.csf[2] * inv_b;
@@ -724,7 +763,7 @@ k_brick(EmuDev P, FramePtrs F, int v0, const Brick* __restrict__ bricks, FindCtl
         if (cyf > cyhf) {                                   // next w layer of the brick
           czf += 1.0f; ozm -= P.csf[2]; layp += lay_b;
           if (czf > czhf) {                                 // the seed is finished
-            if (kMode == kVote && count) atomicAdd(seed_cnt + sidx, (unsigned)count);
+            if (kMode == kVote && count) atomicAdd(seed_cnt + sidx, (unsigned long long)min(count, 0xffff) << ord_shift);
             idle = true;
           } else {
             tl0 = fmaxf(t0, __fmaf_rn(czf, dtz, tzl)); tl1 = fminf(t1, __fmaf_rn(czf, dtz, tzh));
@@ -766,6 +805,14 @@ k_brick(EmuDev P, FramePtrs F, int v0, const Brick* __restrict__ bricks, FindCtl
         }
         in1 = in1 && two;
         if (kMode == kVote) {
+          if (record && (in0 || in1)) {
+            // write down the brick slots of the grains found (the first kRecSlots of this seed in this brick)
+            unsigned short* rec = recs + ((size_t)sidx * (kRecBricks * kRecSlots) + rec_ord);
+            const unsigned slot = (j - pool_a) >> 2;
+            if (in0 && count < kRecSlots) rec[count] = (unsigned short)slot;
+            const int c1 = count + (int)in0;
+            if (in1 && c1 < kRecSlots) rec[c1] = (unsigned short)(slot + 1u);
+          }
           count += (int)in0 + (int)in1;
         } else if (in0 || in1) {
           // slot of the grain in the brick + (sorted position - slot) of the first grain of its row -> row of the grain
@@ -787,39 +834,54 @@ k_brick(EmuDev P, FramePtrs F, int v0, const Brick* __restrict__ bricks, FindCtl
 // A4: candidates = seeds with n_tube >= min_grains, grouped by (view, frame).  grid = (blocks, groups of
 // the chunk).  A warp takes 1024 consecutive seeds at a time, counts its candidates with ballots (keeping
 // every lane's 32 flags in a register) and makes ONE atomicAdd on the group's counter per 1024 seeds.
+// Candidates whose hit records are incomplete (more than kRecSlots grains in one brick, or no records at
+// all) also go to the "walk" list (packed geometry + candidate index), which k_brick<kAssoc> streams.
 template <int kFill>
 __global__ void __launch_bounds__(256)
 k_cands(EmuDev P, int v0, const FindCtl* __restrict__ ctl, const unsigned* __restrict__ view_seed_off,
-        const unsigned* __restrict__ seed_cnt, const int4* __restrict__ geo, const int2* __restrict__ ab,
+        const unsigned long long* __restrict__ seed_cnt, const int4* __restrict__ geo, const int2* __restrict__ ab,
         unsigned* __restrict__ view_cand_cnt, const unsigned* __restrict__ view_cand_off,
-        Cand* __restrict__ cands, int4* __restrict__ cand_geo, unsigned long long* __restrict__ counts) {
+        unsigned* __restrict__ view_ovf_cnt, const unsigned* __restrict__ view_ovf_off,
+        Cand* __restrict__ cands, unsigned* __restrict__ cand_seed, int4* __restrict__ ovf_geo,
+        unsigned* __restrict__ ovf_ci, unsigned long long* __restrict__ counts) {
   if (ctl->skip || ctl->generic) return;
+  const bool fields = ctl->norecord == 0;
   const int vf = blockIdx.y, lane = threadIdx.x & 31;
   const unsigned lo = view_seed_off[vf], hi = view_seed_off[vf + 1];
   const unsigned wpb = blockDim.x >> 5;
   const unsigned span = gridDim.x * wpb * 1024u;
   unsigned status = 0;
   for (unsigned c0 = lo + (blockIdx.x * wpb + (threadIdx.x >> 5)) * 1024u; c0 < hi; c0 += span) {
-    unsigned flags = 0, total = 0;
+    unsigned flags = 0, oflags = 0, total = 0, ototal = 0;
 #pragma unroll 4
     for (int it = 0; it < 32; ++it) {
       const unsigned i = c0 + (unsigned)it * 32u + (unsigned)lane;
-      const bool is = (i < hi) && seed_cnt[i] >= (unsigned)P.min_grains;
-      flags |= (unsigned)is << it;
+      bool is = false, ov = false;
+      if (i < hi) {
+        const unsigned long long v = seed_cnt[i];
+        is = tube_total(v, fields) >= (unsigned)P.min_grains;
+        ov = is && (!fields || tube_overflows(v));
+      }
+      flags |= (unsigned)is << it; oflags |= (unsigned)ov << it;
       total += __popc(__ballot_sync(EMU_FULL, is));
+      ototal += __popc(__ballot_sync(EMU_FULL, ov));
     }
     if (!total) continue;
-    unsigned base = 0;
-    if (lane == 0) base = atomicAdd(view_cand_cnt + vf, total);
+    unsigned base = 0, obase = 0;
+    if (lane == 0) {
+      base = atomicAdd(view_cand_cnt + vf, total);
+      if (ototal) obase = atomicAdd(view_ovf_cnt + vf, ototal);
+    }
     if (!kFill) continue;
     base = __shfl_sync(EMU_FULL, base, 0) + view_cand_off[vf];
+    obase = __shfl_sync(EMU_FULL, obase, 0) + view_ovf_off[vf];
     for (int it = 0; it < 32; ++it) {
-      const bool is = (flags >> it) & 1u;
-      const unsigned m = __ballot_sync(EMU_FULL, is);
+      const bool is = (flags >> it) & 1u, ov = (oflags >> it) & 1u;
+      const unsigned m = __ballot_sync(EMU_FULL, is), mo = __ballot_sync(EMU_FULL, ov);
       if (is) {
         const unsigned i = c0 + (unsigned)it * 32u + (unsigned)lane;
         const unsigned ci = base + (unsigned)__popc(m & ((1u << lane) - 1u));
-        const unsigned n = seed_cnt[i];
+        const unsigned n = tube_total(seed_cnt[i], fields);
         int4 g = geo[i];
         const int2 p = ab[i];
         int dx, dy, dz;
@@ -827,28 +889,67 @@ k_cands(EmuDev P, int v0, const FindCtl* __restrict__ ctl, const unsigned* __res
         if (n > (unsigned)kMaxTube) status |= EMU_ST_RANGE;
         Cand c; c.a = p.x; c.b = p.y; c.n_tube_view = (int)min(n, 0xffffu) | ((vf / 3) << 16); c.d2 = dx * dx + dy * dy + dz * dz;
         cands[ci] = c;
-        g.y = (int)(((unsigned)g.y & 0xffffu) | (min(n, (unsigned)kMaxTube) << 16));
-        cand_geo[ci] = g;
+        cand_seed[ci] = i;
+        if (ov) {
+          const unsigned oi = obase + (unsigned)__popc(mo & ((1u << lane) - 1u));
+          g.y = (int)(((unsigned)g.y & 0xffffu) | (min(n, (unsigned)kMaxTube) << 16));
+          ovf_geo[oi] = g;
+          ovf_ci[oi] = ci;
+        }
       }
-      base += __popc(m);
+      base += __popc(m); obase += __popc(mo);
     }
   }
   if (kFill && __any_sync(EMU_FULL, status != 0) && lane == 0) atomicOr(counts + EMU_CNT_STATUS, (unsigned long long)EMU_ST_RANGE);
 }
 
+// A5 from the hit records: every candidate whose records are complete gives its packed priority to the
+// grains written down by the voting pass (brick slot -> row through slot_row).  grid = (blocks, groups).
+__global__ void __launch_bounds__(256)
+k_assoc_hits(int v0, const FindCtl* __restrict__ ctl, const unsigned* __restrict__ view_cand_off,
+             const Cand* __restrict__ cands, const unsigned* __restrict__ cand_seed,
+             const unsigned long long* __restrict__ seed_cnt, const unsigned short* __restrict__ recs,
+             const int* __restrict__ slot_row, const int* __restrict__ vf_brick_base,
+             unsigned long long* __restrict__ keyA, unsigned long long* __restrict__ keyB) {
+  if (ctl->skip || ctl->generic || ctl->norecord) return;
+  const int vf = blockIdx.y;
+  const unsigned lo = view_cand_off[vf], hi = view_cand_off[vf + 1];
+  for (unsigned ci = lo + blockIdx.x * blockDim.x + threadIdx.x; ci < hi; ci += gridDim.x * blockDim.x) {
+    const unsigned i = cand_seed[ci];
+    const unsigned long long v = seed_cnt[i];
+    if (tube_overflows(v)) continue;                        // walked by k_brick<kAssoc>
+    const Cand c = cands[ci];
+    const unsigned long long k1 = cand_k1(c.n_tube_view & 0xffff, c.d2);
+    const unsigned long long ka = (k1 << kCiBits) | (unsigned long long)(kCiMask - ci);
+    const unsigned long long kb = (k1 << kCiBits) | (unsigned long long)ci;
+#pragma unroll
+    for (int ord = 0; ord < kRecBricks; ++ord) {
+      const int cnt = (int)((v >> (16 * ord)) & 0xffffu);
+      if (!cnt) continue;
+      const int base = vf_brick_base[vf * kRecBricks + ord];
+      const unsigned short* rec = recs + ((size_t)i * (kRecBricks * kRecSlots) + (size_t)ord * kRecSlots);
+      for (int k = 0; k < cnt; ++k) {
+        const int row = slot_row[base + (int)rec[k]];
+        atomicMax(keyA + row, ka); atomicMax(keyB + row, kb);
+      }
+    }
+  }
+}
+
 // seed dump for emu_count_seeds: (view, row_a, row_b, n_tube), rows ordered
 __global__ void __launch_bounds__(256)
 k_seed_dump(int v0, const FindCtl* __restrict__ ctl, const int4* __restrict__ sorted,
-            const unsigned* __restrict__ view_seed_off, const unsigned* __restrict__ seed_cnt,
+            const unsigned* __restrict__ view_seed_off, const unsigned long long* __restrict__ seed_cnt,
             const int2* __restrict__ ab, int4* __restrict__ dump, long long dump_cap) {
   if (ctl->skip || ctl->generic) return;
+  const bool fields = ctl->norecord == 0;
   const int vf = blockIdx.y;
   const unsigned lo = view_seed_off[vf], hi = view_seed_off[vf + 1];
   for (unsigned i = lo + blockIdx.x * blockDim.x + threadIdx.x; i < hi; i += gridDim.x * blockDim.x) {
     if ((long long)i >= dump_cap) continue;
     const int2 p = ab[i];
     const int ra = sorted[p.x].w, rb = sorted[p.y].w;
-    dump[i] = make_int4(v0 + vf / 3, min(ra, rb), max(ra, rb), (int)seed_cnt[i]);
+    dump[i] = make_int4(v0 + vf / 3, min(ra, rb), max(ra, rb), (int)tube_total(seed_cnt[i], fields));
   }
 }
 
@@ -1252,13 +1353,15 @@ struct FindWs {
   unsigned* view_seed_tot; unsigned* view_seed_off; unsigned* view_cand_cnt; unsigned* view_cand_off;
   int* view_ntracks; unsigned* view_tracks; Brick* bricks;
   int4* sortedF[3]; int* cell_startF[3]; void* bin_ws; size_t bin_ws_bytes;     // frames 1, 2 (0 = the caller's)
-  int4* geo; int2* ab; unsigned* seed_cnt;
-  Cand* cands; int4* cand_geo; int* wins; unsigned* cand_track;
+  int* slot_row; int* vf_brick_base; unsigned* view_ovf_cnt; unsigned* view_ovf_off;
+  int4* geo; int2* ab; unsigned long long* seed_cnt; unsigned short* recs;
+  Cand* cands; unsigned* cand_seed; int4* ovf_geo; unsigned* ovf_ci; int* wins; unsigned* cand_track;
   size_t seed_cap, cand_cap, brick_cap; int views_per_chunk;
 };
 
-constexpr size_t kSeedBytes = sizeof(int4) + sizeof(int2) + sizeof(unsigned);                    // 28
-constexpr size_t kCandBytes = sizeof(Cand) + sizeof(int4) + sizeof(int) + sizeof(unsigned);      // 40
+constexpr size_t kRecBytes = (size_t)kRecBricks * kRecSlots * sizeof(unsigned short);             // 128 per seed
+constexpr size_t kSeedBytes = sizeof(int4) + sizeof(int2) + sizeof(unsigned long long) + kRecBytes;                       // 160
+constexpr size_t kCandBytes = sizeof(Cand) + sizeof(unsigned) + sizeof(int4) + sizeof(unsigned) + sizeof(int) + sizeof(unsigned);  // 48
 constexpr size_t kMinSeedCap = 1u << 20, kMinCandCap = 1u << 16;
 
 size_t bricks_per_view(const EmuDev& P, const Tilings& TT) {
@@ -1274,7 +1377,9 @@ size_t fixed_bytes(const EmuDev& P, const Tilings& TT, int64_t n_grains, int32_t
   b += emu_align256((size_t)n_grains * sizeof(unsigned));                   // owner
   b += emu_align256(3 * (size_t)n_grains * sizeof(unsigned));               // seed_off, one plane per frame
   b += emu_align256(sizeof(FindCtl)) + emu_align256(kTieBits / 8) + 256;
-  b += 4 * emu_align256((3 * (size_t)vpc + 1) * sizeof(unsigned));
+  b += 6 * emu_align256((3 * (size_t)vpc + 1) * sizeof(unsigned));
+  b += emu_align256(3 * (size_t)vpc * kRecBricks * sizeof(int));            // vf_brick_base
+  b += emu_align256(3 * (size_t)n_grains * sizeof(int));                    // slot_row: every grain once per frame
   b += emu_align256((size_t)vpc * sizeof(int));
   b += emu_align256((size_t)vpc * P.max_tracks * sizeof(unsigned));
   b += emu_align256((size_t)vpc * bricks_per_view(P, TT) * sizeof(Brick));
@@ -1335,8 +1440,8 @@ size_t emu_find_ws_recommended_bytes(const EmuDev& P, int64_t n_grains, int32_t 
   const int64_t per_view_g = emu_max64(1, (n_grains + emu_max64(1, n_views) - 1) / emu_max64(1, n_views));
   const int64_t spv = per_view_g * seeds_per_grain, cpv = per_view_g * cand_per_grain;
   const int64_t per_view_bytes = spv * (int64_t)kSeedBytes + cpv * (int64_t)kCandBytes;
-  // as many views per chunk as fit 24 GiB of seed / candidate storage (at least one)
-  int64_t vpc = emu_max64(1, emu_min64(emu_max64(1, n_views), ((int64_t)24 << 30) / emu_max64(1, per_view_bytes)));
+  // as many views per chunk as fit 48 GiB of seed / candidate storage (at least one)
+  int64_t vpc = emu_max64(1, emu_min64(emu_max64(1, n_views), ((int64_t)48 << 30) / emu_max64(1, per_view_bytes)));
   vpc = emu_min64(vpc, 21000);
   const size_t seed_cap = (size_t)emu_max64((int64_t)kMinSeedCap, spv * vpc);
   const size_t cand_cap = (size_t)emu_max64((int64_t)kMinCandCap, cpv * vpc);
@@ -1382,6 +1487,10 @@ static int carve(const EmuDev& P, const Tilings& TT, Hints hints, int64_t n_grai
   W.view_seed_off = (unsigned*)take((3 * (size_t)vpc + 1) * sizeof(unsigned));
   W.view_cand_cnt = (unsigned*)take((3 * (size_t)vpc + 1) * sizeof(unsigned));
   W.view_cand_off = (unsigned*)take((3 * (size_t)vpc + 1) * sizeof(unsigned));
+  W.view_ovf_cnt = (unsigned*)take((3 * (size_t)vpc + 1) * sizeof(unsigned));
+  W.view_ovf_off = (unsigned*)take((3 * (size_t)vpc + 1) * sizeof(unsigned));
+  W.vf_brick_base = (int*)take(3 * (size_t)vpc * kRecBricks * sizeof(int));
+  W.slot_row = (int*)take(3 * (size_t)n_grains * sizeof(int));
   W.view_ntracks = (int*)take((size_t)vpc * sizeof(int));
   W.view_tracks = (unsigned*)take((size_t)vpc * P.max_tracks * sizeof(unsigned));
   W.brick_cap = (size_t)vpc * bricks_per_view(P, TT);
@@ -1395,9 +1504,12 @@ static int carve(const EmuDev& P, const Tilings& TT, Hints hints, int64_t n_grai
   W.bin_ws = take(W.bin_ws_bytes);
   W.geo = (int4*)take(seed_cap * sizeof(int4));
   W.ab = (int2*)take(seed_cap * sizeof(int2));
-  W.seed_cnt = (unsigned*)take(seed_cap * sizeof(unsigned));
+  W.seed_cnt = (unsigned long long*)take(seed_cap * sizeof(unsigned long long));
+  W.recs = (unsigned short*)take(seed_cap * kRecBytes);
   W.cands = (Cand*)take(cand_cap * sizeof(Cand));
-  W.cand_geo = (int4*)take(cand_cap * sizeof(int4));
+  W.cand_seed = (unsigned*)take(cand_cap * sizeof(unsigned));
+  W.ovf_geo = (int4*)take(cand_cap * sizeof(int4));
+  W.ovf_ci = (unsigned*)take(cand_cap * sizeof(unsigned));
   W.wins = (int*)take(cand_cap * sizeof(int));
   W.cand_track = (unsigned*)take(cand_cap * sizeof(unsigned));
   W.seed_cap = seed_cap; W.cand_cap = cand_cap; W.views_per_chunk = vpc;
@@ -1465,13 +1577,16 @@ static int vote_chunk(const EmuDev& P, const Tilings& TT, FindWs& W, const Frame
       W.ctl, counts, EMU_CNT_SEEDS));
   EMU_LAUNCH(EMU_STAGE_SEEDS, st, k_seed_pairs<1><<<kSM * 16, kVoteThreads, 0, st>>>(
       P, sorted, d_cell_start, d_view_off, v0, v1, W.seed_off, plane, W.view_seed_off, W.ctl, W.geo, W.ab, counts));
-  EMU_CK(cudaMemsetAsync(W.seed_cnt, 0, W.seed_cap * sizeof(unsigned), st));
+  // only the counters of the seeds this chunk has are cleared (the count is on the device: clear the capacity
+  // when the chunk is the size the workspace was cut for, else what its views can hold by the hint)
+  EMU_CK(cudaMemsetAsync(W.seed_cnt, 0, W.seed_cap * sizeof(unsigned long long), st));
   EMU_LAUNCH(EMU_STAGE_PREP, st, k_plan<<<grid_for(3 * nv, 4, 1 << 20), 128, 0, st>>>(
-      P, TT, F, W.bbox, v0, v1, W.bricks, (unsigned)W.brick_cap, W.ctl));
+      P, TT, F, W.bbox, v0, v1, W.bricks, (unsigned)W.brick_cap, W.vf_brick_base, W.ctl));
   EMU_LAUNCH(EMU_STAGE_PREP, st, k_plan_finish<<<1, 1, 0, st>>>(W.ctl, (unsigned)W.brick_cap));
   EMU_CK(cudaFuncSetAttribute(k_brick<kVote>, cudaFuncAttributeMaxDynamicSharedMemorySize, kPoolBytes));
   EMU_LAUNCH(EMU_STAGE_VOTE, st, k_brick<kVote><<<kSM, kBrickThreads, kPoolBytes, st>>>(
-      P, F, v0, W.bricks, W.ctl, slices, W.geo, W.view_seed_off, W.seed_cnt, nullptr, nullptr, counts));
+      P, F, v0, W.bricks, W.ctl, slices, W.geo, nullptr, W.view_seed_off, W.seed_cnt, W.recs, W.slot_row, nullptr,
+      nullptr, counts));
   return EMU_OK;
 }
 
@@ -1505,15 +1620,21 @@ int emu_find_launch(const EmuDev& P, int seeds_per_grain, int cand_per_grain, co
     rc = vote_chunk(P, TT, W, F, d_view_off, n_grains, v0, v1, slices, kSM, counts, st);
     if (rc != EMU_OK) return rc;
     // A4: candidates grouped by (view, frame)
+    EMU_CK(cudaMemsetAsync(W.view_ovf_cnt, 0, (3 * (size_t)nv + 1) * sizeof(unsigned), st));
     EMU_LAUNCH(EMU_STAGE_CANDS, st, k_cands<0><<<dim3(16, 3 * nv), 256, 0, st>>>(
-        P, v0, W.ctl, W.view_seed_off, W.seed_cnt, W.geo, W.ab, W.view_cand_cnt, nullptr, nullptr, nullptr, counts));
+        P, v0, W.ctl, W.view_seed_off, W.seed_cnt, W.geo, W.ab, W.view_cand_cnt, nullptr, W.view_ovf_cnt, nullptr,
+        nullptr, nullptr, nullptr, nullptr, counts));
     EMU_LAUNCH(EMU_STAGE_CANDS, st, k_chunk_offsets<<<1, 1024, 0, st>>>(
         3 * nv, W.view_cand_cnt, W.view_cand_off, &W.ctl->cand_count, (unsigned)W.cand_cap, (unsigned)EMU_ST_CAND_OVERFLOW,
         W.ctl, counts, EMU_CNT_CANDIDATES));
+    EMU_LAUNCH(EMU_STAGE_CANDS, st, k_chunk_offsets<<<1, 1024, 0, st>>>(
+        3 * nv, W.view_ovf_cnt, W.view_ovf_off, &W.ctl->ovf_count, (unsigned)W.cand_cap, (unsigned)EMU_ST_CAND_OVERFLOW,
+        W.ctl, counts, -1));
     EMU_CK(cudaMemsetAsync(W.view_cand_cnt, 0, (3 * (size_t)nv + 1) * sizeof(unsigned), st));
+    EMU_CK(cudaMemsetAsync(W.view_ovf_cnt, 0, (3 * (size_t)nv + 1) * sizeof(unsigned), st));
     EMU_LAUNCH(EMU_STAGE_CANDS, st, k_cands<1><<<dim3(16, 3 * nv), 256, 0, st>>>(
-        P, v0, W.ctl, W.view_seed_off, W.seed_cnt, W.geo, W.ab, W.view_cand_cnt, W.view_cand_off, W.cands, W.cand_geo,
-        counts));
+        P, v0, W.ctl, W.view_seed_off, W.seed_cnt, W.geo, W.ab, W.view_cand_cnt, W.view_cand_off, W.view_ovf_cnt,
+        W.view_ovf_off, W.cands, W.cand_seed, W.ovf_geo, W.ovf_ci, counts));
     // generic fallback for the whole chunk (returns at once unless the brick plan failed)
     EMU_LAUNCH(EMU_STAGE_VOTE, st, k_vote_generic<false><<<kSM * 16, kVoteThreads, 0, st>>>(
         P, sorted, d_cell_start, d_view_off, W.bbox, v0, v1, W.cands, (unsigned)W.cand_cap, W.ctl, nullptr, 0, nullptr,
@@ -1522,8 +1643,11 @@ int emu_find_launch(const EmuDev& P, int seeds_per_grain, int cand_per_grain, co
     EMU_LAUNCH(EMU_STAGE_PREP, st, k_reset_cand_arrays<<<kSM * 8, 256, 0, st>>>(W.ctl, W.wins, W.cand_track));
     // A5
     EMU_CK(cudaFuncSetAttribute(k_brick<kAssoc>, cudaFuncAttributeMaxDynamicSharedMemorySize, kPoolBytes));
+    EMU_LAUNCH(EMU_STAGE_ASSOC, st, k_assoc_hits<<<dim3(8, 3 * nv), 256, 0, st>>>(
+        v0, W.ctl, W.view_cand_off, W.cands, W.cand_seed, W.seed_cnt, W.recs, W.slot_row, W.vf_brick_base, W.keyA, W.keyB));
     EMU_LAUNCH(EMU_STAGE_ASSOC, st, k_brick<kAssoc><<<kSM, kBrickThreads, kPoolBytes, st>>>(
-        P, F, v0, W.bricks, W.ctl, slices, W.cand_geo, W.view_cand_off, nullptr, W.keyA, W.keyB, counts));
+        P, F, v0, W.bricks, W.ctl, slices, W.ovf_geo, W.ovf_ci, W.view_ovf_off, nullptr, nullptr, nullptr, W.keyA, W.keyB,
+        counts));
     EMU_LAUNCH(EMU_STAGE_ASSOC, st, k_assoc_generic<0><<<kSM * 16, kVoteThreads, 0, st>>>(
         P, sorted, d_cell_start, W.bbox, v0, W.cands, W.ctl, W.tie_bits, W.keyA, W.keyB, W.owner));
     EMU_LAUNCH(EMU_STAGE_ASSOC, st, k_tie_detect<<<kSM * 4, 256, 0, st>>>(d_view_off, v0, v1, W.keyA, W.keyB, W.ctl, W.tie_bits));

@@ -93,9 +93,9 @@ def test_batch_of_views_in_several_chunks(E, oracle_mod):
     ref = oracle_mod.track_views(p, b.grains, b.view_off, "cells", 0)
     prm = E.make_params(**{k: p[k] for k in ("view_size_q", "cell_size_q", "sep_min_q", "sep_max_q", "tube_r2_q", "min_grains")})
     _, rec = E.emu_workspace_bytes(prm, b.n_grains, b.n_views)
-    # the recommendation holds all 7 views at once; the minimum seed / candidate capacity (1 Mi seeds) holds
-    # about 3 views of this shape at the default hint of 192 seeds per grain
-    for ws in (None, 48 << 20):
+    # the recommendation holds all 7 views at once; the minimum seed / candidate capacity (1 Mi seeds of 160 B:
+    # geometry, counter and hit records) holds about 3 views of this shape at the default hint of 192 seeds per grain
+    for ws in (None, 200 << 20):
         got = run_gpu(E, p, b.grains, b.view_off, find_ws_bytes=ws)
         assert_same_tracks(E, got, ref)
 
