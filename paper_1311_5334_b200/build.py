@@ -26,7 +26,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
         if not os.path.exists(nvcc):
             nvcc = "nvcc"
-        cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + SOURCES
+        extra = os.environ.get("EMU_NVCC_EXTRA", "").split()       # tuning experiments only (e.g. -DEMU_REFILL=12)
+        cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + SOURCES
         subprocess.run(cmd, check=True, cwd=CSRC)
     return LIB
 

@@ -40,7 +40,16 @@ constexpr unsigned kCiMask = (1u << kCiBits) - 1u;
 constexpr unsigned kNone = 0xffffffffu;
 constexpr int kMaxTube = 8191;                    // n_tube field of the packed priority: 13 bits
 
-constexpr int kBrickThreads = 1024;               // one persistent block per SM
+#ifndef EMU_BRICK_THREADS
+#define EMU_BRICK_THREADS 1024
+#endif
+#ifndef EMU_REFILL
+#define EMU_REFILL 8
+#endif
+#ifndef EMU_REFILL_STOP
+#define EMU_REFILL_STOP 4
+#endif
+constexpr int kBrickThreads = EMU_BRICK_THREADS;  // one persistent block per SM
 constexpr int kPoolBytes = 222 * 1024;            // dynamic shared memory of a brick: grains | row table | cell table
 constexpr int kGrab = 128;                        // seeds a warp takes from the block's stream at a time
 constexpr int kTieBits = 1 << 16;                 // bitmap of tied priorities
@@ -497,13 +506,21 @@ __global__ void k_plan_finish(FindCtl* ctl, unsigned brick_cap) {
 // fma(v1, d2, -rn(v2 d1)): the products stay below 2^27, so |c_f - c| <= 4 + 2^-24 |c| per component, and
 // s_f = |c_f|^2 carries a relative error below 2^-22.  With m_up = R_up (|dx| + |dy| + |dz|) >= sqrt(T),
 // T = r2 D2, delta = 16 + 2^-21 m_up and band = 1.01 (2 m_up delta + delta^2) + 2^-20 T:
-//   s_f <= T - band  =>  in the tube;   s_f > T + band  =>  outside;   otherwise the exact 64-bit
+//   s_f < T - band  =>  in the tube;   s_f > T + band  =>  outside;   |s_f - T| <= band: the exact 64-bit
 // integer predicate (emu_in_tube) decides.  The result is therefore the exact one in every case
 // (DESIGN.md section 6 has the derivation).
 enum { kVote = 0, kAssoc = 1 };
-constexpr int kRefill = 8;                        // idle lanes of a warp that trigger a refill from the seed stream
-constexpr int kRefillStop = 4;                    // the refill goes on while at least this many lanes are still idle
+constexpr int kRefill = EMU_REFILL;                        // idle lanes of a warp that trigger a refill from the seed stream
+constexpr int kRefillStop = EMU_REFILL_STOP;                    // the refill goes on while at least this many lanes are still idle
+constexpr int kPairs = 1;                         // pairs of grains a lane tests at most per iteration (the run of a row)
 
+// 1 / x for |x| >= 1 (a component of d): one MUFU.RCP, no range handling (relative error 2^-23: the traversal
+// bounds only have to be a superset and carry 2 q of slack)
+__device__ __forceinline__ float rcp_fast(float x) {
+  float r;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+  return r;
+}
 __device__ __forceinline__ unsigned lds_u32(unsigned addr) {
   unsigned v;
   asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr));
@@ -653,7 +670,8 @@ k_brick(EmuDev P, FramePtrs F, int v0, const Brick* __restrict__ bricks, FindCtl
     float ay = 0.f, dx = 1.f, dy = 0.f, dz = 0.f;
     float a = 0.f, y0 = 0.f;                         // v(u) = y0 + a u
     float oxm = 0.f, oym = 0.f, ozm = 0.f;           // magic-biased origin of v = P - A for the current row
-    float Tlo = 0.f, Thi = 0.f;
+    float T = 0.f, band = 0.f;                       // r2 D2 and the half-width of the float test's error band
+    unsigned short* rec = nullptr;                   // hit record of the lane's seed in this brick
     float t0 = 0.f, t1 = 0.f, tl0 = 0.f, tl1 = 0.f;  // u interval of the line inside the brick / inside the layer
     float dty = 0.f, tyl = 0.f, tyh = 0.f, dtz = 0.f, tzl = 0.f, tzh = 0.f;
     float cyf = 1.f, cyhf = 0.f, czf = 0.f, czhf = -1.f;   // current / last row of the layer, current / last layer
@@ -704,13 +722,13 @@ k_brick(EmuDev P, FramePtrs F, int v0, const Brick* __restrict__ bricks, FindCtl
             dx = magic_lo16((unsigned)q.z) - (kMagicF + 2048.0f); dy = magic_hi16((unsigned)q.z) - (kMagicF + 2048.0f);
             dz = magic_lo16((unsigned)q.w) - (kMagicF + 2048.0f);
             // du >= 1 (the seed is oriented along +u and u is its dominant axis)
-            const float inv_dx = __fdividef(1.0f, dx);
+            const float inv_dx = rcp_fast(dx);
             a = dy * inv_dx;
             const float bz = dz * inv_dx;
             y0 = __fmaf_rn(-a, ax, ay);
             const float z0 = __fmaf_rn(-bz, ax, az);
-            const float inv_a = dy != 0.f ? __fdividef(dx, dy) : 0.0f;
-            const float inv_b = dz != 0.f ? __fdividef(dx, dz) : 0.0f;
+            const float inv_a = dy != 0.f ? dx * rcp_fast(dy) : 0.0f;
+            const float inv_b = dz != 0.f ? dx * rcp_fast(dz) : 0.0f;
             // clip the line against the brick's extent (already widened by R): an interval of u
             t0 = blo[0]; t1 = bhi[0];
             bool hit = true;
@@ -721,13 +739,13 @@ k_brick(EmuDev P, FramePtrs F, int v0, const Brick* __restrict__ bricks, FindCtl
             if (hit && t0 <= t1) {
               const float D2 = __fmaf_rn(dx, dx, __fmaf_rn(dy, dy, dz * dz));        // exact: < 2^22
               {
-                const float T = r2f * D2;
+                T = r2f * D2;
                 const float m_up = P.Rup * (dx + fabsf(dy) + fabsf(dz));
                 const float delta = __fmaf_rn(m_up, 4.76837158203125e-7f, 16.0f);   // 16 + 2^-21 m_up
-                const float band = __fmaf_rn(1.01f * delta, __fmaf_rn(2.0f, m_up, delta), T * 9.5367431640625e-7f);
-                Tlo = T - band; Thi = T + band;
+                band = __fmaf_rn(1.01f * delta, __fmaf_rn(2.0f, m_up, delta), T * 9.5367431640625e-7f);
               }
               sidx = idx; count = 0;
+              if (record) rec = recs + ((size_t)idx * (kRecBricks * kRecSlots) + rec_ord);
               if (kMode == kAssoc) {
                 const unsigned long long k1 = cand_k1((int)((unsigned)q.y >> 16), __float2int_rn(D2));
                 const unsigned ci = __ldg(item_ci + idx);            // the streamed list is the "walk" list
@@ -757,28 +775,29 @@ k_brick(EmuDev P, FramePtrs F, int v0, const Brick* __restrict__ bricks, FindCtl
         break;                                              // the slice is exhausted and every lane is done
       }
 
-      // ---------------- ROW: lanes whose run is used up move to the next row of cells ----------------
+      // ---------------- LAYER: lanes that have used up the rows of their w layer move to the next one ----------------
       if (!idle && j >= e) {
-        cyf += 1.0f; rowp += row_b; oym -= P.csf[1];
-        if (cyf > cyhf) {                                   // next w layer of the brick
-          czf += 1.0f; ozm -= P.csf[2]; layp += lay_b;
-          if (czf > czhf) {                                 // the seed is finished
-            if (kMode == kVote && count) atomicAdd(seed_cnt + sidx, (unsigned long long)min(count, 0xffff) << ord_shift);
-            idle = true;
-          } else {
-            tl0 = fmaxf(t0, __fmaf_rn(czf, dtz, tzl)); tl1 = fminf(t1, __fmaf_rn(czf, dtz, tzh));
-            cyf = 1.f; cyhf = 0.f;
-            if (tl0 <= tl1) {
-              const float ya = __fmaf_rn(a, tl0, y0), yb = __fmaf_rn(a, tl1, y0);
-              const int cyi = max(B.cy0, rn_int(__fmaf_rn(fminf(ya, yb), P.inv_cs[1], P.klo[1])));
-              cyhf = fminf(cy1f, rn_flt(__fmaf_rn(fmaxf(ya, yb), P.inv_cs[1], P.khi[1])));
-              cyf = int_f(cyi);
-              rowp = layp + (unsigned)cyi * row_b;
-              oym = __fmaf_rn(-cyf, P.csf[1], ay + kMagicF);
-            }
+       if (cyf >= cyhf) {
+        czf += 1.0f; ozm -= P.csf[2]; layp += lay_b;
+        if (czf > czhf) {                                   // the seed is finished
+          if (kMode == kVote && count) atomicAdd(seed_cnt + sidx, (unsigned long long)min(count, 0xffff) << ord_shift);
+          idle = true;
+        } else {
+          tl0 = fmaxf(t0, __fmaf_rn(czf, dtz, tzl)); tl1 = fminf(t1, __fmaf_rn(czf, dtz, tzh));
+          cyf = 1.f; cyhf = 0.f;                            // an empty layer: stepped over in the next round
+          if (tl0 <= tl1) {
+            const float ya = __fmaf_rn(a, tl0, y0), yb = __fmaf_rn(a, tl1, y0);
+            const int cyi = max(B.cy0, rn_int(__fmaf_rn(fminf(ya, yb), P.inv_cs[1], P.klo[1]))) - 1;   // the row before the first
+            cyhf = fminf(cy1f, rn_flt(__fmaf_rn(fmaxf(ya, yb), P.inv_cs[1], P.khi[1])));
+            cyf = int_f(cyi);
+            rowp = layp + (unsigned)cyi * row_b;
+            oym = __fmaf_rn(-cyf, P.csf[1], ay + kMagicF);
           }
         }
-        if (!idle && cyf <= cyhf) {                         // row cyf of layer czf
+       }
+        // ---------------- ROW: ... and to the next row of cells of their layer ----------------
+        if (!idle && cyf < cyhf) {
+          cyf += 1.0f; rowp += row_b; oym -= P.csf[1];
           const float ta = fmaxf(tl0, __fmaf_rn(cyf, dty, tyl)), tb = fminf(tl1, __fmaf_rn(cyf, dty, tyh));
           if (ta <= tb) {
             const int c0 = max(B.cx0, rn_int(__fmaf_rn(ta, P.inv_cs[0], P.klo[0])));
@@ -791,36 +810,41 @@ k_brick(EmuDev P, FramePtrs F, int v0, const Brick* __restrict__ bricks, FindCtl
           }
         }
       }
-
-      // ---------------- TEST: up to two grains of the pending run ----------------
-      if (j < e) {
-        const unsigned g0 = lds_u32(j), g1 = lds_u32_off4(j);   // g1 may lie beyond the run (still inside the pool)
-        const bool two = j + 4u < e;
-        float v0x, v0y, v0z, v1x, v1y, v1z;
-        const float s0 = tube_s(g0, v0x, v0y, v0z), s1 = tube_s(g1, v1x, v1y, v1z);
-        bool in0 = s0 <= Tlo, in1 = s1 <= Tlo;
-        if ((s0 > Tlo && s0 <= Thi) || (s1 > Tlo && s1 <= Thi)) {      // inside the error band: the exact predicate
-          if (s0 > Tlo && s0 <= Thi) in0 = exact_in(v0x, v0y, v0z);
-          if (s1 > Tlo && s1 <= Thi) in1 = exact_in(v1x, v1y, v1z);
-        }
-        in1 = in1 && two;
-        if (kMode == kVote) {
-          if (record && (in0 || in1)) {
-            // write down the brick slots of the grains found (the first kRecSlots of this seed in this brick)
-            unsigned short* rec = recs + ((size_t)sidx * (kRecBricks * kRecSlots) + rec_ord);
-            const unsigned slot = (j - pool_a) >> 2;
-            if (in0 && count < kRecSlots) rec[count] = (unsigned short)slot;
-            const int c1 = count + (int)in0;
-            if (in1 && c1 < kRecSlots) rec[c1] = (unsigned short)(slot + 1u);
+      // ---------------- TEST: up to kPairs pairs of grains of the pending run ----------------
+      {
+#pragma unroll 1
+        for (int pr = 0; pr < kPairs; ++pr) {
+          if (j >= e) break;
+          {
+            const unsigned g0 = lds_u32(j), g1 = lds_u32_off4(j);   // g1 may lie beyond the run (still inside the pool)
+            float v0x, v0y, v0z, v1x, v1y, v1z;
+            const float s0 = tube_s(g0, v0x, v0y, v0z), s1 = tube_s(g1, v1x, v1y, v1z);
+            bool in0 = s0 <= T, in1 = s1 <= T;
+            if (fminf(fabsf(s0 - T), fabsf(s1 - T)) <= band) {     // inside the error band: the exact predicate
+              if (fabsf(s0 - T) <= band) in0 = exact_in(v0x, v0y, v0z);
+              if (fabsf(s1 - T) <= band) in1 = exact_in(v1x, v1y, v1z);
+            }
+            in1 = in1 && (j + 4u < e);
+            if (kMode == kVote) {
+              if (record) {
+                // write down the brick slots of the grains found (the first kRecSlots of this seed in this brick)
+                const unsigned slot = (j - pool_a) >> 2;
+                if (in0) rec[min(count, kRecSlots - 1)] = (unsigned short)slot;
+                count += (int)in0;
+                if (in1) rec[min(count, kRecSlots - 1)] = (unsigned short)(slot + 1u);
+                count += (int)in1;
+              } else {
+                count += (int)in0 + (int)in1;
+              }
+            } else if (in0 || in1) {
+              // slot of the grain in the brick + (sorted position - slot) of the first grain of its row -> row of the grain
+              const int pos = (int)((j - pool_a) >> 2) + (int)lds_u32(rowp + delta_o);
+              if (in0) { const int row = __ldg(&sorted[pos].w); atomicMax(keyA + row, ka); atomicMax(keyB + row, kb); }
+              if (in1) { const int row = __ldg(&sorted[pos + 1].w); atomicMax(keyA + row, ka); atomicMax(keyB + row, kb); }
+            }
+            j += 8u;
           }
-          count += (int)in0 + (int)in1;
-        } else if (in0 || in1) {
-          // slot of the grain in the brick + (sorted position - slot) of the first grain of its row -> row of the grain
-          const int pos = (int)((j - pool_a) >> 2) + (int)lds_u32(rowp + delta_o);
-          if (in0) { const int row = __ldg(&sorted[pos].w); atomicMax(keyA + row, ka); atomicMax(keyB + row, kb); }
-          if (in1) { const int row = __ldg(&sorted[pos + 1].w); atomicMax(keyA + row, ka); atomicMax(keyB + row, kb); }
         }
-        j += 8u;
       }
     }
     n_tests += item_tests >> 2;
