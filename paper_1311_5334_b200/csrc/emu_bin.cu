@@ -94,6 +94,217 @@ k_bin_place(EmuDev P, int frame, const int4* __restrict__ tmp, const int* __rest
   }
 }
 
+// ---------------------------------------------------------------------------------------------
+// The fast path: ONE kernel, one block per view.  The per-cell counters of a view live in shared memory
+// as BYTES (four to a word), so the histogram and the scatter cursors never touch HBM; the grains are
+// read twice (the second time mostly from L2: a view is about 1 MB) and written once, cell_start is
+// written once and read back from L2.
+//   A  histogram: byte counters (a cell that overflows 255 sends the view to the slow variant)
+//   B  exclusive scan over the cells, four cells per thread and tile -> cell_start
+//   C  scatter: position = cell_start[cell] + (counter-- - 1); the order inside a cell is arbitrary
+//   D  canonical order inside a cell (ascending row): cells of 2..8 grains are sorted in place by
+//      one thread, larger ones by the whole block through the scratch array
+// kSmem = false is the same algorithm with 32-bit counters in global memory, for the views the fast
+// variant flagged (redo[v] != 0).
+constexpr int kViewThreads = 512;
+constexpr int kUnroll = 8;                          // independent grain loads per thread (the kernel is latency-bound otherwise)
+constexpr int kSmallCell = 8;
+constexpr int kBigCap = 64;
+#ifndef EMU_BIN_SMEM_CELLS
+#define EMU_BIN_SMEM_CELLS (200 * 1024)
+#endif
+constexpr int kMaxSmemCells = EMU_BIN_SMEM_CELLS;          // byte counters that fit the shared memory of one block
+
+template <bool kSmem>
+__global__ void __launch_bounds__(kViewThreads)
+k_bin_view(EmuDev P, int frame, const int4* __restrict__ grains, const int* __restrict__ view_off, int n_views,
+           int n_grains, int4* __restrict__ sorted, int* __restrict__ cell_start, int* __restrict__ gcount,
+           int4* __restrict__ tmp, int* __restrict__ redo, unsigned long long* __restrict__ status) {
+  extern __shared__ unsigned cnt_s[];               // kSmem: ceil(ncell / 4) words of byte counters
+  __shared__ int warp_sum[kViewThreads / 32];
+  __shared__ int carry_s, flag_s, nbig_s;
+  __shared__ int big_s[kBigCap];
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  const int ncell = P.fr[frame].ncell;
+  const int nwords = (ncell + 3) >> 2;
+  bool bad = false;
+
+  for (int v = blockIdx.x; v < n_views; v += gridDim.x) {
+    if (!kSmem && redo[v] == 0) continue;
+    const int g0 = __ldg(view_off + v), g1 = __ldg(view_off + v + 1);
+    const size_t cbase = (size_t)v * ncell;
+    int* gc = kSmem ? nullptr : gcount + cbase;
+    // ---- zero the counters ----
+    if (kSmem) { for (int w = tid; w < nwords; w += kViewThreads) cnt_s[w] = 0u; }
+    else { for (int c = tid; c < ncell; c += kViewThreads) gc[c] = 0; }
+    if (tid == 0) { flag_s = 0; nbig_s = 0; carry_s = g0; }
+    __syncthreads();
+    // ---- A: histogram ----
+    bool ovf = false;
+    for (int i0 = g0 + tid; i0 < g1; i0 += kUnroll * kViewThreads) {
+      int4 gg[kUnroll];
+#pragma unroll
+      for (int u = 0; u < kUnroll; ++u) {              // kUnroll independent 16-byte loads in flight per thread
+        const int i = i0 + u * kViewThreads;
+        gg[u] = i < g1 ? __ldg(grains + i) : make_int4(0, 0, 0, 0);
+      }
+#pragma unroll
+      for (int u = 0; u < kUnroll; ++u) {
+        if (i0 + u * kViewThreads >= g1) break;
+        const int4 g = emu_to_frame(frame, gg[u]);
+        bad |= (abs(g.x) >= (1 << 17)) | (abs(g.y) >= (1 << 17)) | (abs(g.z) >= (1 << 17));
+        const int c = emu_cell_of_frame(P, frame, g.x, g.y, g.z);
+        if (kSmem) {
+          const int sh = 8 * (c & 3);
+          const unsigned old = atomicAdd(&cnt_s[c >> 2], 1u << sh);
+          ovf |= ((old >> sh) & 0xffu) == 0xffu;
+        } else {
+          atomicAdd(gc + c, 1);
+        }
+      }
+    }
+    if (kSmem) {
+      if (ovf) flag_s = 1;
+      __syncthreads();
+      if (flag_s) {                                   // a cell holds more than 255 grains: the slow variant redoes the view
+        if (tid == 0) redo[v] = 1;
+        __syncthreads();
+        continue;
+      }
+    } else {
+      __syncthreads();
+    }
+    // ---- B: exclusive scan, four cells per thread and tile ----
+    for (int w0 = 0; w0 < nwords; w0 += kViewThreads) {
+      const int w = w0 + tid;
+      int c4[4] = {0, 0, 0, 0};
+      if (w < nwords) {
+        if (kSmem) {
+          const unsigned x = cnt_s[w];
+          c4[0] = x & 0xff; c4[1] = (x >> 8) & 0xff; c4[2] = (x >> 16) & 0xff; c4[3] = x >> 24;
+        } else {
+#pragma unroll
+          for (int k = 0; k < 4; ++k) if (4 * w + k < ncell) c4[k] = gc[4 * w + k];
+        }
+      }
+      const int mine = c4[0] + c4[1] + c4[2] + c4[3];
+      int incl = mine;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(EMU_FULL, incl, o); if (lane >= o) incl += y; }
+      if (lane == 31) warp_sum[wid] = incl;
+      __syncthreads();
+      if (wid == 0) {
+        int x = (lane < kViewThreads / 32) ? warp_sum[lane] : 0, xi = x;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(EMU_FULL, xi, o); if (lane >= o) xi += y; }
+        if (lane < kViewThreads / 32) warp_sum[lane] = xi - x;
+      }
+      __syncthreads();
+      int run = carry_s + warp_sum[wid] + incl - mine;
+      if (w < nwords) {
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+          if (4 * w + k < ncell) cell_start[cbase + 4 * w + k] = run;
+          run += c4[k];
+        }
+      }
+      __syncthreads();
+      if (tid == kViewThreads - 1) carry_s = run;
+      __syncthreads();
+    }
+    // ---- C: scatter.  The counters start again from zero and count up: a grain's rank inside its cell is the old
+    //      value, and afterwards every counter holds its cell's count again (phase D reads it) ----
+    if (kSmem) { for (int w = tid; w < nwords; w += kViewThreads) cnt_s[w] = 0u; }
+    else { for (int c = tid; c < ncell; c += kViewThreads) gc[c] = 0; }
+    __syncthreads();
+    for (int i0 = g0 + tid; i0 < g1; i0 += kUnroll * kViewThreads) {
+      int4 gg[kUnroll];
+      int start[kUnroll], rank[kUnroll];
+#pragma unroll
+      for (int u = 0; u < kUnroll; ++u) {
+        const int i = i0 + u * kViewThreads;
+        gg[u] = i < g1 ? __ldg(grains + i) : make_int4(0, 0, 0, 0);
+      }
+#pragma unroll
+      for (int u = 0; u < kUnroll; ++u) {              // all the cell_start loads are issued before any is used
+        const int i = i0 + u * kViewThreads;
+        start[u] = -1; rank[u] = 0;
+        if (i < g1) {
+          gg[u] = emu_to_frame(frame, gg[u]);
+          const int c = emu_cell_of_frame(P, frame, gg[u].x, gg[u].y, gg[u].z);
+          start[u] = cell_start[cbase + c];
+          if (kSmem) {
+            const int sh = 8 * (c & 3);
+            rank[u] = (int)((atomicAdd(&cnt_s[c >> 2], 1u << sh) >> sh) & 0xffu);
+          } else {
+            rank[u] = atomicAdd(gc + c, 1);
+          }
+          if (frame == 0) gg[u].w = i;                // payload replaced by the row; frames 1, 2 carry it already
+        }
+      }
+#pragma unroll
+      for (int u = 0; u < kUnroll; ++u) if (start[u] >= 0) sorted[start[u] + rank[u]] = gg[u];
+    }
+    __syncthreads();
+    // ---- D: ascending row inside every cell (only cells of two or more grains touch memory) ----
+    for (int w = tid; w < nwords; w += kViewThreads) {
+      int c4[4] = {0, 0, 0, 0};
+      if (kSmem) {
+        const unsigned x = cnt_s[w];
+        if (!((x + 0x7e7e7e7eu) & 0x80808080u) && !(x & 0x80808080u)) continue;    // every byte is 0 or 1
+        c4[0] = x & 0xff; c4[1] = (x >> 8) & 0xff; c4[2] = (x >> 16) & 0xff; c4[3] = x >> 24;
+      } else {
+#pragma unroll
+        for (int k = 0; k < 4; ++k) if (4 * w + k < ncell) c4[k] = gc[4 * w + k];
+      }
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        const int n = c4[k];
+        if (n < 2) continue;
+        const int c = 4 * w + k;
+        int slot = kBigCap;
+        if (n > kSmallCell) slot = atomicAdd(&nbig_s, 1);
+        if (slot < kBigCap) { big_s[slot] = c; continue; }
+        const int s = cell_start[cbase + c];
+        if (n == 2) {                                 // the common case: one compare, at most one swap
+          const int4 p = sorted[s], q = sorted[s + 1];
+          if (q.w < p.w) { sorted[s] = q; sorted[s + 1] = p; }
+          continue;
+        }
+        for (int i = 1; i < n; ++i) {                 // insertion sort in place
+          const int4 key = sorted[s + i];
+          int j = i - 1;
+          while (j >= 0) {
+            const int4 q = sorted[s + j];
+            if (q.w <= key.w) break;
+            sorted[s + j + 1] = q;
+            --j;
+          }
+          if (j != i - 1) sorted[s + j + 1] = key;
+        }
+      }
+    }
+    __syncthreads();
+    const int nbig = min(nbig_s, kBigCap);
+    for (int b = 0; b < nbig; ++b) {                  // big cells: rank sort by the whole block through tmp
+      const int c = big_s[b];
+      const int s = cell_start[cbase + c];
+      const int e = (c + 1 < ncell) ? cell_start[cbase + c + 1] : g1;
+      for (int i = s + tid; i < e; i += kViewThreads) {
+        const int4 g = sorted[i];
+        int rank = 0;
+        for (int k = s; k < e; ++k) rank += (sorted[k].w < g.w);
+        tmp[s + rank] = g;
+      }
+      __syncthreads();
+      for (int i = s + tid; i < e; i += kViewThreads) sorted[i] = tmp[i];
+      __syncthreads();
+    }
+  }
+  if (status && __any_sync(EMU_FULL, bad) && lane == 0) atomicOr(status, (unsigned long long)EMU_ST_COORD);
+  if (kSmem && blockIdx.x == 0 && tid == 0) cell_start[(size_t)n_views * ncell] = n_grains;
+}
+
 }  // namespace
 
 size_t emu_bin_ws_bytes(const EmuDev& P, int64_t n_grains, int32_t n_views) {
@@ -101,7 +312,8 @@ size_t emu_bin_ws_bytes(const EmuDev& P, int64_t n_grains, int32_t n_views) {
   for (int f = 1; f < 3; ++f) if (P.fr[f].ncell > ncell) ncell = P.fr[f].ncell;     // one scratch serves every frame
   size_t cnt = emu_align256((size_t)n_views * ncell * sizeof(int));
   size_t tmp = emu_align256((size_t)n_grains * sizeof(int4));
-  return cnt + tmp + 256;
+  size_t redo = emu_align256(((size_t)n_views + 1) * sizeof(int));
+  return cnt + tmp + redo + 256;
 }
 
 int emu_bin_launch(const EmuDev& P, int frame, const int32_t* d_grains, const int32_t* d_view_off, int64_t n_grains,
@@ -111,8 +323,25 @@ int emu_bin_launch(const EmuDev& P, int frame, const int32_t* d_grains, const in
   char* ws = (char*)emu_align_ptr(d_ws);
   int* count = (int*)ws;
   const int ncell = P.fr[frame].ncell;
-  int4* tmp = (int4*)(ws + emu_align256((size_t)n_views * ncell * sizeof(int)));
+  int ncell_max = P.fr[0].ncell;
+  for (int f = 1; f < 3; ++f) if (P.fr[f].ncell > ncell_max) ncell_max = P.fr[f].ncell;
+  int4* tmp = (int4*)(ws + emu_align256((size_t)n_views * ncell_max * sizeof(int)));
+  int* redo = (int*)((char*)tmp + emu_align256((size_t)n_grains * sizeof(int4)));
   const int n = (int)n_grains;
+  if (ncell <= kMaxSmemCells) {
+    // one block per view, byte counters in shared memory; the views it flags are redone with global counters
+    const size_t smem = (size_t)((ncell + 3) / 4) * 4;
+    if (cudaFuncSetAttribute(k_bin_view<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return EMU_ERR_CUDA;
+    if (cudaMemsetAsync(redo, 0, ((size_t)n_views + 1) * sizeof(int), st) != cudaSuccess) return EMU_ERR_CUDA;
+    const int blocks = (int)emu_max64(1, emu_min64(n_views, 148 * 8));
+    EMU_LAUNCH(frame == 0 ? EMU_STAGE_BIN_SCATTER : EMU_STAGE_PREP, st, k_bin_view<true><<<blocks, kViewThreads, smem, st>>>(
+        P, frame, (const int4*)d_grains, d_view_off, n_views, n, (int4*)d_sorted, d_cell_start, count, tmp, redo,
+        (unsigned long long*)d_status));
+    EMU_LAUNCH(frame == 0 ? EMU_STAGE_BIN_PLACE : EMU_STAGE_PREP, st, k_bin_view<false><<<blocks, kViewThreads, 0, st>>>(
+        P, frame, (const int4*)d_grains, d_view_off, n_views, n, (int4*)d_sorted, d_cell_start, count, tmp, redo,
+        (unsigned long long*)d_status));
+    return cudaGetLastError() == cudaSuccess ? EMU_OK : EMU_ERR_CUDA;
+  }
   if (cudaMemsetAsync(count, 0, (size_t)n_views * ncell * sizeof(int), st) != cudaSuccess) return EMU_ERR_CUDA;
   int blocks = (int)emu_min64((n_grains + kBinThreads - 1) / kBinThreads, 148 * 16);
   if (blocks < 1) blocks = 1;
