@@ -950,24 +950,35 @@ k_assoc_hits(int v0, const FindCtl* __restrict__ ctl, const unsigned* __restrict
   if (ctl->skip || ctl->generic || ctl->norecord) return;
   const int vf = blockIdx.y;
   const unsigned lo = view_cand_off[vf], hi = view_cand_off[vf + 1];
-  for (unsigned ci = lo + blockIdx.x * blockDim.x + threadIdx.x; ci < hi; ci += gridDim.x * blockDim.x) {
+  // one thread per (candidate, brick ordinal): the record is read with two 16-byte loads, the rows of its grains
+  // with independent loads, and the priorities leave as fire-and-forget atomics (no thread waits on one)
+  const unsigned n4 = (hi - lo) * (unsigned)kRecBricks;
+  for (unsigned t = blockIdx.x * blockDim.x + threadIdx.x; t < n4; t += gridDim.x * blockDim.x) {
+    const unsigned ci = lo + t / (unsigned)kRecBricks;
+    const int ord = (int)(t % (unsigned)kRecBricks);
     const unsigned i = cand_seed[ci];
     const unsigned long long v = seed_cnt[i];
     if (tube_overflows(v)) continue;                        // walked by k_brick<kAssoc>
+    const int cnt = (int)((v >> (16 * ord)) & 0xffffu);
+    if (!cnt) continue;
     const Cand c = cands[ci];
     const unsigned long long k1 = cand_k1(c.n_tube_view & 0xffff, c.d2);
     const unsigned long long ka = (k1 << kCiBits) | (unsigned long long)(kCiMask - ci);
     const unsigned long long kb = (k1 << kCiBits) | (unsigned long long)ci;
+    const int base = vf_brick_base[vf * kRecBricks + ord];
+    const uint4* rec = reinterpret_cast<const uint4*>(recs + ((size_t)i * (kRecBricks * kRecSlots) + (size_t)ord * kRecSlots));
+    const uint4 r0 = __ldg(rec);
+    const uint4 r1 = cnt > 8 ? __ldg(rec + 1) : make_uint4(0u, 0u, 0u, 0u);
+    const unsigned w[8] = {r0.x, r0.y, r0.z, r0.w, r1.x, r1.y, r1.z, r1.w};
+    int rows[kRecSlots];
 #pragma unroll
-    for (int ord = 0; ord < kRecBricks; ++ord) {
-      const int cnt = (int)((v >> (16 * ord)) & 0xffffu);
-      if (!cnt) continue;
-      const int base = vf_brick_base[vf * kRecBricks + ord];
-      const unsigned short* rec = recs + ((size_t)i * (kRecBricks * kRecSlots) + (size_t)ord * kRecSlots);
-      for (int k = 0; k < cnt; ++k) {
-        const int row = slot_row[base + (int)rec[k]];
-        atomicMax(keyA + row, ka); atomicMax(keyB + row, kb);
-      }
+    for (int k = 0; k < kRecSlots; ++k) {
+      const int slot = (int)((w[k >> 1] >> (16 * (k & 1))) & 0xffffu);
+      rows[k] = k < cnt ? slot_row[base + slot] : -1;
+    }
+#pragma unroll
+    for (int k = 0; k < kRecSlots; ++k) {
+      if (rows[k] >= 0) { atomicMax(keyA + rows[k], ka); atomicMax(keyB + rows[k], kb); }
     }
   }
 }
@@ -1499,22 +1510,26 @@ static int carve(const EmuDev& P, const Tilings& TT, Hints hints, int64_t n_grai
   const int64_t spv = per_view_g * hints.seeds_per_grain, cpv = per_view_g * hints.cand_per_grain;
   // views per chunk: the most whose expected seeds and candidates fit what is left after the fixed part
   // (3 groups per view must fit the 65 535 blocks of grid.y)
-  int vpc = n_views > 0 ? (int)emu_min64(n_views, 21000) : 1;
   size_t seed_cap = 0, cand_cap = 0;
-  for (;;) {
+  auto fits = [&](int vpc, bool relaxed) {
     const size_t fx = fixed_bytes(P, TT, n_grains, n_views, vpc) + 16 * 256;
-    if (fx + kMinSeedCap * kSeedBytes + kMinCandCap * kCandBytes <= ws_bytes) {
-      const size_t avail = ws_bytes - fx;
-      // what is available is split between seeds and candidates in the proportion of the hints
-      const double ws_seed = (double)spv * kSeedBytes, ws_cand = (double)cpv * kCandBytes;
-      seed_cap = (size_t)((double)avail * ws_seed / (ws_seed + ws_cand) / kSeedBytes);
-      if (seed_cap < kMinSeedCap) seed_cap = kMinSeedCap;
-      cand_cap = (avail - seed_cap * kSeedBytes) / kCandBytes;
-      if (cand_cap >= kMinCandCap && ((int64_t)seed_cap >= spv * vpc || vpc == 1)) break;
-    }
-    if (vpc == 1) return EMU_ERR_CAPACITY;
-    vpc = (vpc + 1) / 2;
+    if (fx + kMinSeedCap * kSeedBytes + kMinCandCap * kCandBytes > ws_bytes) return false;
+    const size_t avail = ws_bytes - fx;
+    // what is available is split between seeds and candidates in the proportion of the hints
+    const double ws_seed = (double)spv * kSeedBytes, ws_cand = (double)cpv * kCandBytes;
+    seed_cap = (size_t)((double)avail * ws_seed / (ws_seed + ws_cand) / kSeedBytes);
+    if (seed_cap < kMinSeedCap) seed_cap = kMinSeedCap;
+    cand_cap = (avail - seed_cap * kSeedBytes) / kCandBytes;
+    return cand_cap >= kMinCandCap && ((int64_t)seed_cap >= spv * vpc || relaxed);
+  };
+  int lo = 1, hi = n_views > 0 ? (int)emu_min64(n_views, 21000) : 1;
+  if (!fits(1, true)) return EMU_ERR_CAPACITY;
+  while (lo < hi) {                                   // the largest chunk that fits (the predicate is monotone)
+    const int mid = lo + (hi - lo + 1) / 2;
+    if (fits(mid, false)) lo = mid; else hi = mid - 1;
   }
+  const int vpc = lo;
+  fits(vpc, vpc == 1);                                // sets seed_cap / cand_cap for the chunk size chosen
   if (cand_cap > (size_t)kCiMask) cand_cap = kCiMask;
   if (seed_cap > (size_t)0x7fffffff) seed_cap = 0x7fffffff;
   char* p = (char*)emu_align_ptr(d_ws);
@@ -1687,7 +1702,7 @@ int emu_find_launch(const EmuDev& P, int seeds_per_grain, int cand_per_grain, co
     EMU_LAUNCH(EMU_STAGE_PREP, st, k_reset_cand_arrays<<<kSM * 8, 256, 0, st>>>(W.ctl, W.wins, W.cand_track));
     // A5
     EMU_CK(cudaFuncSetAttribute(k_brick<kAssoc>, cudaFuncAttributeMaxDynamicSharedMemorySize, kPoolBytes));
-    EMU_LAUNCH(EMU_STAGE_ASSOC, st, k_assoc_hits<<<dim3(8, 3 * nv), 256, 0, st>>>(
+    EMU_LAUNCH(EMU_STAGE_ASSOC, st, k_assoc_hits<<<dim3(48, 3 * nv), 256, 0, st>>>(
         v0, W.ctl, W.view_cand_off, W.cands, W.cand_seed, W.seed_cnt, W.recs, W.slot_row, W.vf_brick_base, W.keyA, W.keyB));
     EMU_LAUNCH(EMU_STAGE_ASSOC, st, k_brick<kAssoc><<<kSM, kBrickThreads, kPoolBytes, st>>>(
         P, F, v0, W.bricks, W.ctl, slices, W.ovf_geo, W.ovf_ci, W.view_ovf_off, nullptr, nullptr, nullptr, W.keyA, W.keyB,
