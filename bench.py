@@ -35,7 +35,10 @@ VIEW_AREA_CM2 = 350e-4 * 300e-4  # 350 x 300 um = 1.05e-3 cm^2 per view
 # them live; the constants serve the runs that have no such leg (N > 1).
 ALG_PER_SEED = {(8.0, 8.0, 8.0): (317.7, 2.88), (3.0, 4.0, 4.0): (102.1, 2.26)}
 INSTR_PER_TEST, INSTR_PER_PAIR = 18, 9
-BIN_BYTES_PER_GRAIN = 32.7       # 16 B read + 16 B written + 4 B per cell
+BIN_BYTES_PER_GRAIN = 32.0       # 16 B read + 16 B written per grain; + 4 B per cell of the grid
+# DRAM bytes (read + write) of one k_brick<kVote> launch per view of the launch, from the committed ncu --set full
+# capture profiles/r1c_k_brick_full.txt (24 views: 31.6 GB read + 21.1 GB written)
+VOTE_DRAM_BYTES_PER_VIEW = (31.616565e9 + 21.088184e9) / 24
 
 
 def _gen_view(v):
@@ -299,8 +302,13 @@ def main():
     if alg is not None and stage_launches["vote"]:
         alg_instr = seeds * (alg[0] * INSTR_PER_TEST + alg[1] * INSTR_PER_PAIR)   # per step, all vote launches
         achieved = alg_instr / (stage_ms["vote"] / args.steps * 1e-3) / 1e12
-        roofline = {"kernel": "k_brick<kVote> (A2 seeds are streamed in, A3 tube count, shared-memory bricks)", "bound": "alu", "achieved": achieved, "peak": alu_peak,
-                    "unit": "Tlane-instr/s", "frac": achieved / alu_peak, "traffic": None,
+        views_per_launch = V * args.steps / stage_launches["vote"]
+        roofline = {"kernel": "k_brick<kVote> (A2 seeds are streamed in, A3 tube count + hit records, shared-memory bricks, "
+                              "three frames)", "bound": "alu", "achieved": achieved, "peak": alu_peak,
+                    "unit": "Tlane-instr/s", "frac": achieved / alu_peak,
+                    "traffic": VOTE_DRAM_BYTES_PER_VIEW * views_per_launch,
+                    "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of profiles/r1c_k_brick_full.txt per view "
+                                      "x views per launch",
                     "peak_source": f"148 SM x 4 schedulers x 32 lanes x {sm_max:.0f} MHz ({peaks['_source']} max SM clock)",
                     "algorithmic": f"{seeds} seeds x ({alg[0]:.1f} tests x {INSTR_PER_TEST} + {alg[1]:.2f} pair tests x "
                                    f"{INSTR_PER_PAIR}) lane-instr, oracle counters at the same cell size",
@@ -308,9 +316,12 @@ def main():
                     "share_of_step": stage_ms["vote"] / args.steps / ms_step}
     bin_ms = sum(stage_ms[k] for k in ("bin_count", "bin_scan", "bin_scatter", "bin_place")) / args.steps
     hbm = float(peaks["hbm_gbs"])
-    bin_gbs = BIN_BYTES_PER_GRAIN * n / (bin_ms * 1e-3) / 1e9 if bin_ms > 0 else 0.0
-    roofline_bin = {"kernel": "emu_bin_grains (count+scan+scatter+place)", "bound": "hbm", "achieved": bin_gbs,
-                    "peak": hbm, "unit": "GB/s", "frac": bin_gbs / hbm, "traffic": None, "ms": bin_ms,
+    ncell = int(E.emu_grid_cells(prm)[0])
+    bin_bytes = BIN_BYTES_PER_GRAIN * n + 4.0 * ncell * V
+    bin_gbs = bin_bytes / (bin_ms * 1e-3) / 1e9 if bin_ms > 0 else 0.0
+    roofline_bin = {"kernel": "emu_bin_grains: k_bin_view (one block per view, byte counters in shared memory)", "bound": "hbm",
+                    "achieved": bin_gbs, "peak": hbm, "unit": "GB/s", "frac": bin_gbs / hbm, "traffic": None, "ms": bin_ms,
+                    "algorithmic_bytes_per_grain": bin_bytes / max(1, n),
                     "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peaks['_source']})"}
 
     val = n_total / (ms_step * 1e-3)

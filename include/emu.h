@@ -39,6 +39,9 @@ typedef struct emu_params {
   int32_t view_size_q[3];      /* box [0,size) per axis; 1 <= size <= 65536 (1024 um)                      */
   int32_t cell_size_q[3];      /* > 0.  Paper: 32 px x 32 px x 1 frame.  Has NO effect on the      */
                                /* track list (reading Q10); it only steers the speed of the search.        */
+                               /* emu_find_tracks bins every view twice more with permuted axes (y,x,z)    */
+                               /* and (z,x,y) and applies the SAME triple to the permuted coordinates:     */
+                               /* [0] = size along a line's dominant axis, [1], [2] = across it.           */
   int32_t sep_min_q;           /* seed <=> sep_min_q^2 <= D2 < sep_max_q^2 (reading Q1; "smaller      */
   int32_t sep_max_q;           /*  than 25 um" = 1600).  1 <= sep_min_q < sep_max_q <= 2048                */
   int32_t tube_r2_q;           /* tube radius squared, q^2; 0.8 um -> floor(0.64*4096) = 2621 (reading Q3) */
@@ -46,8 +49,9 @@ typedef struct emu_params {
   int32_t min_grains;          /* threshold, >= 2: n >= min_grains (reading Q6; "e.g. 5")             */
   int32_t max_tracks_per_view; /* capacity of the track list per view, 1..65536                            */
   int32_t reserved[4];         /* sizing hints for the internal chunks of emu_find_tracks:                 */
-                               /* [0] = expected candidates per grain (0 = default 48),                    */
-                               /* [1] = expected seeds per grain (0 = default 192); [2], [3] must be 0     */
+                               /* [0] = expected candidates per grain (0 = default 48; 48 B each),         */
+                               /* [1] = expected seeds per grain (0 = default 192; 160 B each: geometry,   */
+                               /*       counter and the hit record of the voting pass); [2], [3] must be 0 */
 } emu_params;
 
 typedef struct emu_track {     /* 32 B */

@@ -33,9 +33,12 @@ def _mess_up(g, size_q):
     return g
 
 
+# (200, 200, 100) um: one cell per view with about 1 700 grains - the byte counters of the fast binning kernel
+# overflow and the view is redone with 32-bit counters; (40, 2, 60) um: about 20 grains per cell (block rank sort)
 @pytest.mark.parametrize("cfg,cell_um,messy", [(0, (8.0, 8.0, 8.0), False), (0, (3.0, 17.0, 5.5), True),
                                                (1, (8.0, 8.0, 8.0), False), (1, (4.0, 4.0, 4.0), True),
-                                               (3, (40.0, 2.0, 60.0), False)])
+                                               (3, (40.0, 2.0, 60.0), False), (0, (200.0, 200.0, 100.0), False),
+                                               (1, (3.0, 4.0, 4.0), False)])
 def test_binning_bit_exact(E, oracle_mod, cfg, cell_um, messy):
     b = make_batch(CONFIGS[cfg], cfg, n_views=3 if cfg == 0 else 1)
     p = default_params(cfg, cell_um=cell_um)
@@ -77,6 +80,20 @@ def test_track_list_bit_exact(E, config_oracle, cfg, cell_um):
     got = run_gpu(E, p, b.grains, b.view_off)
     assert_same_tracks(E, got, ref)
     assert len(got["tracks"]) > 0
+
+
+@pytest.mark.parametrize("cell_um", [(2.0, 4.0, 4.0), (0.5, 4.0, 4.0)])
+def test_several_bricks_per_frame(E, config_oracle, cell_um):
+    """Config 1 with fine cells along u: the cell tables no longer fit one shared-memory brick.  2 um: two bricks per
+    (view, frame), hit records with two ordinals; 0.5 um: more than four bricks, the records are switched off and every
+    candidate is walked a second time.  Per-seed counts and the track list may not notice."""
+    b, p, ref = config_oracle(1)
+    p = dict(p, cell_size_q=default_params(1, cell_um=cell_um)["cell_size_q"])
+    dump, counts = seed_dump_gpu(E, p, b.grains, b.view_off, ref.counters["seeds"] + 16)
+    a = dump[np.lexsort((dump[:, 2], dump[:, 1], dump[:, 0]))]
+    r = ref.seed_dump[np.lexsort((ref.seed_dump[:, 2], ref.seed_dump[:, 1], ref.seed_dump[:, 0]))]
+    assert np.array_equal(a, r)
+    assert_same_tracks(E, run_gpu(E, p, b.grains, b.view_off), ref)
 
 
 @pytest.mark.parametrize("cell_um", [(4.0, 4.0, 4.0), (2.0, 16.0, 3.0), (100.0, 100.0, 50.0), (1.0, 9.0, 25.0)])
@@ -166,3 +183,46 @@ def test_capacity_and_range_errors_are_reported(E):
     prm = E.make_params((6400, 6400, 3200), (512, 512, 512), 256, 1280, 2621, 8, tube_ext_q=100)
     with pytest.raises(E.EmuError):
         E.emu_workspace_bytes(prm, 10, 1)
+
+
+def test_bench_workload_sampled_views(E, oracle_mod):
+    """BASELINE.json configs[4] as bench.py runs it (same generator, parameters, 3x4x4 um cells, recommended workspace,
+    hence the same kernels, frames, three bricks per frame and several internal chunks): 20 views through the CUDA
+    path; views 0, 9 and 19 are compared with the oracle element by element, and the properties that hold at any
+    size are checked on all of them."""
+    import bench
+    V = 20
+    grains, off = bench.make_workload(0, V)
+    p = bench.params_dict()
+    got = run_gpu(E, p, grains, off)
+    counts = got["counts"]
+    assert int(counts[E.EMU_CNT["status"]]) == 0
+    toff, tr, mem = got["track_off"], got["tracks"], got["members"]
+    assert toff[0] == 0 and np.all(np.diff(toff) >= 0) and toff[-1] == len(tr) == int(counts[E.EMU_CNT["tracks"]])
+    assert np.all(np.repeat(np.arange(V), np.diff(toff)) == tr["view"])
+    assert np.all(tr["n_members"] >= p["min_grains"]) and np.all(tr["n_tube"] >= tr["n_members"])
+    assert np.array_equal(tr["member_off"], np.concatenate(([0], np.cumsum(tr["n_members"])[:-1])))
+    assert len(mem) == int(tr["n_members"].sum()) and len(np.unique(mem)) == len(mem)        # exclusive association
+    mview = np.searchsorted(off, mem, side="right") - 1
+    assert np.array_equal(mview, np.repeat(tr["view"], tr["n_members"]))                     # members stay in their view
+    sample = [0, 9, 19]
+    sub = np.concatenate([grains[off[v]:off[v + 1]] for v in sample])
+    soff = np.zeros(len(sample) + 1, np.int32)
+    soff[1:] = np.cumsum([off[v + 1] - off[v] for v in sample])
+    ref = oracle_mod.track_views(p, sub, soff, "cells", len(sample))
+    for k, v in enumerate(sample):
+        shift = int(off[v]) - int(soff[k])
+        g = tr[toff[v]:toff[v + 1]]
+        r = ref.tracks[ref.track_off[k]:ref.track_off[k + 1]]
+        assert len(g) == len(r) and len(g) > 500
+        for f in ("n_tube", "n_members", "seed_d2"):
+            assert np.array_equal(g[f], r[f]), (v, f)
+        assert np.array_equal(g["seed_a"] - shift, r["seed_a"]) and np.array_equal(g["seed_b"] - shift, r["seed_b"])
+        gm = mem[g["member_off"][0]:g["member_off"][-1] + g["n_members"][-1]] - shift
+        rm = ref.members[r["member_off"][0]:r["member_off"][-1] + r["n_members"][-1]]
+        assert np.array_equal(gm, rm)
+        gf, rf = got["fits"][toff[v]:toff[v + 1]], ref.fits[ref.track_off[k]:ref.track_off[k + 1]]
+        for f in ("axis", "n", "u_min", "u_max"):
+            assert np.array_equal(gf[f], rf[f])
+        assert np.all(np.abs(gf["slope"] - rf["slope"]) <= 1e-5 * np.maximum(np.abs(gf["slope"]), np.abs(rf["slope"])) + 1e-12)
+        assert np.all(np.abs(gf["icpt"] - rf["icpt"]) <= 1e-5 * np.maximum(np.abs(gf["icpt"]), np.abs(rf["icpt"])) + 1e-6)
