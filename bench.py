@@ -257,6 +257,8 @@ def main():
     # end to end: ONE C-ABI call on pinned host buffers per step (H2D + path + D2H inside the call)
     e2e = None
     if not args.no_e2e:
+        del B                                               # one workspace at a time (each is sized for 180 GB of HBM)
+        torch.cuda.empty_cache()
         H = E.HostPath(prm, n, V)
         H.h_grains[:n].copy_(torch.from_numpy(grains))
         H.h_view_off.copy_(torch.from_numpy(off))

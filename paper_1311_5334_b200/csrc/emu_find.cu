@@ -43,6 +43,9 @@ constexpr int kMaxTube = 8191;                    // n_tube field of the packed 
 #ifndef EMU_BRICK_THREADS
 #define EMU_BRICK_THREADS 1024
 #endif
+#ifndef EMU_CHUNK_GIB
+#define EMU_CHUNK_GIB 96
+#endif
 #ifndef EMU_REFILL
 #define EMU_REFILL 8
 #endif
@@ -1495,8 +1498,8 @@ size_t emu_find_ws_recommended_bytes(const EmuDev& P, int64_t n_grains, int32_t 
   const int64_t per_view_g = emu_max64(1, (n_grains + emu_max64(1, n_views) - 1) / emu_max64(1, n_views));
   const int64_t spv = per_view_g * seeds_per_grain, cpv = per_view_g * cand_per_grain;
   const int64_t per_view_bytes = spv * (int64_t)kSeedBytes + cpv * (int64_t)kCandBytes;
-  // as many views per chunk as fit 48 GiB of seed / candidate storage (at least one)
-  int64_t vpc = emu_max64(1, emu_min64(emu_max64(1, n_views), ((int64_t)48 << 30) / emu_max64(1, per_view_bytes)));
+  // as many views per chunk as fit EMU_CHUNK_GIB (96) GiB of seed / candidate storage (at least one)
+  int64_t vpc = emu_max64(1, emu_min64(emu_max64(1, n_views), ((int64_t)EMU_CHUNK_GIB << 30) / emu_max64(1, per_view_bytes)));
   vpc = emu_min64(vpc, 21000);
   const size_t seed_cap = (size_t)emu_max64((int64_t)kMinSeedCap, spv * vpc);
   const size_t cand_cap = (size_t)emu_max64((int64_t)kMinCandCap, cpv * vpc);
