@@ -305,15 +305,219 @@ k_bin_view(EmuDev P, int frame, const int4* __restrict__ grains, const int* __re
   if (kSmem && blockIdx.x == 0 && tid == 0) cell_start[(size_t)n_views * ncell] = n_grains;
 }
 
+// ---------------------------------------------------------------------------------------------
+// The two-pass path (the default whenever its plan fits): HBM sees only streams.
+//   pass 1  k_bin_split: the cell range of a view is cut into K chunks of cpc cells; every grain goes to
+//           the scratch region of its (view, chunk).  A block takes tiles of 2 048 grains of one view (eight
+//           per thread, held in registers), counts them per chunk in shared memory, reserves its ranges
+//           with K atomics and writes the grains out: a tile leaves about 1 KB per chunk in one piece.
+//   pass 2  k_bin_chunk: one block per (view, chunk).  The chunk (<= kChunkCap grains) is read in a stream,
+//           counted per cell and scanned in shared memory (16-bit counters), placed into a shared-memory
+//           buffer in cell order, put into ascending row order inside every cell, and written out in a
+//           stream, with its part of cell_start.
+// A view with a chunk fuller than the scratch region is flagged and redone by k_bin_view<false>.
+constexpr int kSplitThreads = 256;
+constexpr int kSplitPer = 8;                         // grains per thread and tile
+constexpr int kChunkThreads = 256;
+constexpr int kChunkPer = 6;                         // grains per thread of a chunk block (held in registers)
+constexpr int kChunkCap = kChunkThreads * kChunkPer; // grains of a chunk: 1 536 = 24 KB of shared memory
+constexpr int kMaxChunks = 128;
+constexpr int kMaxChunkCells = 12288;                // cells of a chunk: 2 x 16 bits each in shared memory
+
+struct SplitPlan { int K, cpc, cap; float inv_cpc; };
+
+__device__ __forceinline__ int chunk_of(int cell, const SplitPlan& S) {
+  int k = (int)(((float)cell + 0.5f) * S.inv_cpc);    // cell < 2^24: within one of the truth
+  k -= (k * S.cpc > cell);
+  k += ((k + 1) * S.cpc <= cell);
+  return k;
+}
+
+__global__ void __launch_bounds__(kSplitThreads)
+k_bin_split(EmuDev P, int frame, SplitPlan S, const int4* __restrict__ grains, const int* __restrict__ view_off,
+            int n_views, int4* __restrict__ tmp, int* __restrict__ cur, int* __restrict__ redo,
+            unsigned long long* __restrict__ status) {
+  // grid = (tiles, views): block (t, v) takes tile t of view v; a view with more tiles than the grid has is flagged
+  __shared__ int hist_s[kMaxChunks], base_s[kMaxChunks];
+  const int tid = threadIdx.x;
+  const int v = blockIdx.y;
+  const int g0 = __ldg(view_off + v), g1 = __ldg(view_off + v + 1);
+  const int t0 = g0 + (int)blockIdx.x * (kSplitThreads * kSplitPer);
+  if (blockIdx.x == 0 && tid == 0 && (long long)(g1 - g0) > (long long)gridDim.x * (kSplitThreads * kSplitPer)) redo[v] = 1;
+  if (t0 >= g1) return;
+  bool bad = false;
+  int4 gg[kSplitPer];
+  int kk[kSplitPer], rr[kSplitPer];
+  if (tid < S.K) hist_s[tid] = 0;
+#pragma unroll
+  for (int u = 0; u < kSplitPer; ++u) {
+    const int i = t0 + u * kSplitThreads + tid;
+    gg[u] = i < g1 ? __ldg(grains + i) : make_int4(0, 0, 0, 0);
+  }
+  __syncthreads();
+#pragma unroll
+  for (int u = 0; u < kSplitPer; ++u) {
+    const int i = t0 + u * kSplitThreads + tid;
+    kk[u] = -1; rr[u] = 0;
+    if (i < g1) {
+      gg[u] = emu_to_frame(frame, gg[u]);
+      if (frame == 0) gg[u].w = i;                     // payload replaced by the row; frames 1, 2 carry it already
+      bad |= (abs(gg[u].x) >= (1 << 17)) | (abs(gg[u].y) >= (1 << 17)) | (abs(gg[u].z) >= (1 << 17));
+      kk[u] = chunk_of(emu_cell_of_frame(P, frame, gg[u].x, gg[u].y, gg[u].z), S);
+      rr[u] = atomicAdd(&hist_s[kk[u]], 1);
+    }
+  }
+  __syncthreads();
+  if (tid < S.K) {
+    const int h = hist_s[tid];
+    int b = 0;
+    if (h) {
+      b = atomicAdd(cur + (size_t)v * S.K + tid, h);
+      if (b + h > S.cap) redo[v] = 1;                  // the region is full: k_bin_view<false> redoes the view
+    }
+    base_s[tid] = b;
+  }
+  __syncthreads();
+#pragma unroll
+  for (int u = 0; u < kSplitPer; ++u) {
+    if (kk[u] < 0) continue;
+    const int slot = base_s[kk[u]] + rr[u];
+    if (slot < S.cap) tmp[((size_t)v * S.K + kk[u]) * S.cap + slot] = gg[u];
+  }
+  if (status && __any_sync(EMU_FULL, bad) && (tid & 31) == 0) atomicOr(status, (unsigned long long)EMU_ST_COORD);
+}
+
+__global__ void __launch_bounds__(kChunkThreads)
+k_bin_chunk(EmuDev P, int frame, SplitPlan S, const int* __restrict__ view_off, int n_views, int n_grains,
+            const int4* __restrict__ tmp, const int* __restrict__ cur, const int* __restrict__ redo,
+            int4* __restrict__ sorted, int* __restrict__ cell_start) {
+  extern __shared__ __align__(16) unsigned char chunk_smem[];
+  __shared__ int warp_sum[kChunkThreads / 32];
+  __shared__ int base_s;
+  const int k = blockIdx.x, v = blockIdx.y;
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  const int ncell = P.fr[frame].ncell;
+  if (k == 0 && v == 0 && tid == 0) cell_start[(size_t)n_views * ncell] = n_grains;
+  if (redo[v]) return;
+  const int c_lo = k * S.cpc, nc = min(ncell, c_lo + S.cpc) - c_lo;
+  if (nc <= 0) return;
+  int4* buf = reinterpret_cast<int4*>(chunk_smem);                                   // [cap]
+  unsigned short* cnt = reinterpret_cast<unsigned short*>(chunk_smem + (size_t)S.cap * 16);   // [cpc] counts
+  unsigned short* pre = cnt + ((S.cpc + 1) & ~1);                                    // [cpc] exclusive prefix
+  unsigned* cntw = reinterpret_cast<unsigned*>(cnt);
+  const int n = min(cur[(size_t)v * S.K + k], S.cap);
+  const int4* src = tmp + ((size_t)v * S.K + k) * S.cap;
+  // position of the chunk's first grain: the view's start + the grains of the chunks before
+  if (wid == 0) {
+    int sum = 0;
+    for (int q = lane; q < k; q += 32) sum += cur[(size_t)v * S.K + q];
+    sum = __reduce_add_sync(EMU_FULL, sum);
+    if (lane == 0) base_s = __ldg(view_off + v) + sum;
+  }
+  for (int w = tid; w < (nc + 1) / 2; w += kChunkThreads) cntw[w] = 0u;
+  __syncthreads();
+  const int base = base_s;
+  // ---- count per cell (the chunk's grains stay in registers: one batch of independent loads) ----
+  int4 gg[kChunkPer];
+  int cc[kChunkPer];
+#pragma unroll
+  for (int u = 0; u < kChunkPer; ++u) {
+    const int i = tid + u * kChunkThreads;
+    gg[u] = i < n ? __ldg(src + i) : make_int4(0, 0, 0, 0);
+  }
+#pragma unroll
+  for (int u = 0; u < kChunkPer; ++u) {
+    cc[u] = -1;
+    if (tid + u * kChunkThreads < n) {
+      cc[u] = emu_cell_of_frame(P, frame, gg[u].x, gg[u].y, gg[u].z) - c_lo;
+      atomicAdd(&cntw[cc[u] >> 1], 1u << (16 * (cc[u] & 1)));
+    }
+  }
+  __syncthreads();
+  // ---- exclusive scan over the cells of the chunk: a run of consecutive cells per thread ----
+  const int per = (nc + kChunkThreads - 1) / kChunkThreads;
+  const int c0 = tid * per, c1 = min(nc, c0 + per);
+  int mine = 0;
+  for (int c = c0; c < c1; ++c) mine += cnt[c];
+  int incl = mine;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(EMU_FULL, incl, o); if (lane >= o) incl += y; }
+  if (lane == 31) warp_sum[wid] = incl;
+  __syncthreads();
+  if (wid == 0) {
+    int x = (lane < kChunkThreads / 32) ? warp_sum[lane] : 0, xi = x;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(EMU_FULL, xi, o); if (lane >= o) xi += y; }
+    if (lane < kChunkThreads / 32) warp_sum[lane] = xi - x;
+  }
+  __syncthreads();
+  int run = warp_sum[wid] + incl - mine;
+  for (int c = c0; c < c1; ++c) { pre[c] = (unsigned short)run; run += cnt[c]; }
+  __syncthreads();
+  for (int c = tid; c < nc; c += kChunkThreads) cell_start[(size_t)v * ncell + c_lo + c] = base + (int)pre[c];
+  for (int w = tid; w < (nc + 1) / 2; w += kChunkThreads) cntw[w] = 0u;
+  __syncthreads();
+  // ---- place; the counters count up again ----
+#pragma unroll
+  for (int u = 0; u < kChunkPer; ++u) {
+    if (cc[u] < 0) continue;
+    const int sh = 16 * (cc[u] & 1);
+    const int r = (int)((atomicAdd(&cntw[cc[u] >> 1], 1u << sh) >> sh) & 0xffffu);
+    buf[(int)pre[cc[u]] + r] = gg[u];
+  }
+  __syncthreads();
+  // ---- ascending row inside every cell ----
+  for (int c = tid; c < nc; c += kChunkThreads) {
+    const int m = cnt[c];
+    if (m < 2) continue;
+    int4* q = buf + pre[c];
+    for (int i = 1; i < m; ++i) {
+      const int4 key = q[i];
+      int j = i - 1;
+      while (j >= 0 && q[j].w > key.w) { q[j + 1] = q[j]; --j; }
+      q[j + 1] = key;
+    }
+  }
+  __syncthreads();
+  for (int i = tid; i < n; i += kChunkThreads) sorted[base + i] = buf[i];
+}
+
+// plan of the two-pass path for one frame; K = 0: not applicable (the one-kernel paths take over)
+SplitPlan split_plan(const EmuDev& P, int frame, int64_t n_grains, int32_t n_views) {
+  SplitPlan S; S.K = 0; S.cpc = 1; S.cap = 0; S.inv_cpc = 1.0f;
+  const int ncell = P.fr[frame].ncell;
+  if (n_views < 1 || n_grains < 1 || ncell >= (1 << 24)) return S;
+  const double avg = (double)n_grains / n_views;
+  // the fewest chunks whose scratch region (1.6 x the average chunk + 256) fits the shared-memory buffer
+  int K = (int)emu_max64(1, (int64_t)(avg * 1.6 / (double)(kChunkCap - 256 - 64)) + 1);
+  K = (int)emu_max64(K, ((int64_t)ncell + kMaxChunkCells - 1) / kMaxChunkCells);
+  if (K > kMaxChunks) return S;
+  const int cpc = (ncell + K - 1) / K;
+  const int cap = (((int)(avg / K * 1.6) + 256) + 63) & ~63;
+  if (cap > kChunkCap) return S;
+  S.K = (ncell + cpc - 1) / cpc; S.cpc = cpc; S.cap = cap; S.inv_cpc = 1.0f / (float)cpc;
+  return S;
+}
+
+size_t split_tmp_grains(const EmuDev& P, int64_t n_grains, int32_t n_views) {
+  size_t m = (size_t)n_grains;
+  for (int f = 0; f < 3; ++f) {
+    const SplitPlan S = split_plan(P, f, n_grains, n_views);
+    if (S.K) m = emu_max64((int64_t)m, (int64_t)n_views * S.K * S.cap);
+  }
+  return m;
+}
+
 }  // namespace
 
 size_t emu_bin_ws_bytes(const EmuDev& P, int64_t n_grains, int32_t n_views) {
   int ncell = P.fr[0].ncell;
   for (int f = 1; f < 3; ++f) if (P.fr[f].ncell > ncell) ncell = P.fr[f].ncell;     // one scratch serves every frame
   size_t cnt = emu_align256((size_t)n_views * ncell * sizeof(int));
-  size_t tmp = emu_align256((size_t)n_grains * sizeof(int4));
+  size_t tmp = emu_align256(split_tmp_grains(P, n_grains, n_views) * sizeof(int4));
   size_t redo = emu_align256(((size_t)n_views + 1) * sizeof(int));
-  return cnt + tmp + redo + 256;
+  size_t cur = emu_align256((size_t)n_views * kMaxChunks * sizeof(int));
+  return cnt + tmp + redo + cur + 256;
 }
 
 int emu_bin_launch(const EmuDev& P, int frame, const int32_t* d_grains, const int32_t* d_view_off, int64_t n_grains,
@@ -326,8 +530,28 @@ int emu_bin_launch(const EmuDev& P, int frame, const int32_t* d_grains, const in
   int ncell_max = P.fr[0].ncell;
   for (int f = 1; f < 3; ++f) if (P.fr[f].ncell > ncell_max) ncell_max = P.fr[f].ncell;
   int4* tmp = (int4*)(ws + emu_align256((size_t)n_views * ncell_max * sizeof(int)));
-  int* redo = (int*)((char*)tmp + emu_align256((size_t)n_grains * sizeof(int4)));
+  int* redo = (int*)((char*)tmp + emu_align256(split_tmp_grains(P, n_grains, n_views) * sizeof(int4)));
+  int* cur = (int*)((char*)redo + emu_align256(((size_t)n_views + 1) * sizeof(int)));
   const int n = (int)n_grains;
+  const SplitPlan S = split_plan(P, frame, n_grains, n_views);
+  if (S.K > 0 && n_views <= 65535) {
+    // two passes: split into chunks of cells, then one chunk per block in shared memory
+    const size_t smem = (size_t)S.cap * 16 + 2 * (size_t)((S.cpc + 1) & ~1) * sizeof(unsigned short);
+    if (cudaFuncSetAttribute(k_bin_chunk, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return EMU_ERR_CUDA;
+    if (cudaMemsetAsync(redo, 0, ((size_t)n_views + 1) * sizeof(int), st) != cudaSuccess) return EMU_ERR_CUDA;
+    if (cudaMemsetAsync(cur, 0, (size_t)n_views * S.K * sizeof(int), st) != cudaSuccess) return EMU_ERR_CUDA;
+    const int blocks = (int)emu_max64(1, emu_min64(n_views, 148 * 8));
+    const int tile = kSplitThreads * kSplitPer;
+    const int tiles = (int)emu_min64(65535, 2 * ((n_grains / n_views + tile - 1) / tile) + 2);   // per view; larger views are redone
+    EMU_LAUNCH(frame == 0 ? EMU_STAGE_BIN_COUNT : EMU_STAGE_PREP, st, k_bin_split<<<dim3(tiles, n_views), kSplitThreads, 0, st>>>(
+        P, frame, S, (const int4*)d_grains, d_view_off, n_views, tmp, cur, redo, (unsigned long long*)d_status));
+    EMU_LAUNCH(frame == 0 ? EMU_STAGE_BIN_SCATTER : EMU_STAGE_PREP, st, k_bin_chunk<<<dim3(S.K, n_views), kChunkThreads, smem, st>>>(
+        P, frame, S, d_view_off, n_views, n, tmp, cur, redo, (int4*)d_sorted, d_cell_start));
+    EMU_LAUNCH(frame == 0 ? EMU_STAGE_BIN_PLACE : EMU_STAGE_PREP, st, k_bin_view<false><<<blocks, kViewThreads, 0, st>>>(
+        P, frame, (const int4*)d_grains, d_view_off, n_views, n, (int4*)d_sorted, d_cell_start, count, tmp, redo,
+        (unsigned long long*)d_status));
+    return cudaGetLastError() == cudaSuccess ? EMU_OK : EMU_ERR_CUDA;
+  }
   if (ncell <= kMaxSmemCells) {
     // one block per view, byte counters in shared memory; the views it flags are redone with global counters
     const size_t smem = (size_t)((ncell + 3) / 4) * 4;
