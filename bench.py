@@ -321,7 +321,7 @@ def main():
     ncell = int(E.emu_grid_cells(prm)[0])
     bin_bytes = BIN_BYTES_PER_GRAIN * n + 4.0 * ncell * V
     bin_gbs = bin_bytes / (bin_ms * 1e-3) / 1e9 if bin_ms > 0 else 0.0
-    roofline_bin = {"kernel": "emu_bin_grains: k_bin_view (one block per view, byte counters in shared memory)", "bound": "hbm",
+    roofline_bin = {"kernel": "emu_bin_grains: k_bin_split + k_bin_chunk (two passes: chunks of cells through a scratch array, then one chunk per block in shared memory)", "bound": "hbm",
                     "achieved": bin_gbs, "peak": hbm, "unit": "GB/s", "frac": bin_gbs / hbm, "traffic": None, "ms": bin_ms,
                     "algorithmic_bytes_per_grain": bin_bytes / max(1, n),
                     "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peaks['_source']})"}

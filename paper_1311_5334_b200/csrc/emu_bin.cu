@@ -318,8 +318,17 @@ k_bin_view(EmuDev P, int frame, const int4* __restrict__ grains, const int* __re
 // A view with a chunk fuller than the scratch region is flagged and redone by k_bin_view<false>.
 constexpr int kSplitThreads = 256;
 constexpr int kSplitPer = 8;                         // grains per thread and tile
-constexpr int kChunkThreads = 256;
-constexpr int kChunkPer = 6;                         // grains per thread of a chunk block (held in registers)
+#ifndef EMU_CHUNK_THREADS
+#define EMU_CHUNK_THREADS 256
+#endif
+#ifndef EMU_CHUNK_PER
+#define EMU_CHUNK_PER 6
+#endif
+#ifndef EMU_CHUNK_MINB
+#define EMU_CHUNK_MINB 3
+#endif
+constexpr int kChunkThreads = EMU_CHUNK_THREADS;
+constexpr int kChunkPer = EMU_CHUNK_PER;                         // grains per thread of a chunk block (held in registers)
 constexpr int kChunkCap = kChunkThreads * kChunkPer; // grains of a chunk: 1 536 = 24 KB of shared memory
 constexpr int kMaxChunks = 128;
 constexpr int kMaxChunkCells = 12288;                // cells of a chunk: 2 x 16 bits each in shared memory
@@ -363,8 +372,12 @@ k_bin_split(EmuDev P, int frame, SplitPlan S, const int4* __restrict__ grains, c
       gg[u] = emu_to_frame(frame, gg[u]);
       if (frame == 0) gg[u].w = i;                     // payload replaced by the row; frames 1, 2 carry it already
       bad |= (abs(gg[u].x) >= (1 << 17)) | (abs(gg[u].y) >= (1 << 17)) | (abs(gg[u].z) >= (1 << 17));
-      kk[u] = chunk_of(emu_cell_of_frame(P, frame, gg[u].x, gg[u].y, gg[u].z), S);
+      const int cell = emu_cell_of_frame(P, frame, gg[u].x, gg[u].y, gg[u].z);
+      kk[u] = chunk_of(cell, S);
       rr[u] = atomicAdd(&hist_s[kk[u]], 1);
+      // the scratch record carries the cell inside its chunk (< 2^14) above the 18 bits of x, so that pass 2 does not
+      // derive it again (a coordinate out of range is reported through `status`; the outputs are then unspecified)
+      gg[u].x = (gg[u].x & 0x3ffff) | ((cell - kk[u] * S.cpc) << 18);
     }
   }
   __syncthreads();
@@ -405,8 +418,16 @@ k_bin_chunk(EmuDev P, int frame, SplitPlan S, const int* __restrict__ view_off, 
   unsigned short* cnt = reinterpret_cast<unsigned short*>(chunk_smem + (size_t)S.cap * 16);   // [cpc] counts
   unsigned short* pre = cnt + ((S.cpc + 1) & ~1);                                    // [cpc] exclusive prefix
   unsigned* cntw = reinterpret_cast<unsigned*>(cnt);
-  const int n = min(cur[(size_t)v * S.K + k], S.cap);
   const int4* src = tmp + ((size_t)v * S.K + k) * S.cap;
+  // the loads of the chunk's grains leave before its size is known (the scratch region is cap grains long; what lies
+  // beyond the size is ignored), so that the two global latencies overlap
+  int4 gg[kChunkPer];
+#pragma unroll
+  for (int u = 0; u < kChunkPer; ++u) {
+    const int i = tid + u * kChunkThreads;
+    gg[u] = i < S.cap ? __ldg(src + i) : make_int4(0, 0, 0, 0);
+  }
+  const int n = min(cur[(size_t)v * S.K + k], S.cap);
   // position of the chunk's first grain: the view's start + the grains of the chunks before
   if (wid == 0) {
     int sum = 0;
@@ -418,18 +439,13 @@ k_bin_chunk(EmuDev P, int frame, SplitPlan S, const int* __restrict__ view_off, 
   __syncthreads();
   const int base = base_s;
   // ---- count per cell (the chunk's grains stay in registers: one batch of independent loads) ----
-  int4 gg[kChunkPer];
   int cc[kChunkPer];
-#pragma unroll
-  for (int u = 0; u < kChunkPer; ++u) {
-    const int i = tid + u * kChunkThreads;
-    gg[u] = i < n ? __ldg(src + i) : make_int4(0, 0, 0, 0);
-  }
 #pragma unroll
   for (int u = 0; u < kChunkPer; ++u) {
     cc[u] = -1;
     if (tid + u * kChunkThreads < n) {
-      cc[u] = emu_cell_of_frame(P, frame, gg[u].x, gg[u].y, gg[u].z) - c_lo;
+      cc[u] = min((int)((unsigned)gg[u].x >> 18), nc - 1);     // the cell inside the chunk, packed by pass 1
+      gg[u].x = (gg[u].x << 14) >> 14;                         // x again (sign-extended 18 bits)
       atomicAdd(&cntw[cc[u] >> 1], 1u << (16 * (cc[u] & 1)));
     }
   }
@@ -466,18 +482,23 @@ k_bin_chunk(EmuDev P, int frame, SplitPlan S, const int* __restrict__ view_off, 
     buf[(int)pre[cc[u]] + r] = gg[u];
   }
   __syncthreads();
-  // ---- ascending row inside every cell ----
-  for (int c = tid; c < nc; c += kChunkThreads) {
-    const int m = cnt[c];
+  // ---- ascending row inside every cell: a grain whose cell holds several looks at the rows of its cell-mates in
+  //      the buffer and moves to the place its own row deserves (rows are distinct: the ranks are a permutation) ----
+  int np[kChunkPer];
+#pragma unroll
+  for (int u = 0; u < kChunkPer; ++u) {
+    np[u] = -1;
+    if (cc[u] < 0) continue;
+    const int m = cnt[cc[u]];
     if (m < 2) continue;
-    int4* q = buf + pre[c];
-    for (int i = 1; i < m; ++i) {
-      const int4 key = q[i];
-      int j = i - 1;
-      while (j >= 0 && q[j].w > key.w) { q[j + 1] = q[j]; --j; }
-      q[j + 1] = key;
-    }
+    const int p0 = pre[cc[u]];
+    int r = 0;
+    for (int t = 0; t < m; ++t) r += (buf[p0 + t].w < gg[u].w);
+    np[u] = p0 + r;
   }
+  __syncthreads();
+#pragma unroll
+  for (int u = 0; u < kChunkPer; ++u) if (np[u] >= 0) buf[np[u]] = gg[u];
   __syncthreads();
   for (int i = tid; i < n; i += kChunkThreads) sorted[base + i] = buf[i];
 }
