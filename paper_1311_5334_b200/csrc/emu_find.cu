@@ -664,7 +664,7 @@ k_brick(EmuDev P, FramePtrs F, int v0, const Brick* __restrict__ bricks, FindCtl
     const unsigned row_b = 2u * (unsigned)S, lay_b = row_b * (unsigned)H;   // table bytes per row / per w layer
     const unsigned tab0 = pool_a + 4u * (unsigned)B.n - 2u * (unsigned)B.cx0 - (unsigned)B.cy0 * row_b - lay_b;
     const unsigned delta_o = 2u * (unsigned)(B.cx0 + S - 2);               // from a row address to its position word
-    const float cz1f = (float)B.cz1, cy1f = (float)B.cy1;
+    const float cz1f = (float)B.cz1, cy1f = (float)B.cy1, cy0f = (float)B.cy0;
     const int ord_shift = record ? 16 * (B.ord & (kRecBricks - 1)) : 0;   // without records: one plain counter
     const size_t rec_ord = (size_t)(B.ord & (kRecBricks - 1)) * kRecSlots;
 
@@ -675,7 +675,8 @@ k_brick(EmuDev P, FramePtrs F, int v0, const Brick* __restrict__ bricks, FindCtl
     float oxm = 0.f, oym = 0.f, ozm = 0.f;           // magic-biased origin of v = P - A for the current row
     float T = 0.f, band = 0.f;                       // r2 D2 and the half-width of the float test's error band
     unsigned short* rec = nullptr;                   // hit record of the lane's seed in this brick
-    float t0 = 0.f, t1 = 0.f, tl0 = 0.f, tl1 = 0.f;  // u interval of the line inside the brick / inside the layer
+    float t0 = 0.f, t1 = 0.f;                        // u interval of the line inside the brick
+    float pk0 = 0.f, pk1 = 0.f;                      // two values parked between the stages of the refill
     float dty = 0.f, tyl = 0.f, tyh = 0.f, dtz = 0.f, tzl = 0.f, tzh = 0.f;
     float cyf = 1.f, cyhf = 0.f, czf = 0.f, czhf = -1.f;   // current / last row of the layer, current / last layer
     unsigned rowp = 0, layp = 0;                     // table address of the current row / of row 0 of the current layer
@@ -746,7 +747,7 @@ k_brick(EmuDev P, FramePtrs F, int v0, const Brick* __restrict__ bricks, FindCtl
             else hit = hit && (az >= blo[2]) && (az <= bhi[2]);
             if (hit && t0 <= t1) {
               sidx = idx;
-              ozm = az; tl0 = bz; tl1 = z0; dty = inv_a; dtz = inv_b;       // parked for stage 2
+              ozm = az; pk0 = bz; pk1 = z0; dty = inv_a; dtz = inv_b;       // parked for stage 2
               if (kMode == kAssoc) count = (int)((unsigned)q.y >> 16);        // n_tube of the candidate, parked
               fresh = true;
               idle = false;
@@ -756,7 +757,7 @@ k_brick(EmuDev P, FramePtrs F, int v0, const Brick* __restrict__ bricks, FindCtl
           if (__popc(mS) < kRefillStop) break;
         }
         if (fresh) {
-          const float az = ozm, bz = tl0, z0 = tl1, inv_a = dty, inv_b = dtz;
+          const float az = ozm, bz = pk0, z0 = pk1, inv_a = dty, inv_b = dtz;
           const float D2 = __fmaf_rn(dx, dx, __fmaf_rn(dy, dy, dz * dz));        // exact: < 2^22
           {
             T = r2f * D2;
@@ -790,31 +791,27 @@ k_brick(EmuDev P, FramePtrs F, int v0, const Brick* __restrict__ bricks, FindCtl
         break;                                              // the slice is exhausted and every lane is done
       }
 
-      // ---------------- LAYER: lanes that have used up the rows of their w layer move to the next one ----------------
+      // ---------------- ADVANCE: lanes whose run is used up move to the next row of cells; a lane whose layer has no
+      //                  row left takes the next w layer in the same breath.  ONE instruction sequence serves both
+      //                  cases: the layer's u interval and row range are functions of the layer index and are simply
+      //                  derived again on every step (it costs less than a second, thinly populated code path) ----
       if (!idle && j >= e) {
-       if (cyf >= cyhf) {
-        czf += 1.0f; ozm -= P.csf[2]; layp += lay_b;
+        const bool nl = cyf >= cyhf;                        // the rows of the layer are used up
+        if (nl) { czf += 1.0f; ozm -= P.csf[2]; layp += lay_b; }
         if (czf > czhf) {                                   // the seed is finished
           if (kMode == kVote && count) atomicAdd(seed_cnt + sidx, (unsigned long long)min(count, 0xffff) << ord_shift);
           idle = true;
         } else {
-          tl0 = fmaxf(t0, __fmaf_rn(czf, dtz, tzl)); tl1 = fminf(t1, __fmaf_rn(czf, dtz, tzh));
-          cyf = 1.f; cyhf = 0.f;                            // an empty layer: stepped over in the next round
-          if (tl0 <= tl1) {
-            const float ya = __fmaf_rn(a, tl0, y0), yb = __fmaf_rn(a, tl1, y0);
-            const int cyi = max(B.cy0, rn_int(__fmaf_rn(fminf(ya, yb), P.inv_cs[1], P.klo[1]))) - 1;   // the row before the first
-            cyhf = fminf(cy1f, rn_flt(__fmaf_rn(fmaxf(ya, yb), P.inv_cs[1], P.khi[1])));
-            cyf = int_f(cyi);
-            rowp = layp + (unsigned)cyi * row_b;
-            oym = __fmaf_rn(-cyf, P.csf[1], ay + kMagicF);
-          }
-        }
-       }
-        // ---------------- ROW: ... and to the next row of cells of their layer ----------------
-        if (!idle && cyf < cyhf) {
-          cyf += 1.0f; rowp += row_b; oym -= P.csf[1];
+          const float tl0 = fmaxf(t0, __fmaf_rn(czf, dtz, tzl)), tl1 = fminf(t1, __fmaf_rn(czf, dtz, tzh));
+          const float ya = __fmaf_rn(a, tl0, y0), yb = __fmaf_rn(a, tl1, y0);
+          const float cyl = fmaxf(cy0f, rn_flt(__fmaf_rn(fminf(ya, yb), P.inv_cs[1], P.klo[1])));
+          const float cyh = fminf(cy1f, rn_flt(__fmaf_rn(fmaxf(ya, yb), P.inv_cs[1], P.khi[1])));
+          cyf = nl ? cyl : cyf + 1.0f;
+          cyhf = tl0 <= tl1 ? cyh : cyf;                    // an empty layer has no further row
+          rowp = layp + (unsigned)rn_int(cyf) * row_b;
+          oym = __fmaf_rn(-cyf, P.csf[1], ay + kMagicF);
           const float ta = fmaxf(tl0, __fmaf_rn(cyf, dty, tyl)), tb = fminf(tl1, __fmaf_rn(cyf, dty, tyh));
-          if (ta <= tb) {
+          if (ta <= tb && cyf <= cyh) {
             const int c0 = max(B.cx0, rn_int(__fmaf_rn(ta, P.inv_cs[0], P.klo[0])));
             const int c1 = min(B.cx1, rn_int(__fmaf_rn(tb, P.inv_cs[0], P.khi[0])));
             if (c0 <= c1) {
