@@ -419,15 +419,13 @@ k_bin_chunk(EmuDev P, int frame, SplitPlan S, const int* __restrict__ view_off, 
   unsigned short* pre = cnt + ((S.cpc + 1) & ~1);                                    // [cpc] exclusive prefix
   unsigned* cntw = reinterpret_cast<unsigned*>(cnt);
   const int4* src = tmp + ((size_t)v * S.K + k) * S.cap;
-  // the loads of the chunk's grains leave before its size is known (the scratch region is cap grains long; what lies
-  // beyond the size is ignored), so that the two global latencies overlap
-  int4 gg[kChunkPer];
+  const int n = min(cur[(size_t)v * S.K + k], S.cap);
+  int4 gg[kChunkPer];                                  // the chunk's grains stay in registers: one batch of independent loads
 #pragma unroll
   for (int u = 0; u < kChunkPer; ++u) {
     const int i = tid + u * kChunkThreads;
-    gg[u] = i < S.cap ? __ldg(src + i) : make_int4(0, 0, 0, 0);
+    gg[u] = i < n ? __ldg(src + i) : make_int4(0, 0, 0, 0);
   }
-  const int n = min(cur[(size_t)v * S.K + k], S.cap);
   // position of the chunk's first grain: the view's start + the grains of the chunks before
   if (wid == 0) {
     int sum = 0;
