@@ -47,10 +47,10 @@ constexpr int kMaxTube = 8191;                    // n_tube field of the packed 
 #define EMU_CHUNK_GIB 96
 #endif
 #ifndef EMU_REFILL
-#define EMU_REFILL 8
+#define EMU_REFILL 10
 #endif
 #ifndef EMU_REFILL_STOP
-#define EMU_REFILL_STOP 4
+#define EMU_REFILL_STOP 6
 #endif
 constexpr int kBrickThreads = EMU_BRICK_THREADS;  // one persistent block per SM
 constexpr int kPoolBytes = 222 * 1024;            // dynamic shared memory of a brick: grains | row table | cell table
@@ -815,9 +815,10 @@ k_brick(EmuDev P, FramePtrs F, int v0, const Brick* __restrict__ bricks, FindCtl
             const int c0 = max(B.cx0, rn_int(__fmaf_rn(ta, P.inv_cs[0], P.klo[0])));
             const int c1 = min(B.cx1, rn_int(__fmaf_rn(tb, P.inv_cs[0], P.khi[0])));
             if (c0 <= c1) {
-              j = pool_a + 4u * lds_u16(rowp + 2u * (unsigned)c0);
-              e = pool_a + 4u * lds_u16(rowp + 2u * (unsigned)c1 + 2u);
-              item_tests += e - j;
+              const unsigned sj = lds_u16(rowp + 2u * (unsigned)c0), se = lds_u16(rowp + 2u * (unsigned)c1 + 2u);
+              j = pool_a + 4u * sj;
+              e = pool_a + 4u * se;
+              item_tests += se - sj;
             }
           }
         }
@@ -859,7 +860,7 @@ k_brick(EmuDev P, FramePtrs F, int v0, const Brick* __restrict__ bricks, FindCtl
         }
       }
     }
-    n_tests += item_tests >> 2;
+    n_tests += item_tests;
   }
 
   for (int o = 16; o; o >>= 1) n_tests += __shfl_xor_sync(EMU_FULL, n_tests, o);
