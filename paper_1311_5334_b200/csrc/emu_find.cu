@@ -283,8 +283,15 @@ k_seed_pairs(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ 
       int s = __ldg(cell_start + rb + cxa);
       const int e = __ldg(cell_start + rb + cxb + 1);
       s = max(s, a + 1);
-      for (int j = s; j < e; ++j) {
-        const int4 B = __ldg(sorted + j);
+      for (int j0 = s; j0 < e; j0 += 4) {
+       int4 Bq[4];
+#pragma unroll
+       for (int q = 0; q < 4; ++q) Bq[q] = (j0 + q < e) ? __ldg(sorted + j0 + q) : make_int4(0, 0, 0, 0);   // four loads in flight
+#pragma unroll
+       for (int q = 0; q < 4; ++q) {
+        const int j = j0 + q;
+        if (j >= e) break;
+        const int4 B = Bq[q];
         const int dx = B.x - A.x, dy = B.y - A.y, dz = B.z - A.z;
         // |d| can exceed 2^15 for far out-of-box grains: compare in 64 bits
         const long long d2 = (long long)dx * dx + (long long)dy * dy + (long long)dz * dz;
@@ -302,6 +309,7 @@ k_seed_pairs(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ 
             ab[idx] = make_int2(a, j);
           }
         }
+       }
       }
     }
     if (!kFill) {
