@@ -840,28 +840,33 @@ k_brick(EmuDev P, FramePtrs F, int v0, const Brick* __restrict__ bricks, FindCtl
             const unsigned g0 = lds_u32(j), g1 = lds_u32_off4(j);   // g1 may lie beyond the run (still inside the pool)
             float v0x, v0y, v0z, v1x, v1y, v1z;
             const float s0 = tube_s(g0, v0x, v0y, v0z), s1 = tube_s(g1, v1x, v1y, v1z);
-            bool in0 = s0 <= T, in1 = s1 <= T;
-            if (fminf(fabsf(s0 - T), fabsf(s1 - T)) <= band) {     // inside the error band: the exact predicate
-              if (fabsf(s0 - T) <= band) in0 = exact_in(v0x, v0y, v0z);
-              if (fabsf(s1 - T) <= band) in1 = exact_in(v1x, v1y, v1z);
-            }
-            in1 = in1 && (j + 4u < e);
-            if (kMode == kVote) {
-              if (record) {
-                // write down the brick slots of the grains found (the first kRecSlots of this seed in this brick)
-                const unsigned slot = (j - pool_a) >> 2;
-                if (in0) rec[min(count, kRecSlots - 1)] = (unsigned short)slot;
-                count += (int)in0;
-                if (in1) rec[min(count, kRecSlots - 1)] = (unsigned short)(slot + 1u);
-                count += (int)in1;
-              } else {
-                count += (int)in0 + (int)in1;
+            // what a pair of decisions does: VOTE counts and writes the brick slots of the grains found into the hit
+            // record (the first kRecSlots of this seed in this brick), ASSOC joins the priority maximum of the grains
+            auto commit = [&](bool in0, bool in1) {
+              if (kMode == kVote) {
+                if (record) {
+                  const unsigned slot = (j - pool_a) >> 2;
+                  if (in0) rec[min(count, kRecSlots - 1)] = (unsigned short)slot;
+                  count += (int)in0;
+                  if (in1) rec[min(count, kRecSlots - 1)] = (unsigned short)(slot + 1u);
+                  count += (int)in1;
+                } else {
+                  count += (int)in0 + (int)in1;
+                }
+              } else if (in0 || in1) {
+                // slot of the grain in the brick + (sorted position - slot) of the first grain of its row -> row of the grain
+                const int pos = (int)((j - pool_a) >> 2) + (int)lds_u32(rowp + delta_o);
+                if (in0) { const int row = __ldg(&sorted[pos].w); atomicMax(keyA + row, ka); atomicMax(keyB + row, kb); }
+                if (in1) { const int row = __ldg(&sorted[pos + 1].w); atomicMax(keyA + row, ka); atomicMax(keyB + row, kb); }
               }
-            } else if (in0 || in1) {
-              // slot of the grain in the brick + (sorted position - slot) of the first grain of its row -> row of the grain
-              const int pos = (int)((j - pool_a) >> 2) + (int)lds_u32(rowp + delta_o);
-              if (in0) { const int row = __ldg(&sorted[pos].w); atomicMax(keyA + row, ka); atomicMax(keyB + row, kb); }
-              if (in1) { const int row = __ldg(&sorted[pos + 1].w); atomicMax(keyA + row, ka); atomicMax(keyB + row, kb); }
+            };
+            const bool two = j + 4u < e;
+            if (fminf(fabsf(s0 - T), fabsf(s1 - T)) > band) {      // the common case: the float test decides both
+              commit(s0 <= T, (s1 <= T) && two);
+            } else {                                               // inside the error band: the exact predicate
+              const bool in0 = fabsf(s0 - T) <= band ? exact_in(v0x, v0y, v0z) : (s0 <= T);
+              const bool in1 = fabsf(s1 - T) <= band ? exact_in(v1x, v1y, v1z) : (s1 <= T);
+              commit(in0, in1 && two);
             }
             j += 8u;
           }
