@@ -46,6 +46,9 @@ constexpr int kMaxTube = 8191;                    // n_tube field of the packed 
 #ifndef EMU_CHUNK_GIB
 #define EMU_CHUNK_GIB 96
 #endif
+#ifndef EMU_ITEMS_PER_SM
+#define EMU_ITEMS_PER_SM 12
+#endif
 #ifndef EMU_REFILL
 #define EMU_REFILL 10
 #endif
@@ -1603,12 +1606,12 @@ static int sm_count() {
 
 #define EMU_CK(x) do { if ((x) != cudaSuccess) return EMU_ERR_CUDA; } while (0)
 
-static int choose_slices(const Tilings& TT, int nv, int n_sm) {
+static int choose_slices(const Tilings& TT, int nv, int n_sm, int per_sm) {
   // enough work items that every SM gets several even when the chunk holds few views
   int64_t bricks = 0;
   for (int f = 0; f < 3; ++f) bricks += (int64_t)nv * TT.t[f].tx * TT.t[f].ty;
   bricks = emu_max64(1, bricks);
-  int64_t s = (4 * (int64_t)n_sm + bricks - 1) / bricks;
+  int64_t s = (per_sm * (int64_t)n_sm + bricks - 1) / bricks;
   if (s < 1) s = 1;
   if (s > 256) s = 256;
   return (int)s;
@@ -1687,7 +1690,8 @@ int emu_find_launch(const EmuDev& P, int seeds_per_grain, int cand_per_grain, co
   for (int v0 = 0; v0 < n_views; v0 += W.views_per_chunk) {
     const int v1 = (int)emu_min64(n_views, (int64_t)v0 + W.views_per_chunk);
     const int nv = v1 - v0;
-    const int slices = choose_slices(TT, nv, kSM);
+    const int slices = choose_slices(TT, nv, kSM, EMU_ITEMS_PER_SM);      // the voting pass: fine items, short tail
+    const int slices_walk = choose_slices(TT, nv, kSM, 4);                // the walk list is short: staging would dominate
     EMU_CK(cudaMemsetAsync(W.view_ntracks, 0, (size_t)nv * sizeof(int), st));
     EMU_CK(cudaMemsetAsync(W.tie_bits, 0, kTieBits / 8, st));
     rc = vote_chunk(P, TT, W, F, d_view_off, n_grains, v0, v1, slices, kSM, counts, st);
@@ -1719,7 +1723,7 @@ int emu_find_launch(const EmuDev& P, int seeds_per_grain, int cand_per_grain, co
     EMU_LAUNCH(EMU_STAGE_ASSOC, st, k_assoc_hits<<<dim3(48, 3 * nv), 256, 0, st>>>(
         v0, W.ctl, W.view_cand_off, W.cands, W.cand_seed, W.seed_cnt, W.recs, W.slot_row, W.vf_brick_base, W.keyA, W.keyB));
     EMU_LAUNCH(EMU_STAGE_ASSOC, st, k_brick<kAssoc><<<kSM, kBrickThreads, kPoolBytes, st>>>(
-        P, F, v0, W.bricks, W.ctl, slices, W.ovf_geo, W.ovf_ci, W.view_ovf_off, nullptr, nullptr, nullptr, W.keyA, W.keyB,
+        P, F, v0, W.bricks, W.ctl, slices_walk, W.ovf_geo, W.ovf_ci, W.view_ovf_off, nullptr, nullptr, nullptr, W.keyA, W.keyB,
         counts));
     EMU_LAUNCH(EMU_STAGE_ASSOC, st, k_assoc_generic<0><<<kSM * 16, kVoteThreads, 0, st>>>(
         P, sorted, d_cell_start, W.bbox, v0, W.cands, W.ctl, W.tie_bits, W.keyA, W.keyB, W.owner));
@@ -1760,7 +1764,7 @@ int emu_count_seeds_launch(const EmuDev& P, int seeds_per_grain, int cand_per_gr
   rc = prepare_frames(P, W, F, d_sorted, d_cell_start, d_view_off, n_grains, n_views, kSM, st);
   if (rc != EMU_OK) return rc;
   if (n_views > 0) {
-    rc = vote_chunk(P, TT, W, F, d_view_off, n_grains, 0, n_views, choose_slices(TT, n_views, kSM), kSM, counts, st);
+    rc = vote_chunk(P, TT, W, F, d_view_off, n_grains, 0, n_views, choose_slices(TT, n_views, kSM, EMU_ITEMS_PER_SM), kSM, counts, st);
     if (rc != EMU_OK) return rc;
     EMU_LAUNCH(EMU_STAGE_CANDS, st, k_seed_dump<<<dim3(64, 3 * n_views), 256, 0, st>>>(
         0, W.ctl, sorted, W.view_seed_off, W.seed_cnt, W.ab, (int4*)d_seed_dump, dump_capacity));
