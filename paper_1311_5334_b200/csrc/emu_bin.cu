@@ -321,8 +321,11 @@ constexpr int kSplitPer = 8;                         // grains per thread and ti
 #ifndef EMU_CHUNK_THREADS
 #define EMU_CHUNK_THREADS 256
 #endif
+#ifndef EMU_CHUNK_SLACK
+#define EMU_CHUNK_SLACK 1.3
+#endif
 #ifndef EMU_CHUNK_PER
-#define EMU_CHUNK_PER 6
+#define EMU_CHUNK_PER 10
 #endif
 #ifndef EMU_CHUNK_MINB
 #define EMU_CHUNK_MINB 3
@@ -508,11 +511,11 @@ SplitPlan split_plan(const EmuDev& P, int frame, int64_t n_grains, int32_t n_vie
   if (n_views < 1 || n_grains < 1 || ncell >= (1 << 24)) return S;
   const double avg = (double)n_grains / n_views;
   // the fewest chunks whose scratch region (1.6 x the average chunk + 256) fits the shared-memory buffer
-  int K = (int)emu_max64(1, (int64_t)(avg * 1.6 / (double)(kChunkCap - 256 - 64)) + 1);
+  int K = (int)emu_max64(1, (int64_t)(avg * EMU_CHUNK_SLACK / (double)(kChunkCap - 256 - 64)) + 1);
   K = (int)emu_max64(K, ((int64_t)ncell + kMaxChunkCells - 1) / kMaxChunkCells);
   if (K > kMaxChunks) return S;
   const int cpc = (ncell + K - 1) / K;
-  const int cap = (((int)(avg / K * 1.6) + 256) + 63) & ~63;
+  const int cap = (((int)(avg / K * EMU_CHUNK_SLACK) + 256) + 63) & ~63;
   if (cap > kChunkCap) return S;
   S.K = (ncell + cpc - 1) / cpc; S.cpc = cpc; S.cap = cap; S.inv_cpc = 1.0f / (float)cpc;
   return S;
