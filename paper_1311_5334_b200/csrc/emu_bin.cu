@@ -317,7 +317,10 @@ k_bin_view(EmuDev P, int frame, const int4* __restrict__ grains, const int* __re
 //           stream, with its part of cell_start.
 // A view with a chunk fuller than the scratch region is flagged and redone by k_bin_view<false>.
 constexpr int kSplitThreads = 256;
-constexpr int kSplitPer = 8;                         // grains per thread and tile
+#ifndef EMU_SPLIT_PER
+#define EMU_SPLIT_PER 8
+#endif
+constexpr int kSplitPer = EMU_SPLIT_PER;                         // grains per thread and tile
 #ifndef EMU_CHUNK_THREADS
 #define EMU_CHUNK_THREADS 256
 #endif
