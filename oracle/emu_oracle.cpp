@@ -116,12 +116,22 @@ void bin_view(const Grid& g, const int32_t* grains, int32_t row0, int32_t n,
 }
 
 // O3 predicate - SURVEY 8(c) O3: P in tube <=> |(P-A) x (B-A)|^2 <= r2 * |B-A|^2.
-inline bool in_tube(const Grain& A, i64 dx, i64 dy, i64 dz, i64 r2D2, const Grain& P) {
+// Bounded tube (Fig. 4(b) "along the seed"): with ext = tube_ext_q >= 0 the grain
+// must also lie, along the line, between the two seed grains or at most ext beyond either of them:
+//   -ext |d| <= (P-A).d <= D2 + ext |d|,  compared exactly through squares (s < 0: s^2 <= ext^2 D2, and the same for
+// s - D2 > 0).  Swapping A and B turns s into D2 - s, so the predicate stays orientation-free.  ext = -1: whole line.
+// |s| < 3 * 2^18 * 2^11 < 2^31 and ext <= 2^16, D2 < 2^22: every product below 2^62.
+inline bool in_tube(const Grain& A, i64 dx, i64 dy, i64 dz, i64 r2D2, const Grain& P, i64 d2, i64 ext) {
   i64 vx = (i64)P.x - A.x, vy = (i64)P.y - A.y, vz = (i64)P.z - A.z;
   i64 cx = vy * dz - vz * dy;
   i64 cy = vz * dx - vx * dz;
   i64 cz = vx * dy - vy * dx;
-  return cx * cx + cy * cy + cz * cz <= r2D2;
+  if (cx * cx + cy * cy + cz * cz > r2D2) return false;
+  if (ext < 0) return true;
+  const i64 s = vx * dx + vy * dy + vz * dz, e2d2 = ext * ext * d2;
+  if (s < 0 && s * s > e2d2) return false;
+  if (s > d2 && (s - d2) * (s - d2) > e2d2) return false;
+  return true;
 }
 
 // k(g) = (z, x+y, min(x,y), x, original index), compared lexicographically - SURVEY 8(c) O5.
@@ -248,7 +258,7 @@ void track_view(const emo_params& P, const int32_t* grains, int32_t row0, int32_
     if (mode == 0) {
       for (int32_t p = 0; p < n; ++p) {
         R.cnt[1] += 1;
-        if (in_tube(A, d[0], d[1], d[2], r2D2, G[p])) cur.push_back(p);
+        if (in_tube(A, d[0], d[1], d[2], r2D2, G[p], d2, P.tube_ext_q)) cur.push_back(p);
       }
       return;
     }
@@ -290,7 +300,7 @@ void track_view(const emo_params& P, const int32_t* grains, int32_t row0, int32_
           i64 c0 = rng[0][0] + grid.n[0] * (cy + grid.n[1] * cz), c1 = c0 + (rng[0][1] - rng[0][0]);
           for (int32_t j = cell_start[c0]; j < cell_start[c1 + 1]; ++j) {
             R.cnt[1] += 1;
-            if (in_tube(A, d[0], d[1], d[2], r2D2, G[j])) cur.push_back(j);
+            if (in_tube(A, d[0], d[1], d[2], r2D2, G[j], d2, P.tube_ext_q)) cur.push_back(j);
           }
         }
     }
@@ -389,7 +399,7 @@ bool params_ok(const emo_params* p) {
     if (p->view_size_q[i] <= 0 || p->view_size_q[i] > 65536 || p->cell_size_q[i] <= 0) return false;
   if (p->sep_min_q < 1 || p->sep_max_q <= p->sep_min_q || p->sep_max_q > 2048) return false;
   if (p->tube_r2_q < 0 || p->tube_r2_q >= (1 << 20)) return false;
-  if (p->tube_ext_q != -1) return false;                    // bounded tube = SURVEY 8(f) NEXT-1
+  if (p->tube_ext_q < -1 || p->tube_ext_q > 65536) return false;   // -1 = whole line; >= 0 = bounded tube (NEXT-1)
   if (p->min_grains < 2) return false;
   return true;
 }

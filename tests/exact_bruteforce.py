@@ -23,6 +23,7 @@ def track_view_exact(grains, params):
     smax2 = params["sep_max_q"] ** 2
     r2 = params["tube_r2_q"]
     nmin = params["min_grains"]
+    ext = params.get("tube_ext_q", -1)
     seeds = {}      # (a,b) -> (n_tube, D2, tube set)
     for a in range(n):
         ax, ay, az = grains[a]
@@ -37,8 +38,16 @@ def track_view_exact(grains, params):
                 vv = v[0] * v[0] + v[1] * v[1] + v[2] * v[2]
                 vd = v[0] * d[0] + v[1] * d[1] + v[2] * d[2]
                 dist2 = Fraction(vv) - Fraction(vd * vd, D2)      # squared distance to the infinite line
-                if dist2 <= r2:
-                    tube.append(p)
+                if dist2 > r2:
+                    continue
+                if ext >= 0:
+                    # bounded tube: the foot of P, lam = (v.d)/D2 in units of the seed length,
+                    # must lie in [-ext/|d|, 1 + ext/|d|]; beyond an end the overshoot is compared through its square
+                    lam = Fraction(vd, D2)
+                    over = -lam if lam < 0 else (lam - 1 if lam > 1 else Fraction(0))
+                    if over * over * D2 > ext * ext:
+                        continue
+                tube.append(p)
             seeds[(a, b)] = (len(tube), D2, tube)
     cands = {ab: s for ab, s in seeds.items() if s[0] >= nmin}
 

@@ -406,3 +406,67 @@ def test_seed_density_closed_form(oracle_mod, config_oracle):
     expect_pairs = 0.5 * n * (n / vol) * (slab_ball(20.0) - slab_ball(4.0))
     # tracks add correlated pairs and the x,y edges remove some: the fog-only closed form must hold within 15 %
     assert 0.85 * expect_pairs < r.counters["seeds"] < 1.25 * expect_pairs
+
+
+# --------------------------------------------------------------------------- bounded tube
+
+@pytest.mark.parametrize("ext", [0, 200, 1280])
+@pytest.mark.parametrize("mode", ["brute", "cells"])
+def test_bounded_tube_all_triples_exact_rational(oracle_mod, mode, ext):
+    """tube_ext_q >= 0: every seed's count and the whole track list against the exact-rational brute force, whose
+    axial condition is written through the foot parameter lam = (v.d)/D2 instead of the oracle's squared products."""
+    pts = _tiny_view((1, 2))
+    p = _params((2200, 2000, 1800), cell_q=(300, 512, 700), min_grains=4, tube_ext_q=ext)
+    ref = track_view_exact([tuple(int(c) for c in q) for q in pts], p)
+    g, off = _arr(pts)
+    r = oracle_mod.track_views(p, g, off, mode, 1, seed_dump=True)
+    got = {(int(a), int(b)): int(n) for _, a, b, n in r.seed_dump}
+    assert got == ref["seeds"]
+    assert r.counters["candidates"] == ref["n_candidates"]
+    tl = _track_list(r)
+    assert [(t[1], t[2], t[3], t[5], t[6]) for t in tl] == \
+           [(t["seed_a"], t["seed_b"], t["n_tube"], t["seed_d2"], tuple(t["members"])) for t in ref["tracks"]]
+    whole = oracle_mod.track_views(dict(p, tube_ext_q=-1), g, off, mode, 1, seed_dump=True)
+    w = {(int(a), int(b)): int(n) for _, a, b, n in whole.seed_dump}
+    assert all(got[k] <= w[k] for k in w) and any(got[k] < w[k] for k in w)      # bounding can only remove grains
+
+
+def test_bounded_tube_axial_witness(oracle_mod):
+    """x-directed seed A = (1000,500,500), B = (1640,500,500) (|d| = 640), ext = 100: a grain on the line is counted
+    iff its x lies in [900, 1740] (closed at both ends); ext = 0 keeps [1000, 1640]; the seed grains always count."""
+    base = [(1000, 500, 500), (1640, 500, 500)]
+    for ext, x, expect in ((100, 900, 3), (100, 899, 2), (100, 1740, 3), (100, 1741, 2), (0, 999, 2), (0, 1641, 2),
+                           (0, 1300, 3), (-1, 100, 3), (-1, 3900, 3)):
+        g, off = _arr(base + [(x, 500, 500)])
+        p = _params((4000, 2000, 2000), min_grains=2, sep_min_q=640, sep_max_q=641, tube_ext_q=ext)
+        r = oracle_mod.track_views(p, g, off, "brute", 1, seed_dump=True)
+        d = {(int(a), int(b)): int(n) for _, a, b, n in r.seed_dump}
+        assert d == {(0, 1): expect}, (ext, x)
+    # a skew seed, d = (300, 400, 0), |d| = 500, ext = 50: the grain at A - 0.1 d = (-30, -40) off A is at axial
+    # distance 50 (in), at A - 0.102 d it is out; exact at the boundary: s = -25 000, s^2 = 6.25e8 = 50^2 * 250 000
+    A, B = (1000, 1000, 500), (1300, 1400, 500)
+    for P3, expect in (((970, 960, 500), 3), ((969, 959, 500), 2)):
+        g, off = _arr([A, B, P3])
+        p = _params((4000, 4000, 2000), min_grains=2, sep_min_q=450, sep_max_q=550, tube_ext_q=50)
+        r = oracle_mod.track_views(p, g, off, "brute", 1, seed_dump=True)
+        assert {(int(a), int(b)): int(n) for _, a, b, n in r.seed_dump} == {(0, 1): expect}
+
+
+def test_bounded_tube_is_orientation_and_order_free(oracle_mod, config_oracle):
+    """x<->y swap and grain-order permutation leave the bounded-tube track list unchanged (after mapping)."""
+    b, p, _ = config_oracle(0)
+    p = dict(p, tube_ext_q=640)
+    r0 = oracle_mod.track_views(p, b.grains, b.view_off, "cells", 1)
+    perm = np.random.default_rng(5).permutation(len(b.grains))
+    gp = b.grains[perm]
+    r1 = oracle_mod.track_views(p, gp, b.view_off, "cells", 1)
+    inv = perm                                   # new row i holds old row perm[i]
+    t0 = sorted((min(t["seed_a"], t["seed_b"]), max(t["seed_a"], t["seed_b"]), t["n_tube"], t["n_members"]) for t in r0.tracks)
+    t1 = sorted((min(inv[t["seed_a"]], inv[t["seed_b"]]), max(inv[t["seed_a"]], inv[t["seed_b"]]), t["n_tube"], t["n_members"])
+                for t in r1.tracks)
+    assert t0 == t1 and len(t0) > 0
+    gs = b.grains.copy(); gs[:, [0, 1]] = gs[:, [1, 0]]
+    ps = dict(p, view_size_q=(p["view_size_q"][1], p["view_size_q"][0], p["view_size_q"][2]),
+              cell_size_q=(p["cell_size_q"][1], p["cell_size_q"][0], p["cell_size_q"][2]))
+    r2 = oracle_mod.track_views(ps, gs, b.view_off, "cells", 1)
+    assert r2.tracks.tobytes() == r0.tracks.tobytes() and r2.members.tobytes() == r0.members.tobytes()
