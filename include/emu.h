@@ -45,7 +45,10 @@ typedef struct emu_params {
   int32_t sep_min_q;           /* seed <=> sep_min_q^2 <= D2 < sep_max_q^2 (reading Q1; "smaller      */
   int32_t sep_max_q;           /*  than 25 um" = 1600).  1 <= sep_min_q < sep_max_q <= 2048                */
   int32_t tube_r2_q;           /* tube radius squared, q^2; 0.8 um -> floor(0.64*4096) = 2621 (reading Q3) */
-  int32_t tube_ext_q;          /* -1 = count along the whole line (reading Q4).  >= 0: EMU_ERR_INVALID     */
+  int32_t tube_ext_q;          /* -1 = count along the whole line (reading Q4, the contract).  >= 0 (<=     */
+                               /* 65536): bounded tube (Fig. 4(b) "along the seed"): a grain counts   */
+                               /* only if its foot on the line lies between the seed grains or at most     */
+                               /* tube_ext_q beyond either; exact; runs on the global-memory kernels       */
   int32_t min_grains;          /* threshold, >= 2: n >= min_grains (reading Q6; "e.g. 5")             */
   int32_t max_tracks_per_view; /* capacity of the track list per view, 1..65536                            */
   int32_t reserved[4];         /* sizing hints for the internal chunks of emu_find_tracks:                 */

@@ -16,7 +16,7 @@ bool params_ok(const emu_params* p) {
     if (p->view_size_q[i] < 1 || p->view_size_q[i] > 65536 || p->cell_size_q[i] < 1) return false;
   if (p->sep_min_q < 1 || p->sep_max_q <= p->sep_min_q || p->sep_max_q > 2048) return false;
   if (p->tube_r2_q < 0 || p->tube_r2_q >= (1 << 20)) return false;
-  if (p->tube_ext_q != -1) return false;            // bounded tube: DESIGN.md "next" row, not built
+  if (p->tube_ext_q < -1 || p->tube_ext_q > 65536) return false;   // -1 = whole line; >= 0 = bounded tube
   if (p->min_grains < 2 || p->min_grains > 8191) return false;
   if (p->max_tracks_per_view < 1 || p->max_tracks_per_view > 65536) return false;
   if (p->reserved[0] < 0 || p->reserved[1] < 0 || p->reserved[2] || p->reserved[3]) return false;
@@ -57,6 +57,7 @@ EmuDev make_dev(const emu_params* p) {
     d.fr[f].ncell = fc > 0x7fffffff ? -1 : (int)fc;
     if ((int64_t)d.fr[f].n[0] * d.cs[0] > 65536) d.packed_ok = 0;
   }
+  d.ext = p->tube_ext_q;
   d.min_grains = p->min_grains;
   d.max_tracks = p->max_tracks_per_view;
   return d;

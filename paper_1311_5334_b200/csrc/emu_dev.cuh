@@ -28,6 +28,7 @@ struct EmuDev {           // passed by value to every kernel
   float Rw;               // walk radius: ceil(sqrt(r2)) + 2 q of slack for the float bounds
   int min_grains;
   int max_tracks;
+  int ext;                // tube_ext_q: -1 = whole line, >= 0 = bounded tube
   // brick kernels (emu_find.cu): cell index of a dilated bound without a float->int conversion,
   //   lo = rn(x * inv_cs + klo), hi = rn(x * inv_cs + khi), klo = -(Rw * inv_cs + 0.5), khi = Rw * inv_cs - 0.5
   float klo[3], khi[3];
@@ -96,6 +97,18 @@ __device__ __forceinline__ bool emu_in_tube(int px, int py, int pz, int ax, int 
   return s <= r2D2;
 }
 
+// Bounded tube (tube_ext_q >= 0, Fig. 4(b) "along the seed"): along the line the grain must
+// lie between the two seed grains or at most ext beyond either:  -ext |d| <= (P-A).d <= D2 + ext |d|, compared exactly
+// through squares.  |s| < 2^31, ext <= 2^16, D2 < 2^22: every product below 2^62.  ext < 0: the whole line.
+__device__ __forceinline__ bool emu_axial_ok(int ext, long long s, long long d2) {
+  if (ext < 0) return true;
+  const long long e2d2 = (long long)ext * ext * d2;
+  if (s < 0 && s * s > e2d2) return false;
+  const long long t = s - d2;
+  if (t > 0 && t * t > e2d2) return false;
+  return true;
+}
+
 __device__ __forceinline__ int emu_clampcell_f(float x, float inv_cs, int n) {
   return (int)fminf(fmaxf(floorf(x * inv_cs), 0.0f), (float)(n - 1));
 }
@@ -127,6 +140,7 @@ __device__ __forceinline__ int emu_walk_tube(const EmuDev& P, const EmuBox& bb, 
   const float inv_dz = dz ? 1.0f / (float)dz : 0.0f;
   const int nx = P.n[0], ny = P.n[1], nz = P.n[2];
   int tests = 0;
+  const long long d2 = (long long)dx * dx + (long long)dy * dy + (long long)dz * dz;
   int cz_lo = 0, cz_hi = nz - 1;
   if (dz == 0) {
     cz_lo = emu_clampcell_f(faz - R, P.inv_cs[2], nz);
@@ -162,7 +176,8 @@ __device__ __forceinline__ int emu_walk_tube(const EmuDev& P, const EmuBox& bb, 
       for (int j = s; j < e; ++j) {
         int4 p = __ldg(sorted + j);
         ++tests;
-        if (emu_in_tube(p.x, p.y, p.z, ax, ay, az, dx, dy, dz, r2D2)) hit(j);
+        if (emu_in_tube(p.x, p.y, p.z, ax, ay, az, dx, dy, dz, r2D2) &&
+            emu_axial_ok(P.ext, (long long)(p.x - ax) * dx + (long long)(p.y - ay) * dy + (long long)(p.z - az) * dz, d2)) hit(j);
       }
     }
   }

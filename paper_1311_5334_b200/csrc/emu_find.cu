@@ -442,7 +442,7 @@ k_plan(EmuDev P, Tilings TT, FramePtrs F, const EmuBox* __restrict__ bbox, int v
   if (cell_start[vbase + P.fr[f].ncell] == cell_start[vbase]) return;          // empty view: no bricks
   {
     const EmuBox bb = bbox[v];                                               // lab coordinates
-    bool in_box = P.packed_ok != 0;
+    bool in_box = P.packed_ok != 0 && P.ext < 0;                            // the bounded tube runs on the generic kernels
 #pragma unroll
     for (int a = 0; a < 3; ++a) in_box = in_box && bb.lo[a] >= 0 && bb.hi[a] < P.n[a] * P.cs[a];
 #pragma unroll

@@ -49,7 +49,7 @@ def test_host_only_calls(E):
     assert bin_b >= 64000 * 16 and find_b > 0
     assert E.emu_host_arena_bytes(prm, 64000, 1) > bin_b
     # documented range violations -> EMU_ERR_INVALID
-    for bad in (dict(tube_ext_q=10), dict(min_grains=1), dict(sep_max_q=4096)):
+    for bad in (dict(tube_ext_q=-2), dict(min_grains=1), dict(sep_max_q=4096)):
         kw = dict(view_size_q=(22400, 19200, 3200), cell_size_q=(256, 256, 256), sep_min_q=256, sep_max_q=1280,
                   tube_r2_q=2621, min_grains=8)
         kw.update(bad)

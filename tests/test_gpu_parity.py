@@ -180,7 +180,7 @@ def test_capacity_and_range_errors_are_reported(E):
     g = b.grains.copy(); g[5, 0] = 1 << 17
     got = run_gpu(E, default_params(0), g, b.view_off)
     assert int(got["counts"][E.EMU_CNT["status"]]) & E.EMU_ST["coord"]
-    prm = E.make_params((6400, 6400, 3200), (512, 512, 512), 256, 1280, 2621, 8, tube_ext_q=100)
+    prm = E.make_params((6400, 6400, 3200), (512, 512, 512), 256, 1280, 2621, 8, tube_ext_q=-2)
     with pytest.raises(E.EmuError):
         E.emu_workspace_bytes(prm, 10, 1)
 
@@ -226,3 +226,21 @@ def test_bench_workload_sampled_views(E, oracle_mod):
             assert np.array_equal(gf[f], rf[f])
         assert np.all(np.abs(gf["slope"] - rf["slope"]) <= 1e-5 * np.maximum(np.abs(gf["slope"]), np.abs(rf["slope"])) + 1e-12)
         assert np.all(np.abs(gf["icpt"] - rf["icpt"]) <= 1e-5 * np.maximum(np.abs(gf["icpt"]), np.abs(rf["icpt"])) + 1e-6)
+
+
+@pytest.mark.parametrize("cfg,ext_q", [(0, 0), (0, 640), (2, 320), (3, 1280)])
+def test_bounded_tube_bit_exact(E, oracle_mod, cfg, ext_q):
+    """tube_ext_q >= 0 (a grain counts only if its foot lies between the seed grains or at most
+    tube_ext_q beyond either).  Per-seed counts and the track list against the oracle."""
+    b = make_config(cfg)
+    p = dict(default_params(cfg), tube_ext_q=ext_q)
+    ref = oracle_mod.track_views(p, b.grains, b.view_off, "cells", 1, seed_dump=True)
+    dump, counts = seed_dump_gpu(E, p, b.grains, b.view_off, ref.counters["seeds"] + 16)
+    assert int(counts[E.EMU_CNT["seeds"]]) == ref.counters["seeds"]
+    a = dump[np.lexsort((dump[:, 2], dump[:, 1], dump[:, 0]))]
+    r = ref.seed_dump[np.lexsort((ref.seed_dump[:, 2], ref.seed_dump[:, 1], ref.seed_dump[:, 0]))]
+    assert np.array_equal(a, r)
+    got = run_gpu(E, p, b.grains, b.view_off, tube_ext_q=ext_q)
+    assert_same_tracks(E, got, ref)
+    whole = oracle_mod.track_views(default_params(cfg), b.grains, b.view_off, "cells", 1)
+    assert ref.counters["candidates"] < whole.counters["candidates"]
