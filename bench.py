@@ -64,9 +64,14 @@ def make_workload(first_view: int, n_views: int):
     return np.concatenate(gs), off
 
 
+TUBE_EXT_Q = -1                  # -1 = the contract (whole line); >= 0: the bounded tube of SURVEY 8(f) NEXT-1 (--tube-ext-um)
+
+
 def params_dict():
     from emu_synth import default_params
-    return default_params(CFG, cell_um=CELL_UM, max_tracks_per_view=4096)
+    p = default_params(CFG, cell_um=CELL_UM, max_tracks_per_view=4096)
+    p["tube_ext_q"] = TUBE_EXT_Q
+    return p
 
 
 class ClockSampler:
@@ -173,7 +178,8 @@ def workload_config(views_per_gpu: int, n_gpus: int) -> dict:
     return {"workload": "BASELINE.json configs[4] throughput batch: independent 350x300x50 um views, fog 10/1000 um^3, "
                         "300 isotropic through tracks per view, int32 coords at 1/64 um, seeded synthetic (key (4, view))",
             "views_per_gpu": views_per_gpu, "views_total": views_per_gpu * n_gpus,
-            "tracking": "tube r2 2621 q^2 (0.8 um), pair separation 256..1280 q (4..20 um), min 8 grains, whole-line tube",
+            "tracking": "tube r2 2621 q^2 (0.8 um), pair separation 256..1280 q (4..20 um), min 8 grains, " +
+                        ("whole-line tube" if TUBE_EXT_Q < 0 else f"bounded tube, {TUBE_EXT_Q} q beyond the seed grains (NEXT-1, not the contract)"),
             "cell_um": list(CELL_UM), "parallelism": f"views sharded over {n_gpus} GPU(s), no collective",
             "l2": "inputs (about 1 GB of grains per step) exceed the 126 MB L2; no flush needed"}
 
@@ -191,10 +197,15 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cell-um", type=float, nargs=3, default=None, help="override the cell size of the 3D hash (um)")
+    ap.add_argument("--tube-ext-um", type=float, default=None,
+                    help="bounded tube (SURVEY 8(f) NEXT-1): axial extent beyond the seed grains in um; default: whole line")
     args = ap.parse_args()
     if args.cell_um is not None:
         global CELL_UM
         CELL_UM = tuple(float(x) for x in args.cell_um)
+    if args.tube_ext_um is not None:
+        global TUBE_EXT_Q
+        TUBE_EXT_Q = int(round(args.tube_ext_um * 64))
     if args.impl == "reference":
         run_reference(args)
         return
@@ -220,7 +231,7 @@ def main():
     grains, off = make_workload(first_view, V)
     n = int(off[-1])
     prm = E.make_params(**{k: p[k] for k in ("view_size_q", "cell_size_q", "sep_min_q", "sep_max_q", "tube_r2_q",
-                                             "min_grains", "max_tracks_per_view")})
+                                             "min_grains", "max_tracks_per_view", "tube_ext_q")})
     d_grains = torch.from_numpy(grains).cuda()
     d_off = torch.from_numpy(off).cuda()
     B = E.PathBuffers(prm, n, V)

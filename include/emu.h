@@ -48,7 +48,7 @@ typedef struct emu_params {
   int32_t tube_ext_q;          /* -1 = count along the whole line (reading Q4, the contract).  >= 0 (<=     */
                                /* 65536): bounded tube (Fig. 4(b) "along the seed"): a grain counts   */
                                /* only if its foot on the line lies between the seed grains or at most     */
-                               /* tube_ext_q beyond either; exact; runs on the global-memory kernels       */
+                               /* tube_ext_q beyond either (exact: compared through squares in 64 bits)     */
   int32_t min_grains;          /* threshold, >= 2: n >= min_grains (reading Q6; "e.g. 5")             */
   int32_t max_tracks_per_view; /* capacity of the track list per view, 1..65536                            */
   int32_t reserved[4];         /* sizing hints for the internal chunks of emu_find_tracks:                 */

@@ -442,7 +442,7 @@ k_plan(EmuDev P, Tilings TT, FramePtrs F, const EmuBox* __restrict__ bbox, int v
   if (cell_start[vbase + P.fr[f].ncell] == cell_start[vbase]) return;          // empty view: no bricks
   {
     const EmuBox bb = bbox[v];                                               // lab coordinates
-    bool in_box = P.packed_ok != 0 && P.ext < 0;                            // the bounded tube runs on the generic kernels
+    bool in_box = P.packed_ok != 0;
 #pragma unroll
     for (int a = 0; a < 3; ++a) in_box = in_box && bb.lo[a] >= 0 && bb.hi[a] < P.n[a] * P.cs[a];
 #pragma unroll
@@ -559,7 +559,11 @@ struct BrickShared {
   int carry;
 };
 
-template <int kMode>
+// kBounded: the bounded tube (tube_ext_q >= 0).  The walk is clipped to the part of the line between the seed grains
+// plus the extension, and the test adds the axial condition -E |d| <= (P-A).d <= D2 + E |d| in float, as
+// |s_f - D2/2| <= D2/2 + E |d|, with its own error band (|s_f - s| <= 16: three products below 2^27; E |d| through
+// sqrtf: relative 2^-22 of at most 2^27) and the exact predicate emu_axial_ok inside the band.
+template <int kMode, bool kBounded>
 __global__ void __launch_bounds__(kBrickThreads, 1)
 k_brick(EmuDev P, FramePtrs F, int v0, const Brick* __restrict__ bricks, FindCtl* __restrict__ ctl,
         int slices, const int4* __restrict__ geo, const unsigned* __restrict__ item_ci,
@@ -685,6 +689,7 @@ k_brick(EmuDev P, FramePtrs F, int v0, const Brick* __restrict__ bricks, FindCtl
     float a = 0.f, y0 = 0.f;                         // v(u) = y0 + a u
     float oxm = 0.f, oym = 0.f, ozm = 0.f;           // magic-biased origin of v = P - A for the current row
     float T = 0.f, band = 0.f;                       // r2 D2 and the half-width of the float test's error band
+    float amid = 0.f, ahalf = 0.f, aband = 0.f;      // bounded tube: |(P-A).d - amid| <= ahalf, error band aband
     unsigned short* rec = nullptr;                   // hit record of the lane's seed in this brick
     float t0 = 0.f, t1 = 0.f;                        // u interval of the line inside the brick
     float pk0 = 0.f, pk1 = 0.f;                      // two values parked between the stages of the refill
@@ -709,8 +714,14 @@ k_brick(EmuDev P, FramePtrs F, int v0, const Brick* __restrict__ bricks, FindCtl
     };
     auto exact_in = [&](float vx, float vy, float vz) {
       const int idx = __float2int_rn(dx), idy = __float2int_rn(dy), idz = __float2int_rn(dz);
-      return emu_in_tube(__float2int_rn(vx), __float2int_rn(vy), __float2int_rn(vz), 0, 0, 0, idx, idy, idz,
-                         (long long)P.r2 * (long long)(idx * idx + idy * idy + idz * idz));
+      const int ivx = __float2int_rn(vx), ivy = __float2int_rn(vy), ivz = __float2int_rn(vz);
+      const long long id2 = (long long)(idx * idx + idy * idy + idz * idz);
+      if (!emu_in_tube(ivx, ivy, ivz, 0, 0, 0, idx, idy, idz, (long long)P.r2 * id2)) return false;
+      return !kBounded || emu_axial_ok(P.ext, (long long)ivx * idx + (long long)ivy * idy + (long long)ivz * idz, id2);
+    };
+    // bounded tube: distance of the axial coordinate (P-A).d from the middle of the allowed interval, in float
+    auto axial = [&](float vx, float vy, float vz) {
+      return fabsf(__fmaf_rn(vx, dx, __fmaf_rn(vy, dy, __fmul_rn(vz, dz))) - amid);
     };
 
     for (;;) {
@@ -756,6 +767,11 @@ k_brick(EmuDev P, FramePtrs F, int v0, const Brick* __restrict__ bricks, FindCtl
             else hit = hit && (ay >= blo[1]) && (ay <= bhi[1]);
             if (dz != 0.f) { const float p = (blo[2] - z0) * inv_b, r = (bhi[2] - z0) * inv_b; t0 = fmaxf(t0, fminf(p, r)); t1 = fminf(t1, fmaxf(p, r)); }
             else hit = hit && (az >= blo[2]) && (az <= bhi[2]);
+            if (kBounded) {
+              // the feet of the grains that can count lie between u(A) - E du/|d| and u(B) + E du/|d| (2 q of slack)
+              const float eu = __fmaf_rn((float)P.ext * dx, rsqrtf(__fmaf_rn(dx, dx, __fmaf_rn(dy, dy, dz * dz))) * 1.0001f, 2.0f);
+              t0 = fmaxf(t0, ax - eu); t1 = fminf(t1, ax + dx + eu);
+            }
             if (hit && t0 <= t1) {
               sidx = idx;
               ozm = az; pk0 = bz; pk1 = z0; dty = inv_a; dtz = inv_b;       // parked for stage 2
@@ -775,6 +791,10 @@ k_brick(EmuDev P, FramePtrs F, int v0, const Brick* __restrict__ bricks, FindCtl
             const float m_up = P.Rup * (dx + fabsf(dy) + fabsf(dz));
             const float delta = __fmaf_rn(m_up, 4.76837158203125e-7f, 16.0f);   // 16 + 2^-21 m_up
             band = __fmaf_rn(1.01f * delta, __fmaf_rn(2.0f, m_up, delta), T * 9.5367431640625e-7f);
+          }
+          if (kBounded) {
+            const float L = (float)P.ext * sqrtf(D2);
+            amid = 0.5f * D2; ahalf = amid + L; aband = __fmaf_rn(L, 1.9073486328125e-6f, 160.0f);   // 160 + 2^-19 E |d|
           }
           if (record) rec = recs + ((size_t)sidx * (kRecBricks * kRecSlots) + rec_ord);
           if (kMode == kAssoc) {
@@ -864,7 +884,14 @@ k_brick(EmuDev P, FramePtrs F, int v0, const Brick* __restrict__ bricks, FindCtl
               }
             };
             const bool two = j + 4u < e;
-            if (fminf(fabsf(s0 - T), fabsf(s1 - T)) > band) {      // the common case: the float test decides both
+            if (kBounded) {
+              const float a0 = axial(v0x, v0y, v0z), a1 = axial(v1x, v1y, v1z);
+              if (fminf(fabsf(s0 - T), fabsf(s1 - T)) > band && fminf(fabsf(a0 - ahalf), fabsf(a1 - ahalf)) > aband) {
+                commit(s0 <= T && a0 <= ahalf, (s1 <= T && a1 <= ahalf) && two);
+              } else {                                             // inside one of the error bands: the exact predicates
+                commit(exact_in(v0x, v0y, v0z), exact_in(v1x, v1y, v1z) && two);
+              }
+            } else if (fminf(fabsf(s0 - T), fabsf(s1 - T)) > band) {   // the common case: the float test decides both
               commit(s0 <= T, (s1 <= T) && two);
             } else {                                               // inside the error band: the exact predicate
               const bool in0 = fabsf(s0 - T) <= band ? exact_in(v0x, v0y, v0z) : (s0 <= T);
@@ -1659,8 +1686,9 @@ static int vote_chunk(const EmuDev& P, const Tilings& TT, FindWs& W, const Frame
   EMU_LAUNCH(EMU_STAGE_PREP, st, k_plan<<<grid_for(3 * nv, 4, 1 << 20), 128, 0, st>>>(
       P, TT, F, W.bbox, v0, v1, W.bricks, (unsigned)W.brick_cap, W.vf_brick_base, W.ctl));
   EMU_LAUNCH(EMU_STAGE_PREP, st, k_plan_finish<<<1, 1, 0, st>>>(W.ctl, (unsigned)W.brick_cap));
-  EMU_CK(cudaFuncSetAttribute(k_brick<kVote>, cudaFuncAttributeMaxDynamicSharedMemorySize, kPoolBytes));
-  EMU_LAUNCH(EMU_STAGE_VOTE, st, k_brick<kVote><<<kSM, kBrickThreads, kPoolBytes, st>>>(
+  auto vote_kernel = P.ext >= 0 ? k_brick<kVote, true> : k_brick<kVote, false>;
+  EMU_CK(cudaFuncSetAttribute(vote_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kPoolBytes));
+  EMU_LAUNCH(EMU_STAGE_VOTE, st, vote_kernel<<<kSM, kBrickThreads, kPoolBytes, st>>>(
       P, F, v0, W.bricks, W.ctl, slices, W.geo, nullptr, W.view_seed_off, W.seed_cnt, W.recs, W.slot_row, nullptr,
       nullptr, counts));
   return EMU_OK;
@@ -1719,10 +1747,11 @@ int emu_find_launch(const EmuDev& P, int seeds_per_grain, int cand_per_grain, co
     EMU_LAUNCH(EMU_STAGE_PREP, st, k_cands_finish<<<1, 1, 0, st>>>(W.ctl, (unsigned)W.cand_cap, counts));
     EMU_LAUNCH(EMU_STAGE_PREP, st, k_reset_cand_arrays<<<kSM * 8, 256, 0, st>>>(W.ctl, W.wins, W.cand_track));
     // A5
-    EMU_CK(cudaFuncSetAttribute(k_brick<kAssoc>, cudaFuncAttributeMaxDynamicSharedMemorySize, kPoolBytes));
+    auto walk_kernel = P.ext >= 0 ? k_brick<kAssoc, true> : k_brick<kAssoc, false>;
+    EMU_CK(cudaFuncSetAttribute(walk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kPoolBytes));
     EMU_LAUNCH(EMU_STAGE_ASSOC, st, k_assoc_hits<<<dim3(48, 3 * nv), 256, 0, st>>>(
         v0, W.ctl, W.view_cand_off, W.cands, W.cand_seed, W.seed_cnt, W.recs, W.slot_row, W.vf_brick_base, W.keyA, W.keyB));
-    EMU_LAUNCH(EMU_STAGE_ASSOC, st, k_brick<kAssoc><<<kSM, kBrickThreads, kPoolBytes, st>>>(
+    EMU_LAUNCH(EMU_STAGE_ASSOC, st, walk_kernel<<<kSM, kBrickThreads, kPoolBytes, st>>>(
         P, F, v0, W.bricks, W.ctl, slices_walk, W.ovf_geo, W.ovf_ci, W.view_ovf_off, nullptr, nullptr, nullptr, W.keyA, W.keyB,
         counts));
     EMU_LAUNCH(EMU_STAGE_ASSOC, st, k_assoc_generic<0><<<kSM * 16, kVoteThreads, 0, st>>>(

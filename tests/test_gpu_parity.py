@@ -228,12 +228,15 @@ def test_bench_workload_sampled_views(E, oracle_mod):
         assert np.all(np.abs(gf["icpt"] - rf["icpt"]) <= 1e-5 * np.maximum(np.abs(gf["icpt"]), np.abs(rf["icpt"])) + 1e-6)
 
 
+@pytest.mark.parametrize("cell_um", [(8.0, 8.0, 8.0), (4.0, 4.0, 4.0), (3.0, 4.0, 2.5)])
 @pytest.mark.parametrize("cfg,ext_q", [(0, 0), (0, 640), (2, 320), (3, 1280)])
-def test_bounded_tube_bit_exact(E, oracle_mod, cfg, ext_q):
+def test_bounded_tube_bit_exact(E, oracle_mod, cfg, ext_q, cell_um):
     """tube_ext_q >= 0 (a grain counts only if its foot lies between the seed grains or at most
-    tube_ext_q beyond either).  Per-seed counts and the track list against the oracle."""
+    tube_ext_q beyond either).  Per-seed counts and the track list against the oracle; 8 um cells take the generic
+    global-memory kernels, the finer ones the shared-memory brick kernels (clipped walk, float axial test with the
+    exact fallback)."""
     b = make_config(cfg)
-    p = dict(default_params(cfg), tube_ext_q=ext_q)
+    p = dict(default_params(cfg, cell_um=cell_um), tube_ext_q=ext_q)
     ref = oracle_mod.track_views(p, b.grains, b.view_off, "cells", 1, seed_dump=True)
     dump, counts = seed_dump_gpu(E, p, b.grains, b.view_off, ref.counters["seeds"] + 16)
     assert int(counts[E.EMU_CNT["seeds"]]) == ref.counters["seeds"]
