@@ -424,6 +424,7 @@ k_bin_chunk(EmuDev P, int frame, SplitPlan S, const int* __restrict__ view_off, 
   unsigned short* cnt = reinterpret_cast<unsigned short*>(chunk_smem + (size_t)S.cap * 16);   // [cpc] counts
   unsigned short* pre = cnt + ((S.cpc + 1) & ~1);                                    // [cpc] exclusive prefix
   unsigned* cntw = reinterpret_cast<unsigned*>(cnt);
+  int* wbuf = reinterpret_cast<int*>(pre + ((S.cpc + 1) & ~1));                      // [cap] rows in arrival order
   const int4* src = tmp + ((size_t)v * S.K + k) * S.cap;
   const int n = min(cur[(size_t)v * S.K + k], S.cap);
   int4 gg[kChunkPer];                                  // the chunk's grains stay in registers: one batch of independent loads
@@ -443,14 +444,15 @@ k_bin_chunk(EmuDev P, int frame, SplitPlan S, const int* __restrict__ view_off, 
   __syncthreads();
   const int base = base_s;
   // ---- count per cell (the chunk's grains stay in registers: one batch of independent loads) ----
-  int cc[kChunkPer];
+  int cc[kChunkPer], rk[kChunkPer];                            // cell inside the chunk, arrival rank inside the cell
 #pragma unroll
   for (int u = 0; u < kChunkPer; ++u) {
-    cc[u] = -1;
+    cc[u] = -1; rk[u] = 0;
     if (tid + u * kChunkThreads < n) {
       cc[u] = min((int)((unsigned)gg[u].x >> 18), nc - 1);     // the cell inside the chunk, packed by pass 1
       gg[u].x = (gg[u].x << 14) >> 14;                         // x again (sign-extended 18 bits)
-      atomicAdd(&cntw[cc[u] >> 1], 1u << (16 * (cc[u] & 1)));
+      const int sh = 16 * (cc[u] & 1);
+      rk[u] = (int)((atomicAdd(&cntw[cc[u] >> 1], 1u << sh) >> sh) & 0xffffu);
     }
   }
   __syncthreads();
@@ -475,34 +477,20 @@ k_bin_chunk(EmuDev P, int frame, SplitPlan S, const int* __restrict__ view_off, 
   for (int c = c0; c < c1; ++c) { pre[c] = (unsigned short)run; run += cnt[c]; }
   __syncthreads();
   for (int c = tid; c < nc; c += kChunkThreads) cell_start[(size_t)v * ncell + c_lo + c] = base + (int)pre[c];
-  for (int w = tid; w < (nc + 1) / 2; w += kChunkThreads) cntw[w] = 0u;
+  // ---- the rows of the grains go to their cell's range in arrival order ...
+#pragma unroll
+  for (int u = 0; u < kChunkPer; ++u) if (cc[u] >= 0) wbuf[(int)pre[cc[u]] + rk[u]] = gg[u].w;
   __syncthreads();
-  // ---- place; the counters count up again ----
+  // ---- ... and every grain takes the place its row deserves among its cell-mates (ascending row inside every cell;
+  //      rows are distinct: the ranks are a permutation) ----
 #pragma unroll
   for (int u = 0; u < kChunkPer; ++u) {
     if (cc[u] < 0) continue;
-    const int sh = 16 * (cc[u] & 1);
-    const int r = (int)((atomicAdd(&cntw[cc[u] >> 1], 1u << sh) >> sh) & 0xffffu);
-    buf[(int)pre[cc[u]] + r] = gg[u];
-  }
-  __syncthreads();
-  // ---- ascending row inside every cell: a grain whose cell holds several looks at the rows of its cell-mates in
-  //      the buffer and moves to the place its own row deserves (rows are distinct: the ranks are a permutation) ----
-  int np[kChunkPer];
-#pragma unroll
-  for (int u = 0; u < kChunkPer; ++u) {
-    np[u] = -1;
-    if (cc[u] < 0) continue;
-    const int m = cnt[cc[u]];
-    if (m < 2) continue;
-    const int p0 = pre[cc[u]];
+    const int m = cnt[cc[u]], p0 = pre[cc[u]];
     int r = 0;
-    for (int t = 0; t < m; ++t) r += (buf[p0 + t].w < gg[u].w);
-    np[u] = p0 + r;
+    if (m >= 2) for (int t = 0; t < m; ++t) r += (wbuf[p0 + t] < gg[u].w);
+    buf[p0 + r] = gg[u];
   }
-  __syncthreads();
-#pragma unroll
-  for (int u = 0; u < kChunkPer; ++u) if (np[u] >= 0) buf[np[u]] = gg[u];
   __syncthreads();
   for (int i = tid; i < n; i += kChunkThreads) sorted[base + i] = buf[i];
 }
@@ -561,7 +549,7 @@ int emu_bin_launch(const EmuDev& P, int frame, const int32_t* d_grains, const in
   const SplitPlan S = split_plan(P, frame, n_grains, n_views);
   if (S.K > 0 && n_views <= 65535) {
     // two passes: split into chunks of cells, then one chunk per block in shared memory
-    const size_t smem = (size_t)S.cap * 16 + 2 * (size_t)((S.cpc + 1) & ~1) * sizeof(unsigned short);
+    const size_t smem = (size_t)S.cap * 16 + 2 * (size_t)((S.cpc + 1) & ~1) * sizeof(unsigned short) + (size_t)S.cap * 4;
     if (cudaFuncSetAttribute(k_bin_chunk, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return EMU_ERR_CUDA;
     if (cudaMemsetAsync(redo, 0, ((size_t)n_views + 1) * sizeof(int), st) != cudaSuccess) return EMU_ERR_CUDA;
     if (cudaMemsetAsync(cur, 0, (size_t)n_views * S.K * sizeof(int), st) != cudaSuccess) return EMU_ERR_CUDA;
