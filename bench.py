@@ -37,11 +37,11 @@ ALG_PER_SEED = {(8.0, 8.0, 8.0): (317.7, 2.88), (3.0, 4.0, 4.0): (102.1, 2.26)}
 INSTR_PER_TEST, INSTR_PER_PAIR = 18, 9
 BIN_BYTES_PER_GRAIN = 32.0       # 16 B read + 16 B written per grain; + 4 B per cell of the grid
 # DRAM bytes (read + write) of one k_brick<kVote> launch per view of the launch, from the committed ncu --set full
-# capture profiles/r1d_k_brick_full.txt (16 views: 20.97 GB read + 13.97 GB written)
-VOTE_DRAM_BYTES_PER_VIEW = (20.972941e9 + 13.967086e9) / 16
-# DRAM bytes of the two binning kernels per grain, from profiles/r1d_k_bin_full.txt (65 792 077 grains:
-# k_bin_split 1.067 + 1.009 GB, k_bin_chunk 1.058 + 1.468 GB)
-BIN_DRAM_BYTES_PER_GRAIN = (1.066770e9 + 1.009274e9 + 1.057934e9 + 1.467562e9) / 65792077
+# capture profiles/r1e_k_brick_full.txt (16 views: 20.98 GB read + 13.90 GB written)
+VOTE_DRAM_BYTES_PER_VIEW = (20.978974e9 + 13.904418e9) / 16
+# DRAM bytes of the two binning kernels per grain, from profiles/r1e_k_bin_full.txt (65 792 077 grains:
+# k_bin_split 1.053 + 1.006 GB, k_bin_chunk 1.055 + 1.457 GB)
+BIN_DRAM_BYTES_PER_GRAIN = (1.053481e9 + 1.005627e9 + 1.055078e9 + 1.456763e9) / 65792077
 
 
 def _gen_view(v):
@@ -323,7 +323,7 @@ def main():
                               "three frames)", "bound": "alu", "achieved": achieved, "peak": alu_peak,
                     "unit": "Tlane-instr/s", "frac": achieved / alu_peak,
                     "traffic": VOTE_DRAM_BYTES_PER_VIEW * views_per_launch,
-                    "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of profiles/r1d_k_brick_full.txt per view "
+                    "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of profiles/r1e_k_brick_full.txt per view "
                                       "x views per launch",
                     "peak_source": f"148 SM x 4 schedulers x 32 lanes x {sm_max:.0f} MHz ({peaks['_source']} max SM clock)",
                     "algorithmic": f"{seeds} seeds x ({alg[0]:.1f} tests x {INSTR_PER_TEST} + {alg[1]:.2f} pair tests x "
@@ -337,7 +337,7 @@ def main():
     bin_gbs = bin_bytes / (bin_ms * 1e-3) / 1e9 if bin_ms > 0 else 0.0
     roofline_bin = {"kernel": "emu_bin_grains: k_bin_split + k_bin_chunk (two passes: chunks of cells through a scratch array, then one chunk per block in shared memory)", "bound": "hbm",
                     "achieved": bin_gbs, "peak": hbm, "unit": "GB/s", "frac": bin_gbs / hbm,
-                    "traffic": BIN_DRAM_BYTES_PER_GRAIN * n, "traffic_source": "profiles/r1d_k_bin_full.txt, both passes, per grain x grains",
+                    "traffic": BIN_DRAM_BYTES_PER_GRAIN * n, "traffic_source": "profiles/r1e_k_bin_full.txt, both passes, per grain x grains",
                     "algorithmic_bytes": bin_bytes, "ms": bin_ms,
                     "algorithmic_bytes_per_grain": bin_bytes / max(1, n),
                     "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peaks['_source']})"}
