@@ -197,6 +197,9 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cell-um", type=float, nargs=3, default=None, help="override the cell size of the 3D hash (um)")
+    ap.add_argument("--latency-views", type=int, default=0,
+                    help="also time single views one at a time through the host call (SURVEY 8(f) NEXT-3: the microscope "
+                         "delivers one view every 0.2 s, P:102); adds the key single_view to the JSON line")
     ap.add_argument("--tube-ext-um", type=float, default=None,
                     help="bounded tube (SURVEY 8(f) NEXT-1): axial extent beyond the seed grains in um; default: whole line")
     args = ap.parse_args()
@@ -342,6 +345,35 @@ def main():
                     "algorithmic_bytes_per_grain": bin_bytes / max(1, n),
                     "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peaks['_source']})"}
 
+    single = None
+    if args.latency_views > 0:
+        # one view per host call (H2D + path + D2H inside), config 4 (the bench density) and config 1 (one microscope view)
+        from emu_synth import CONFIGS, default_params, make_view
+        single = {}
+        for cfg_i in (CFG, 1):
+            pp = default_params(cfg_i, cell_um=CELL_UM, max_tracks_per_view=4096)
+            pp["tube_ext_q"] = TUBE_EXT_Q
+            pr = E.make_params(**{k: pp[k] for k in ("view_size_q", "cell_size_q", "sep_min_q", "sep_max_q", "tube_r2_q",
+                                                      "min_grains", "max_tracks_per_view", "tube_ext_q")})
+            views = [make_view(CONFIGS[cfg_i], cfg_i, v)[0] for v in range(args.latency_views)]
+            nmax = max(len(g) for g in views)
+            H1 = E.HostPath(pr, nmax, 1)
+            ts = []
+            for rep_i in range(2):                                  # the first round warms up
+                for g in views:
+                    H1.n_grains = len(g)
+                    H1.h_grains[:len(g)].copy_(torch.from_numpy(g))
+                    H1.h_view_off.copy_(torch.tensor([0, len(g)], dtype=torch.int32))
+                    torch.cuda.synchronize()
+                    t0 = time.perf_counter()
+                    H1.call()
+                    if rep_i:
+                        ts.append((time.perf_counter() - t0) * 1e3)
+            single[f"config{cfg_i}"] = {"views": len(views), "grains_per_view": int(np.mean([len(g) for g in views])),
+                                        "ms_median": float(np.median(ts)), "ms_max": float(np.max(ts))}
+            del H1
+            torch.cuda.empty_cache()
+
     val = n_total / (ms_step * 1e-3)
     line = {
         "metric": "grains_per_s", "value": val, "unit": "grains/s", "n_gpus": world, "steps": args.steps,
@@ -355,6 +387,7 @@ def main():
         "gpu_launches": int(sum(stage_launches.values())),
         "stage_ms_per_step": {k: v / args.steps for k, v in stage_ms.items()},
         "roofline": roofline, "roofline_bin": roofline_bin, "cpu_baseline": cpu, "e2e": e2e, "clocks": clocks,
+        "single_view": single,
     }
     print(json.dumps(line))
     if world > 1:
