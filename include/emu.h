@@ -89,6 +89,7 @@ typedef struct emu_fit {       /* 48 B */
 #define EMU_ST_RANGE 8            /* a count does not fit its field (n_tube >= 8192)                       */
 #define EMU_ST_COORD 16           /* emu_bin_grains saw |coordinate| >= 2^17                               */
 #define EMU_ST_SEED_OVERFLOW 32   /* seed workspace too small: give more workspace / raise reserved[1]     */
+#define EMU_ST_GRAIN_OVERFLOW 64  /* emu_recognize_grains found more grains than d_grains can hold         */
 
 /* Host-only (no CUDA call).  Workspace each call needs for this batch shape; both outputs optional.
  * find_bytes is a recommendation (internal view chunks adapt to whatever >= the minimum is given). */
@@ -142,6 +143,25 @@ int emu_fit_tracks(const emu_params* params, const int32_t* d_grains, const emu_
                    const int32_t* d_track_off, const int32_t* d_members, int32_t n_views,
                    emu_fit* d_fits, void* stream);
 
+/* A0, upstream of the hot path: 3D grain recognition on stacks of filtered frames (P:68-70:
+ * "Each pixel with a pulse height higher than a given threshold is compared to the 3 x 3 x 3 neighboring pixels; the
+ * pixel with the highest pulse height among these will be defining the grain.  The spatial coordinates of the grains
+ * are then computed with a center-of-mass method using the pulse height of each pixel").  Readings R1-R5, DESIGN.md 3b:
+ * voxels outside the stack count as 0; of equal maxima the first in raster order (z, y, x) defines the grain; centre
+ * of mass over the 3x3x3 neighbourhood with weight = pulse height where it exceeds the threshold, else 0;
+ * pos_q = floor(pitch_q * (sum(w i) / sum(w) + 1/2) + 1/2) per axis, exact in integers.
+ *  in : d_vox uint8[n_views][nz][ny][nx] (x fastest); threshold 0..254; pitch_q[3] = voxel pitch in q along x, y, z
+ *       (HOST array, 1..4096 each); nx, ny, nz >= 1, n_views * ny * nz < 2^31.
+ *  out: d_grains int32[<= capacity][4] = x_q, y_q, z_q, pulse height of the defining voxel, view after view, inside
+ *       a view in raster order of the defining voxel - the layout emu_bin_grains takes (its w is payload);
+ *       d_view_off int32[n_views+1]; d_count int64[1] = grains found (may exceed capacity: then d_status gets
+ *       EMU_ST_GRAIN_OVERFLOW and the excess is not written); d_status int64[1], OR-ed, never cleared here.
+ *  d_ws: scratch of emu_recognize_ws_bytes(n_views, ny, nz) bytes. */
+size_t emu_recognize_ws_bytes(int32_t n_views, int32_t ny, int32_t nz);
+int emu_recognize_grains(const uint8_t* d_vox, int32_t n_views, int32_t nx, int32_t ny, int32_t nz, int32_t threshold,
+                         const int32_t* pitch_q, int32_t* d_grains, int64_t capacity, int32_t* d_view_off,
+                         int64_t* d_count, int64_t* d_status, void* d_ws, size_t ws_bytes, void* stream);
+
 /* ---- the whole path on HOST buffers (the end-to-end call: copies in, A1..A7, copies out) --------
  * h_* are HOST pointers owned by the caller (pinned memory makes the copies asynchronous and fast;
  * pageable memory works).  d_arena is one caller-owned DEVICE allocation of at least
@@ -181,6 +201,7 @@ int emu_track_views_host(const emu_params* params, const int32_t* h_grains, cons
 #define EMU_STAGE_FIT 9          /* A6                                                              */
 #define EMU_STAGE_SEEDS 10       /* A2: seed pairs (count, offsets, fill)                           */
 #define EMU_STAGE_CANDS 11       /* A4: threshold -> candidate list                                 */
+#define EMU_STAGE_RECOG 12       /* A0: grain recognition (emu_recognize_grains)                    */
 #define EMU_STAGE_COUNT 16
 typedef struct emu_profile emu_profile;
 emu_profile* emu_profile_create(void);              /* NULL on failure                              */

@@ -16,7 +16,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libemu4pi.so")
 
 EMU_CNT = dict(seeds=0, tests=1, candidates=2, tracks=3, members=4, status=5, pair_tests=6, need=7)
-EMU_ST = dict(cand_overflow=1, track_overflow=2, member_overflow=4, range=8, coord=16, seed_overflow=32)
+EMU_ST = dict(cand_overflow=1, track_overflow=2, member_overflow=4, range=8, coord=16, seed_overflow=32, grain_overflow=64)
 _ERR = {-1: "EMU_ERR_INVALID", -2: "EMU_ERR_CAPACITY", -3: "EMU_ERR_CUDA"}
 
 TRACK_DTYPE = np.dtype([("view", "<i4"), ("seed_a", "<i4"), ("seed_b", "<i4"), ("n_tube", "<i4"),
@@ -38,9 +38,9 @@ class emu_params(C.Structure):
 
 _SYMBOLS = ["emu_workspace_bytes", "emu_grid_cells", "emu_bin_grains", "emu_find_tracks", "emu_count_seeds",
             "emu_fit_tracks", "emu_host_arena_bytes", "emu_track_views_host", "emu_profile_create", "emu_profile_destroy", "emu_profile_begin", "emu_profile_end",
-            "emu_profile_read"]
+            "emu_profile_read", "emu_recognize_ws_bytes", "emu_recognize_grains"]
 EMU_STAGE = dict(bin_count=0, bin_scan=1, bin_scatter=2, bin_place=3, prep=4, vote=5, assoc=6, select=7, emit=8, fit=9,
-                 seeds=10, cands=11)
+                 seeds=10, cands=11, recog=12)
 EMU_STAGE_COUNT = 16
 _lib = None
 
@@ -73,6 +73,10 @@ def _load():
         L.emu_host_arena_bytes.argtypes = [vp, i64, i32, C.POINTER(sz)]
         L.emu_track_views_host.restype = C.c_int
         L.emu_track_views_host.argtypes = [vp, vp, vp, i64, i32, vp, vp, i64, vp, vp, i64, vp, vp, sz, vp]
+        L.emu_recognize_ws_bytes.restype = sz
+        L.emu_recognize_ws_bytes.argtypes = [i32, i32, i32]
+        L.emu_recognize_grains.restype = C.c_int
+        L.emu_recognize_grains.argtypes = [vp, i32, i32, i32, i32, i32, C.POINTER(i32 * 3), vp, i64, vp, vp, vp, vp, sz, vp]
         L.emu_profile_create.restype = vp
         L.emu_profile_create.argtypes = []
         L.emu_profile_destroy.restype = None
@@ -182,6 +186,20 @@ def emu_fit_tracks(params, d_grains, d_tracks, d_track_off, d_members, n_views, 
     _dev(d_members, torch.int32); _dev(d_fits)
     _check(_load().emu_fit_tracks(C.byref(params), _ptr(d_grains), _ptr(d_tracks), _ptr(d_track_off),
                                   _ptr(d_members), n_views, _ptr(d_fits), _stream()), "emu_fit_tracks")
+
+
+def emu_recognize_grains(d_vox, threshold: int, pitch_q, d_grains, d_view_off, d_count, d_status, d_ws):
+    """A0: d_vox uint8 [n_views, nz, ny, nx] on the device -> d_grains int32 [capacity, 4],
+    d_view_off int32 [n_views+1], d_count int64 [1].  Argument marshalling only."""
+    n_views, nz, ny, nx = (int(x) for x in d_vox.shape)
+    pitch = (C.c_int32 * 3)(*[int(x) for x in pitch_q])
+    _check(_load().emu_recognize_grains(_ptr(d_vox), n_views, nx, ny, nz, int(threshold), C.byref(pitch), _ptr(d_grains),
+                                        int(d_grains.shape[0]), _ptr(d_view_off), _ptr(d_count), _ptr(d_status), _ptr(d_ws),
+                                        _nbytes(d_ws), _stream()), "emu_recognize_grains")
+
+
+def emu_recognize_ws_bytes(n_views: int, ny: int, nz: int) -> int:
+    return int(_load().emu_recognize_ws_bytes(int(n_views), int(ny), int(nz)))
 
 
 def emu_host_arena_bytes(params: emu_params, n_grains: int, n_views: int) -> int:

@@ -7,7 +7,7 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libemu4pi.so")
-SOURCES = ["emu_api.cu", "emu_bin.cu", "emu_find.cu", "emu_fit.cu"]
+SOURCES = ["emu_api.cu", "emu_bin.cu", "emu_find.cu", "emu_fit.cu", "emu_recognize.cu"]
 HEADERS = ["emu_dev.cuh", "emu_host.h", os.path.join("..", "..", "include", "emu.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-shared", "-Xcompiler", "-fPIC", "-cudart", "static"]

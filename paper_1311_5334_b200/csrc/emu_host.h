@@ -48,6 +48,11 @@ int emu_count_seeds_launch(const EmuDev& P, int seeds_per_grain, int cand_per_gr
                            int64_t dump_capacity, int64_t* d_counts, void* d_ws, size_t ws_bytes,
                            cudaStream_t st);
 
+// emu_recognize.cu
+int emu_recognize_launch(const uint8_t* d_vox, int32_t n_views, int32_t nx, int32_t ny, int32_t nz, int32_t thr,
+                         const int32_t* pitch_q, int32_t* d_grains, int64_t capacity, int32_t* d_view_off,
+                         int64_t* d_count, int64_t* d_status, void* d_ws, size_t ws_bytes, cudaStream_t st);
+
 // emu_fit.cu
 int emu_fit_launch(const int32_t* d_grains, const emu_track* d_tracks, const int32_t* d_track_off,
                    const int32_t* d_members, int32_t n_views, emu_fit* d_fits, cudaStream_t st);
