@@ -200,6 +200,9 @@ def main():
     ap.add_argument("--latency-views", type=int, default=0,
                     help="also time single views one at a time through the host call (SURVEY 8(f) NEXT-3: the microscope "
                          "delivers one view every 0.2 s, P:102); adds the key single_view to the JSON line")
+    ap.add_argument("--recognize-views", type=int, default=0,
+                    help="also time emu_recognize_grains (SURVEY 8(f) NEXT-4) on this many synthetic 1280 x 1024 x 40 voxel "
+                         "stacks rendered from config-1 views; adds the key recognize to the JSON line")
     ap.add_argument("--tube-ext-um", type=float, default=None,
                     help="bounded tube (SURVEY 8(f) NEXT-1): axial extent beyond the seed grains in um; default: whole line")
     args = ap.parse_args()
@@ -374,6 +377,45 @@ def main():
             del H1
             torch.cuda.empty_cache()
 
+    recog = None
+    if args.recognize_views > 0:
+        from emu_synth import CONFIGS, make_view
+        from emu_synth.voxels import PITCH_Q, THRESHOLD, render_stack
+        shape = (40, 1024, 1280)                                   # the paper's view: 1280 x 1024 px x 40 frames
+        NV = args.recognize_views
+        stacks = []
+        for v in range(NV):
+            g = make_view(CONFIGS[1], 1, v)[0].astype(np.int64)
+            g = g[(g[:, 0] < shape[2] * PITCH_Q[0]) & (g[:, 1] < shape[1] * PITCH_Q[1])]      # the part of the view the stack covers
+            stacks.append(render_stack(shape, g, key=(8, v)))
+        vox = np.stack(stacks)
+        d_vox = torch.from_numpy(vox).cuda()
+        cap = 1 << 20
+        d_g = torch.empty((cap, 4), dtype=torch.int32, device="cuda"); d_o = torch.empty(NV + 1, dtype=torch.int32, device="cuda")
+        d_c = torch.zeros(1, dtype=torch.int64, device="cuda"); d_s = torch.zeros(1, dtype=torch.int64, device="cuda")
+        ws = torch.empty(E.emu_recognize_ws_bytes(NV, shape[1], shape[0]), dtype=torch.uint8, device="cuda")
+        for _ in range(3):
+            E.emu_recognize_grains(d_vox, THRESHOLD, PITCH_Q, d_g, d_o, d_c, d_s, ws)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(5):
+            E.emu_recognize_grains(d_vox, THRESHOLD, PITCH_Q, d_g, d_o, d_c, d_s, ws)
+        e1.record(); torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / 5
+        ng = int(d_c.cpu()[0])
+        from oracle.recognize import recognize_grains as oracle_recognize     # the reported CPU baseline of this stage
+        t0 = time.perf_counter(); ref = oracle_recognize(vox[0], THRESHOLD, PITCH_Q); t_or = time.perf_counter() - t0
+        n0 = int(d_o.cpu()[1])
+        same = bool(n0 == len(ref) and np.array_equal(d_g[:n0].cpu().numpy(), ref))
+        alg = vox.size + 16.0 * ng + 4.0 * NV * shape[0] * shape[1]
+        recog = {"views": NV, "voxels_per_view": int(vox[0].size), "grains": ng, "ms": ms, "views_per_s": NV / (ms * 1e-3),
+                 "roofline": {"bound": "hbm", "achieved": alg / (ms * 1e-3) / 1e9, "peak": float(peaks["hbm_gbs"]), "unit": "GB/s",
+                              "frac": alg / (ms * 1e-3) / 1e9 / float(peaks["hbm_gbs"]),
+                              "algorithmic": "1 B per voxel + 16 B per grain + 4 B per row of voxels"},
+                 "cpu_baseline": {"kind": "oracle (numpy)", "views_per_s": 1.0 / t_or, "cores": 1},
+                 "first_view_identical_to_oracle": same}
+        del d_vox
+
     val = n_total / (ms_step * 1e-3)
     line = {
         "metric": "grains_per_s", "value": val, "unit": "grains/s", "n_gpus": world, "steps": args.steps,
@@ -387,7 +429,7 @@ def main():
         "gpu_launches": int(sum(stage_launches.values())),
         "stage_ms_per_step": {k: v / args.steps for k, v in stage_ms.items()},
         "roofline": roofline, "roofline_bin": roofline_bin, "cpu_baseline": cpu, "e2e": e2e, "clocks": clocks,
-        "single_view": single,
+        "single_view": single, "recognize": recog,
     }
     print(json.dumps(line))
     if world > 1:

@@ -151,7 +151,7 @@ int emu_fit_tracks(const emu_params* params, const int32_t* d_grains, const emu_
  * of mass over the 3x3x3 neighbourhood with weight = pulse height where it exceeds the threshold, else 0;
  * pos_q = floor(pitch_q * (sum(w i) / sum(w) + 1/2) + 1/2) per axis, exact in integers.
  *  in : d_vox uint8[n_views][nz][ny][nx] (x fastest); threshold 0..254; pitch_q[3] = voxel pitch in q along x, y, z
- *       (HOST array, 1..4096 each); nx, ny, nz >= 1, n_views * ny * nz < 2^31.
+ *       (HOST array, 1..4096 each); 1 <= nx <= 65535, ny, nz >= 1, n_views * ny * nz < 2^31.
  *  out: d_grains int32[<= capacity][4] = x_q, y_q, z_q, pulse height of the defining voxel, view after view, inside
  *       a view in raster order of the defining voxel - the layout emu_bin_grains takes (its w is payload);
  *       d_view_off int32[n_views+1]; d_count int64[1] = grains found (may exceed capacity: then d_status gets

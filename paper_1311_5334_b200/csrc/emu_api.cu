@@ -277,7 +277,7 @@ int emu_recognize_grains(const uint8_t* d_vox, int32_t n_views, int32_t nx, int3
                          const int32_t* pitch_q, int32_t* d_grains, int64_t capacity, int32_t* d_view_off,
                          int64_t* d_count, int64_t* d_status, void* d_ws, size_t ws_bytes, void* stream) {
   if (n_views < 0 || nx < 1 || ny < 1 || nz < 1 || threshold < 0 || threshold > 254 || capacity < 0) return EMU_ERR_INVALID;
-  if ((int64_t)n_views * ny * nz >= ((int64_t)1 << 31) - 64 || (int64_t)nx * 4096 >= ((int64_t)1 << 31)) return EMU_ERR_INVALID;
+  if ((int64_t)n_views * ny * nz >= ((int64_t)1 << 31) - 64 || nx > 65535) return EMU_ERR_INVALID;
   if (!pitch_q || !d_view_off || !d_count || !d_status || !d_ws || (n_views > 0 && !d_vox) || (capacity > 0 && !d_grains)) return EMU_ERR_INVALID;
   for (int a = 0; a < 3; ++a) if (pitch_q[a] < 1 || pitch_q[a] > 4096) return EMU_ERR_INVALID;
   if (!aligned16(d_grains)) return EMU_ERR_INVALID;

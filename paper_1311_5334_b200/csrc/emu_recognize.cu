@@ -52,12 +52,20 @@ __device__ bool grain_of(const unsigned char* __restrict__ v, const Recog& R, in
 
 constexpr int kRecogThreads = 256;
 
+// One warp per row.  The voxels above the threshold (1-2 % of a filtered frame) are first gathered, in x order, in a
+// small ring of the warp; whenever 32 of them wait (and at the end of the row) every lane examines ONE of them - its 26
+// neighbours, the raster tie rule, the centre of mass - so the expensive part runs with full warps instead of for one
+// or two lanes of every 128 voxels.
+constexpr int kRing = 1024;                                     // >= 31 waiting + 512 new
+
 template <int kFill>
-__global__ void __launch_bounds__(kRecogThreads)
+__global__ void __launch_bounds__(kRecogThreads, 4)
 k_recog(Recog R, const unsigned char* __restrict__ vox, int n_views, int* __restrict__ row_cnt,
         const int* __restrict__ row_off, int4* __restrict__ grains, long long capacity,
         unsigned long long* __restrict__ status) {
+  __shared__ unsigned short ring_s[kRecogThreads / 32][kRing];
   const int lane = threadIdx.x & 31;
+  unsigned short* ring = ring_s[threadIdx.x >> 5];
   const long long rows_per_view = (long long)R.nz * R.ny, n_rows = rows_per_view * n_views;
   const long long warp0 = (long long)blockIdx.x * (kRecogThreads / 32) + (threadIdx.x >> 5);
   const long long n_warps = (long long)gridDim.x * (kRecogThreads / 32);
@@ -68,39 +76,64 @@ k_recog(Recog R, const unsigned char* __restrict__ vox, int n_views, int* __rest
     const unsigned char* v = vox + (size_t)view * rows_per_view * R.nx;
     const unsigned char* line = v + ((size_t)z * R.ny + y) * R.nx;
     int n_row = 0;                                              // grains of the row so far (warp-uniform)
+    int head = 0, qn = 0;                                       // the ring: first waiting entry, number waiting
     const int base = kFill ? row_off[row] : 0;
-    for (int x0 = 0; x0 < R.nx; x0 += 128) {                    // 4 voxels per lane
-      const int x = x0 + 4 * lane;
-      unsigned q = 0;
-      if (x + 3 < R.nx && (((size_t)(line + x)) & 3) == 0) q = __ldg(reinterpret_cast<const unsigned*>(line + x));
-      else {
-#pragma unroll
-        for (int k = 0; k < 4; ++k) if (x + k < R.nx) q |= (unsigned)__ldg(line + x + k) << (8 * k);
+
+    // examine the first m (<= 32) waiting voxels, one per lane; they are in x order, and so are the grains written
+    auto flush = [&](int m) {
+      __syncwarp();
+      int4 g = make_int4(0, 0, 0, 0);
+      bool ok = false;
+      if (lane < m) {
+        const int x = (int)ring[(head + lane) & (kRing - 1)];
+        ok = grain_of(v, R, x, y, z, (int)__ldg(line + x), g);
       }
+      const unsigned mk = __ballot_sync(EMU_FULL, ok);
+      if (kFill && ok) {
+        const long long at = (long long)base + n_row + __popc(mk & ((1u << lane) - 1u));
+        if (at < capacity) grains[at] = g;
+        else if (status) atomicOr(status, (unsigned long long)EMU_ST_GRAIN_OVERFLOW);
+      }
+      n_row += __popc(mk);
+      head = (head + m) & (kRing - 1); qn -= m;
+    };
+
+    // 16 voxels per lane and step: one 16-byte load, the load of the next step already in flight
+    auto load16 = [&](int x) {
+      uint4 t = make_uint4(0u, 0u, 0u, 0u);
+      if (x + 15 < R.nx && (((size_t)(line + x)) & 15) == 0) {
+        t = __ldg(reinterpret_cast<const uint4*>(line + x));
+      } else if (x < R.nx) {
+        unsigned w[4] = {0u, 0u, 0u, 0u};
+#pragma unroll
+        for (int k = 0; k < 16; ++k) if (x + k < R.nx) w[k >> 2] |= (unsigned)__ldg(line + x + k) << (8 * (k & 3));
+        t = make_uint4(w[0], w[1], w[2], w[3]);
+      }
+      return t;
+    };
+    uint4 nxt = load16(16 * lane);
+    for (int x0 = 0; x0 < R.nx; x0 += 512) {
+      const int x = x0 + 16 * lane;
+      const uint4 cur = nxt;
+      if (x0 + 512 < R.nx) nxt = load16(x + 512);
+      const unsigned q[4] = {cur.x, cur.y, cur.z, cur.w};
       int cnt = 0;
-      int4 g[2];                                                // two neighbours cannot both define a grain: <= 2 per 4
 #pragma unroll
-      for (int k = 0; k < 4; ++k) {
-        const int c = (int)((q >> (8 * k)) & 0xffu);
-        if (c > R.thr) {
-          int4 r;
-          if (grain_of(v, R, x + k, y, z, c, r)) { if (cnt < 2) g[cnt] = r; ++cnt; }
-        }
-      }
-      const unsigned any = __ballot_sync(EMU_FULL, cnt > 0);
-      if (!any) continue;
+      for (int k = 0; k < 16; ++k) cnt += (int)((q[k >> 2] >> (8 * (k & 3))) & 0xffu) > R.thr;
+      if (!__ballot_sync(EMU_FULL, cnt > 0)) continue;
       int incl = cnt;                                           // x order: lanes in order, voxels of a lane in order
 #pragma unroll
       for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(EMU_FULL, incl, o); if (lane >= o) incl += t; }
-      if (kFill) {
-        const long long at = (long long)base + n_row + incl - cnt;
-        for (int k = 0; k < cnt && k < 2; ++k) {
-          if (at + k < capacity) grains[at + k] = g[k];
-          else if (status) atomicOr(status, (unsigned long long)EMU_ST_GRAIN_OVERFLOW);
-        }
+      int at = head + qn + incl - cnt;
+      if (cnt) {
+#pragma unroll
+        for (int k = 0; k < 16; ++k)
+          if ((int)((q[k >> 2] >> (8 * (k & 3))) & 0xffu) > R.thr) { ring[at & (kRing - 1)] = (unsigned short)(x + k); ++at; }
       }
-      n_row += __shfl_sync(EMU_FULL, incl, 31);
+      qn += __shfl_sync(EMU_FULL, incl, 31);
+      while (qn >= 32) flush(32);
     }
+    while (qn > 0) flush(min(qn, 32));
     if (!kFill && lane == 0) row_cnt[row] = n_row;
   }
 }
