@@ -58,8 +58,11 @@ constexpr int kRecogThreads = 256;
 // or two lanes of every 128 voxels.
 constexpr int kRing = 1024;                                     // >= 31 waiting + 512 new
 
+#ifndef EMU_RECOG_MINB
+#define EMU_RECOG_MINB 4
+#endif
 template <int kFill>
-__global__ void __launch_bounds__(kRecogThreads, 4)
+__global__ void __launch_bounds__(kRecogThreads, EMU_RECOG_MINB)
 k_recog(Recog R, const unsigned char* __restrict__ vox, int n_views, int* __restrict__ row_cnt,
         const int* __restrict__ row_off, int4* __restrict__ grains, long long capacity,
         unsigned long long* __restrict__ status) {
