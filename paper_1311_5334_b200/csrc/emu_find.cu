@@ -49,6 +49,9 @@ constexpr int kMaxTube = 8191;                    // n_tube field of the packed 
 #ifndef EMU_ITEMS_PER_SM
 #define EMU_ITEMS_PER_SM 12
 #endif
+#ifndef EMU_BODY_REPS
+#define EMU_BODY_REPS 2
+#endif
 #ifndef EMU_REFILL
 #define EMU_REFILL 10
 #endif
@@ -822,6 +825,8 @@ k_brick(EmuDev P, FramePtrs F, int v0, const Brick* __restrict__ bricks, FindCtl
         break;                                              // the slice is exhausted and every lane is done
       }
 
+#pragma unroll
+      for (int body = 0; body < EMU_BODY_REPS; ++body) {    // advance + test rounds between two looks at the idle lanes
       // ---------------- ADVANCE: lanes whose run is used up move to the next row of cells; a lane whose layer has no
       //                  row left takes the next w layer in the same breath.  ONE instruction sequence serves both
       //                  cases: the layer's u interval and row range are functions of the layer index and are simply
@@ -902,6 +907,7 @@ k_brick(EmuDev P, FramePtrs F, int v0, const Brick* __restrict__ bricks, FindCtl
           }
         }
       }
+      }   // body
     }
     n_tests += item_tests;
   }
