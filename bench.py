@@ -8,7 +8,9 @@ throughput batch of BASELINE.json configs[4]: 1,024 independent views of 350x300
 N > 1 is launched by torchrun, one rank per GPU; every rank processes its own V views (weak scaling, no
 data-path collective - the views are independent).  Rank 0 prints ONE JSON line.
 `--impl reference` times the CPU oracle (oracle/) on a bounded sample of the same workload instead.
-DESIGN.md section 8 states every formula used here.
+Optional extras (off by default, none changes the timed step): --latency-views (single views through the host
+call), --recognize-views (emu_recognize_grains on rendered voxel stacks), --tube-ext-um (the bounded tube of
+SURVEY 8(f) NEXT-1 instead of the contract's whole line).  DESIGN.md section 8 states every formula used here.
 """
 from __future__ import annotations
 

@@ -15,11 +15,15 @@
 //                     du > 0, + the two sorted positions (frame 0)
 //   k_plan            cut every (view, frame) into BRICKS (a tile of cell columns x a run of w layers) that
 //                     fit shared memory
-//   k_brick<VOTE>     persistent blocks: stage one brick's grains + cell table in shared memory, stream
+//   k_brick<kVote>    persistent blocks: stage one brick's grains + cell table in shared memory, stream
 //                     all seeds of the (view, frame) past it; every lane walks its own seed's tube through
-//                     the brick (uniform-grid ray traversal) and counts with the exact integer test (A3)
+//                     the brick (uniform-grid ray traversal), counts with the exact test (float with an exact
+//                     integer fallback inside its error band) and writes the grains it finds into the seed's
+//                     hit record (A3)
 //   k_cands<0/1>      n_tube >= min_grains -> candidate list grouped by (view, frame)            (A4)
-//   k_brick<ASSOC>    the candidates again: atomicMax of a packed priority into each member grain (A5)
+//   k_assoc_hits      the candidates' hit records: atomicMax of a packed priority into each member grain (A5)
+//   k_brick<kAssoc>   the same by a second walk, for the few candidates whose record overflowed
+//   (both k_brick kernels also exist with kBounded = true for the bounded tube, tube_ext_q >= 0)
 //   k_tie_detect, k_assoc_generic<1>   exact settlement of priority ties by (kmin, kmax)
 //   k_wins, k_select  members won per candidate, threshold again
 //   k_track_scan / k_track_emit / k_member_scan / k_member_scatter / k_member_sort: ordered output (A7)
