@@ -69,6 +69,7 @@ k_recog(Recog R, const unsigned char* __restrict__ vox, int n_views, int* __rest
   __shared__ unsigned short ring_s[kRecogThreads / 32][kRing];
   const int lane = threadIdx.x & 31;
   unsigned short* ring = ring_s[threadIdx.x >> 5];
+  const unsigned thr4 = (unsigned)R.thr * 0x01010101u;
   const long long rows_per_view = (long long)R.nz * R.ny, n_rows = rows_per_view * n_views;
   const long long warp0 = (long long)blockIdx.x * (kRecogThreads / 32) + (threadIdx.x >> 5);
   const long long n_warps = (long long)gridDim.x * (kRecogThreads / 32);
@@ -120,9 +121,11 @@ k_recog(Recog R, const unsigned char* __restrict__ vox, int n_views, int* __rest
       const uint4 cur = nxt;
       if (x0 + 512 < R.nx) nxt = load16(x + 512);
       const unsigned q[4] = {cur.x, cur.y, cur.z, cur.w};
+      // four voxels per SIMD byte compare: one mask bit per voxel above the threshold
+      unsigned mk[4];
       int cnt = 0;
 #pragma unroll
-      for (int k = 0; k < 16; ++k) cnt += (int)((q[k >> 2] >> (8 * (k & 3))) & 0xffu) > R.thr;
+      for (int w = 0; w < 4; ++w) { mk[w] = __vcmpgtu4(q[w], thr4) & 0x01010101u; cnt += __popc(mk[w]); }
       if (!__ballot_sync(EMU_FULL, cnt > 0)) continue;
       int incl = cnt;                                           // x order: lanes in order, voxels of a lane in order
 #pragma unroll
@@ -130,8 +133,11 @@ k_recog(Recog R, const unsigned char* __restrict__ vox, int n_views, int* __rest
       int at = head + qn + incl - cnt;
       if (cnt) {
 #pragma unroll
-        for (int k = 0; k < 16; ++k)
-          if ((int)((q[k >> 2] >> (8 * (k & 3))) & 0xffu) > R.thr) { ring[at & (kRing - 1)] = (unsigned short)(x + k); ++at; }
+        for (int w = 0; w < 4; ++w)
+          for (unsigned m = mk[w]; m; m &= m - 1u) {            // the set bits in ascending order = ascending x
+            ring[at & (kRing - 1)] = (unsigned short)(x + 4 * w + ((__ffs((int)m) - 1) >> 3));
+            ++at;
+          }
       }
       qn += __shfl_sync(EMU_FULL, incl, 31);
       while (qn >= 32) flush(32);
