@@ -29,19 +29,26 @@ __device__ __forceinline__ int vox_at(const unsigned char* __restrict__ v, const
 __device__ bool grain_of(const unsigned char* __restrict__ v, const Recog& R, int x, int y, int z, int c, int4& out) {
   long long sw = 0, sx = 0, sy = 0, sz = 0;
   bool ok = true;
+  // which neighbours exist (voxels outside the stack count as 0, R2): six comparisons for all 26
+  const bool in_lo[3] = {x > 0, y > 0, z > 0}, in_hi[3] = {x + 1 < R.nx, y + 1 < R.ny, z + 1 < R.nz};
+  const long long sy_ = R.nx, sz_ = (long long)R.nx * R.ny;
+  const unsigned char* p0 = v + ((size_t)z * R.ny + y) * R.nx + x;
 #pragma unroll
   for (int dz = -1; dz <= 1; ++dz)
 #pragma unroll
     for (int dy = -1; dy <= 1; ++dy)
 #pragma unroll
       for (int dx = -1; dx <= 1; ++dx) {
-        const int n = vox_at(v, R, x + dx, y + dy, z + dz);
+        const bool inside = (dx < 0 ? in_lo[0] : (dx > 0 ? in_hi[0] : true)) && (dy < 0 ? in_lo[1] : (dy > 0 ? in_hi[1] : true)) &&
+                            (dz < 0 ? in_lo[2] : (dz > 0 ? in_hi[2] : true));
+        const int n = inside ? (int)__ldg(p0 + (dz * sz_ + dy * sy_ + dx)) : 0;
         const bool before = dz < 0 || (dz == 0 && (dy < 0 || (dy == 0 && dx < 0)));     // raster order (z, y, x)
         if ((dz | dy | dx) != 0 && (n > c || (before && n == c))) ok = false;
         const int w = n > R.thr ? n : 0;                                               // R3
-        sw += w; sx += (long long)w * (x + dx); sy += (long long)w * (y + dy); sz += (long long)w * (z + dz);
+        sw += w; sx += (long long)(w * dx); sy += (long long)(w * dy); sz += (long long)(w * dz);
       }
   if (!ok) return false;
+  sx += sw * x; sy += sw * y; sz += sw * z;                     // sums of w * absolute index
   // R4: pos_q = floor(p (sum(w i) / sum(w) + 1/2) + 1/2), exact in integers (sw >= c > 0)
   out.x = (int)((2ll * R.pitch[0] * sx + (long long)R.pitch[0] * sw + sw) / (2ll * sw));
   out.y = (int)((2ll * R.pitch[1] * sy + (long long)R.pitch[1] * sw + sw) / (2ll * sw));
