@@ -64,7 +64,10 @@ constexpr int kMaxTube = 8191;                    // n_tube field of the packed 
 #endif
 constexpr int kBrickThreads = EMU_BRICK_THREADS;  // one persistent block per SM
 constexpr int kPoolBytes = 222 * 1024;            // dynamic shared memory of a brick: grains | row table | cell table
-constexpr int kGrab = 128;                        // seeds a warp takes from the block's stream at a time
+#ifndef EMU_GRAB
+#define EMU_GRAB 128
+#endif
+constexpr int kGrab = EMU_GRAB;                        // seeds a warp takes from the block's stream at a time
 constexpr int kTieBits = 1 << 16;                 // bitmap of tied priorities
 
 // shared-memory layout of a brick: n grains of 4 B, then one table row per row of cells: the brick slot
