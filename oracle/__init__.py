@@ -28,7 +28,7 @@ class _Params(C.Structure):
     _fields_ = [("struct_size", C.c_int32), ("view_size_q", C.c_int32 * 3), ("cell_size_q", C.c_int32 * 3),
                 ("sep_min_q", C.c_int32), ("sep_max_q", C.c_int32), ("tube_r2_q", C.c_int32),
                 ("tube_ext_q", C.c_int32), ("min_grains", C.c_int32), ("max_tracks_per_view", C.c_int32),
-                ("reserved", C.c_int32 * 4)]
+                ("reserved", C.c_int32 * 4), ("angle_min_grains", C.c_int32 * 8)]
 
 
 def build(force: bool = False) -> str:
@@ -70,6 +70,7 @@ def _params(p: dict) -> _Params:
     s.sep_min_q = p["sep_min_q"]; s.sep_max_q = p["sep_max_q"]; s.tube_r2_q = p["tube_r2_q"]
     s.tube_ext_q = p.get("tube_ext_q", -1); s.min_grains = p["min_grains"]
     s.max_tracks_per_view = p.get("max_tracks_per_view", 4096)
+    s.angle_min_grains[:] = [int(x) for x in p.get("angle_min_grains", (0,) * 8)]
     return s
 
 

@@ -20,6 +20,10 @@
 //                               that grain ... and again the threshold ... is applied"
 //   O6 fit        BASELINE.json north_star (not in the paper): least-squares line
 //   O7 order      SURVEY.md 8(c) O7: views ascending, tracks best-first
+//   O5b angle cut SURVEY.md 8(f) NEXT-2, PAPER.md:144 (Fig. 8(c)): "a cut on the number of grains is applied
+//                 according to the line drawn in the figure" - the line is not given numerically, so it is a table
+//                 parameter: minimum members per bin of |cos theta| of the FITTED direction, applied after O5
+//                 (reading Q17 in DESIGN.md).  All entries 0 (or <= min_grains): no effect.
 //
 // Two modes give the same result by construction (a test checks it):
 //   mode 0 "brute": no cells at all - every seed is tested against every grain.
@@ -55,6 +59,7 @@ typedef struct emo_params {      // same field order as the library's params str
   int32_t min_grains;
   int32_t max_tracks_per_view;
   int32_t reserved[4];
+  int32_t angle_min_grains[8];   // NEXT-2: minimum members per bin of |cos theta|; 0 = no cut in the bin
 } emo_params;
 
 typedef struct emo_track {       // 32 B
@@ -210,6 +215,45 @@ emo_fit fit_members(const std::vector<Grain>& G, const int32_t* mem, int32_t n) 
   return f;
 }
 
+// O5b - SURVEY 8(f) NEXT-2 / PAPER.md:144.  Bin of |cos theta| of the fitted line, theta = angle to the z axis
+// (the normal of the emulsion layer).  The fitted direction is (1, slope_v, slope_w) along (u, v, w), i.e. proportional
+// to the exact integers (den, num_v, num_w) of O6; cos^2 = c_z^2 / (den^2 + num_v^2 + num_w^2) with c_z the z component
+// (den for u = z, else num_w: z is the second minor axis of u = x and of u = y).  bin = largest k in 0..7 with
+// (k/8)^2 <= cos^2, decided exactly: k^2 S <= 64 c_z^2 in 128-bit integers (|den|, |num| <= 2^60: n < 2^13, |coord| <
+// 2^17, so S < 3 * 2^120 and 49 S < 2^128).  den = 0 (all members coincide): no direction, bin -1 = never cut.
+int angle_bin(const std::vector<Grain>& G, const int32_t* mem, int32_t n) {
+  i64 mn[3], mx[3];
+  for (int i = 0; i < n; ++i) {
+    const Grain& g = G[mem[i]];
+    i64 c[3] = {g.x, g.y, g.z};
+    for (int a = 0; a < 3; ++a) {
+      if (i == 0 || c[a] < mn[a]) mn[a] = c[a];
+      if (i == 0 || c[a] > mx[a]) mx[a] = c[a];
+    }
+  }
+  i64 ex = mx[0] - mn[0], ey = mx[1] - mn[1], ez = mx[2] - mn[2];
+  int u, v, w;
+  if (ez >= ex && ez >= ey) { u = 2; v = 0; w = 1; }
+  else if (ex >= ey)        { u = 0; v = 1; w = 2; }
+  else                      { u = 1; v = 0; w = 2; }
+  i64 Su = 0, Sv = 0, Sw = 0, Suu = 0, Suv = 0, Suw = 0;
+  for (int i = 0; i < n; ++i) {
+    const Grain& g = G[mem[i]];
+    i64 c[3] = {g.x, g.y, g.z};
+    Su += c[u]; Sv += c[v]; Sw += c[w];
+    Suu += c[u] * c[u]; Suv += c[u] * c[v]; Suw += c[u] * c[w];
+  }
+  const i64 N = n, den = N * Suu - Su * Su, nv = N * Suv - Su * Sv, nw = N * Suw - Su * Sw;
+  if (den == 0) return -1;
+  typedef unsigned __int128 u128;
+  auto sq = [](i64 a) { u128 m = (u128)(a < 0 ? -a : a); return m * m; };
+  const u128 S = sq(den) + sq(nv) + sq(nw);
+  const u128 cz2 = (u == 2) ? sq(den) : sq(nw);
+  int bin = 0;
+  for (int k = 1; k <= 7; ++k) if ((u128)(k * k) * S <= (u128)64 * cz2) bin = k;
+  return bin;
+}
+
 void track_view(const emo_params& P, const int32_t* grains, int32_t row0, int32_t n, int32_t view,
                 int mode, bool want_dump, ViewResult& R) {
   std::vector<Grain> G(n);
@@ -245,19 +289,27 @@ void track_view(const emo_params& P, const int32_t* grains, int32_t row0, int32_
     }
   }
 
-  std::vector<Cand> cands;
-  std::vector<int32_t> tube;        // flat in-tube lists of the candidates (local indices)
-  std::vector<int32_t> cur;
+  // what the pair loop produces; in the brute mode several threads each fill one of their own and the parts are
+  // joined afterwards (every later step is a max / count / sort over a total order, so the order of `cands` is
+  // immaterial - and the seed dump is compared as a set)
+  struct Part {
+    std::vector<Cand> cands;
+    std::vector<int32_t> tube;      // flat in-tube lists of the candidates (local indices)
+    std::vector<int32_t> cur;
+    std::vector<int32_t> seed_dump;
+    i64 seeds = 0, tests = 0, pairs = 0;
+  };
 
   // O3 for one seed (a < b local indices): fills `cur` with the grains in the tube.
-  auto count_seed = [&](int32_t a, int32_t b, i64 d2) {
+  auto count_seed = [&](Part& W, int32_t a, int32_t b, i64 d2) {
+    std::vector<int32_t>& cur = W.cur;
     const Grain& A = G[a];
     const i64 d[3] = {(i64)G[b].x - A.x, (i64)G[b].y - A.y, (i64)G[b].z - A.z};
     const i64 r2D2 = r2 * d2;
     cur.clear();
     if (mode == 0) {
       for (int32_t p = 0; p < n; ++p) {
-        R.cnt[1] += 1;
+        W.tests += 1;
         if (in_tube(A, d[0], d[1], d[2], r2D2, G[p], d2, P.tube_ext_q)) cur.push_back(p);
       }
       return;
@@ -299,7 +351,7 @@ void track_view(const emo_params& P, const int32_t* grains, int32_t row0, int32_
           // cells cx0..cx1 of one (cy,cz) row are consecutive, and so are their grains
           i64 c0 = rng[0][0] + grid.n[0] * (cy + grid.n[1] * cz), c1 = c0 + (rng[0][1] - rng[0][0]);
           for (int32_t j = cell_start[c0]; j < cell_start[c1 + 1]; ++j) {
-            R.cnt[1] += 1;
+            W.tests += 1;
             if (in_tube(A, d[0], d[1], d[2], r2D2, G[j], d2, P.tube_ext_q)) cur.push_back(j);
           }
         }
@@ -307,31 +359,58 @@ void track_view(const emo_params& P, const int32_t* grains, int32_t row0, int32_
   };
 
   // O2 + O3 + O4 for the unordered pair {i,j}, i < j.
-  auto try_pair = [&](int32_t i, int32_t j) {
-    R.cnt[6] += 1;
+  auto try_pair = [&](Part& W, int32_t i, int32_t j) {
+    W.pairs += 1;
     i64 dx = (i64)G[j].x - G[i].x, dy = (i64)G[j].y - G[i].y, dz = (i64)G[j].z - G[i].z;
     i64 d2 = dx * dx + dy * dy + dz * dz;
     if (d2 < smin2 || d2 >= smax2) return;                 // reading Q1: smin2 <= D2 < smax2
-    R.cnt[0] += 1;
-    count_seed(i, j, d2);
-    int32_t n_tube = (int32_t)cur.size();
+    W.seeds += 1;
+    count_seed(W, i, j, d2);
+    int32_t n_tube = (int32_t)W.cur.size();
     if (want_dump) {
-      R.seed_dump.push_back(view); R.seed_dump.push_back(std::min(G[i].row, G[j].row));
-      R.seed_dump.push_back(std::max(G[i].row, G[j].row)); R.seed_dump.push_back(n_tube);
+      W.seed_dump.push_back(view); W.seed_dump.push_back(std::min(G[i].row, G[j].row));
+      W.seed_dump.push_back(std::max(G[i].row, G[j].row)); W.seed_dump.push_back(n_tube);
     }
     if (n_tube < P.min_grains) return;                     // O4 (reading Q6: >=)
     Cand c; c.a = i; c.b = j; c.n_tube = n_tube; c.d2 = d2; c.n_members = 0;
     Key5 ka = key5(G[i]), kb = key5(G[j]);
     if (cmp5(ka, kb) <= 0) { c.kmin = ka; c.kmax = kb; } else { c.kmin = kb; c.kmax = ka; }
-    c.mem_off = tube.size();
-    tube.insert(tube.end(), cur.begin(), cur.end());
-    cands.push_back(c);
+    c.mem_off = W.tube.size();
+    W.tube.insert(W.tube.end(), W.cur.begin(), W.cur.end());
+    W.cands.push_back(c);
+  };
+
+  std::vector<Cand> cands;
+  std::vector<int32_t> tube;
+  auto join = [&](Part& W) {                               // append a part to the view's lists
+    for (Cand c : W.cands) { c.mem_off += tube.size(); cands.push_back(c); }
+    tube.insert(tube.end(), W.tube.begin(), W.tube.end());
+    R.seed_dump.insert(R.seed_dump.end(), W.seed_dump.begin(), W.seed_dump.end());
+    R.cnt[0] += W.seeds; R.cnt[1] += W.tests; R.cnt[6] += W.pairs;
   };
 
   if (mode == 0) {
-    for (int32_t i = 0; i < n; ++i)
-      for (int32_t j = i + 1; j < n; ++j) try_pair(i, j);
+    // every pair against every grain.  When this view is the only one in flight (emo_track_views runs a single view
+    // without an outer team) the rows of the pair loop are shared among the threads; each thread fills its own Part.
+    int nt = 1;
+#ifdef _OPENMP
+    nt = omp_in_parallel() ? 1 : omp_get_max_threads();
+#endif
+    std::vector<Part> parts(nt);
+#pragma omp parallel num_threads(nt) if (nt > 1)
+    {
+      int me = 0;
+#ifdef _OPENMP
+      me = omp_get_thread_num();
+#endif
+      Part& W = parts[me];
+#pragma omp for schedule(dynamic, 8)
+      for (int32_t i = 0; i < n; ++i)
+        for (int32_t j = i + 1; j < n; ++j) try_pair(W, i, j);
+    }
+    for (Part& W : parts) join(W);
   } else {
+    Part W;
     // PAPER.md:80 Fig. 4(a): "for each grain ... looping for grains within a given distance",
     // restricted to the cells that can hold them.  Cell index is monotone in
     // the coordinate (also under clamping), so |delta coord| < sep_max bounds the index range.
@@ -344,9 +423,10 @@ void track_view(const emo_params& P, const int32_t* grains, int32_t row0, int32_
           for (i64 cx = lo[0]; cx <= hi[0]; ++cx) {
             i64 cc = cx + grid.n[0] * (cy + grid.n[1] * cz);
             for (int32_t j = cell_start[cc]; j < cell_start[cc + 1]; ++j)
-              if (j > i) try_pair(i, j);                   // reading Q2: each unordered pair once
+              if (j > i) try_pair(W, i, j);                // reading Q2: each unordered pair once
           }
     }
+    join(W);
   }
   R.cnt[2] = (i64)cands.size();
 
@@ -363,6 +443,23 @@ void track_view(const emo_params& P, const int32_t* grains, int32_t row0, int32_
   std::vector<int32_t> trk;
   for (size_t ci = 0; ci < cands.size(); ++ci)
     if (cands[ci].n_members >= P.min_grains) trk.push_back((int32_t)ci);   // threshold again
+  // O5b (NEXT-2): angle-dependent cut on the number of grains; a track that fails it is dropped and its
+  // grains stay unassigned (as for the re-threshold, reading Q8).
+  {
+    bool any = false;
+    for (int k = 0; k < 8; ++k) any = any || P.angle_min_grains[k] > 0;
+    if (any) {
+      std::vector<int32_t> kept;
+      for (int32_t ci : trk) {
+        std::vector<int32_t> mem;
+        for (int32_t g = 0; g < n; ++g) if (owner[g] == ci) mem.push_back(g);
+        const int bin = angle_bin(G, mem.data(), (int32_t)mem.size());
+        if (bin >= 0 && cands[ci].n_members < P.angle_min_grains[bin]) continue;
+        kept.push_back(ci);
+      }
+      trk.swap(kept);
+    }
+  }
   // O7: best first.
   std::sort(trk.begin(), trk.end(), [&](int32_t x, int32_t y) { return better(cands[x], cands[y]); });
 
@@ -401,6 +498,7 @@ bool params_ok(const emo_params* p) {
   if (p->tube_r2_q < 0 || p->tube_r2_q >= (1 << 20)) return false;
   if (p->tube_ext_q < -1 || p->tube_ext_q > 65536) return false;   // -1 = whole line; >= 0 = bounded tube (NEXT-1)
   if (p->min_grains < 2) return false;
+  for (int k = 0; k < 8; ++k) if (p->angle_min_grains[k] < 0) return false;
   return true;
 }
 
@@ -439,9 +537,10 @@ void* emo_track_views(const emo_params* p, const int32_t* grains, const int32_t*
   if (!params_ok(p) || n_views < 0) return nullptr;
   std::vector<ViewResult> vr(n_views);
 #ifdef _OPENMP
-  if (n_threads > 0) omp_set_num_threads(n_threads);
+  omp_set_num_threads(n_threads > 0 ? n_threads : omp_get_num_procs());   // 0 = all cores (the setting persists between calls)
 #endif
-#pragma omp parallel for schedule(dynamic, 1)
+  // (a single view runs without an outer team, so that the brute mode can share its pair loop among the threads)
+#pragma omp parallel for schedule(dynamic, 1) if (n_views > 1)
   for (int32_t v = 0; v < n_views; ++v)
     track_view(*p, grains, view_off[v], view_off[v + 1] - view_off[v], v, mode, want_seed_dump != 0, vr[v]);
   Result* R = new Result();

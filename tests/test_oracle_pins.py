@@ -470,3 +470,133 @@ def test_bounded_tube_is_orientation_and_order_free(oracle_mod, config_oracle):
               cell_size_q=(p["cell_size_q"][1], p["cell_size_q"][0], p["cell_size_q"][2]))
     r2 = oracle_mod.track_views(ps, gs, b.view_off, "cells", 1)
     assert r2.tracks.tobytes() == r0.tracks.tobytes() and r2.members.tobytes() == r0.members.tobytes()
+
+
+# --------------------------------------------------------------------------- later keys of the order (golden)
+
+@pytest.fixture(scope="module")
+def tie_cases():
+    with open(os.path.join(HERE, "golden", "tie_break_keys.json")) as f:
+        return json.load(f)
+
+
+def _check_golden_tracks(res, tracks):
+    assert len(res.tracks) == len(tracks)
+    for t, g in zip(res.tracks, tracks):
+        for k in ("seed_a", "seed_b", "n_tube", "n_members", "seed_d2"):
+            assert int(t[k]) == g[k], (k, int(t[k]), g[k])
+        assert [int(x) for x in res.members[t["member_off"]:t["member_off"] + t["n_members"]]] == g["members"]
+
+
+@pytest.mark.parametrize("mode", ["brute", "cells"])
+@pytest.mark.parametrize("case", range(5))
+def test_tie_break_keys_golden(oracle_mod, tie_cases, case, mode):
+    """min(x,y), x, row of kmin and kmax decide: hand-derived winners, tests/golden."""
+    c = tie_cases["cases"][case]
+    g, off = _arr(c["grains"])
+    r = oracle_mod.track_views(tie_cases["params"], g, off, mode, 1)
+    assert r.counters["seeds"] == c["n_seeds"] and r.counters["candidates"] == c["n_candidates"]
+    _check_golden_tracks(r, c["tracks"])
+
+
+def test_tie_break_keys_mirror_images(oracle_mod, tie_cases):
+    """x <-> y swap of a whole view maps k onto itself except at the x component, so the 'x decides' and 'kmax
+    decides' cases must hand the shared grain to the OTHER line, and the others must not notice."""
+    p = tie_cases["params"]
+    for c in tie_cases["cases"]:
+        g, off = _arr(c["grains"])
+        gs = g.copy(); gs[:, 0], gs[:, 1] = g[:, 1].copy(), g[:, 0].copy()
+        r, rs = oracle_mod.track_views(p, g, off, "brute", 1), oracle_mod.track_views(p, gs, off, "brute", 1)
+        a, b = _track_list(r), _track_list(rs)
+        if c["name"] in ("x_decides", "kmax_decides"):
+            assert a != b and sorted(len(t[6]) for t in a) == sorted(len(t[6]) for t in b) == [8, 9]
+            assert set(a[0][6]) != set(b[0][6])                      # the 9-member track is the other line
+        else:
+            assert a == b
+
+
+@pytest.mark.parametrize("cfg", [1, 3])
+def test_cells_equal_brute_on_a_full_view(oracle_mod, config_oracle, cfg):
+    """Mode 'cells' (the reference of every GPU parity test and of the roofline's tests per seed) against mode
+    'brute' (every seed against every grain, no cells) on one full 350 x 300 x 50 um view: config 1 (1.5 M seeds x 23.6 k
+    grains = 3.5e10 integer tests) and config 3.  The brute pair loop is shared among the host cores."""
+    b, p, ref = config_oracle(cfg)
+    r = oracle_mod.track_views(p, b.grains, b.view_off, "brute", 0, seed_dump=True)
+    assert r.counters["seeds"] == ref.counters["seeds"] and r.counters["candidates"] == ref.counters["candidates"]
+    assert _same(r, ref)
+    a, c = r.seed_dump, ref.seed_dump
+    assert np.array_equal(a[np.lexsort((a[:, 2], a[:, 1], a[:, 0]))], c[np.lexsort((c[:, 2], c[:, 1], c[:, 0]))])
+
+
+# --------------------------------------------------------------------------- NEXT-2: angle-dependent cut
+
+@pytest.fixture(scope="module")
+def angle_golden():
+    with open(os.path.join(HERE, "golden", "angle_cut_tracks.json")) as f:
+        return json.load(f)
+
+
+@pytest.mark.parametrize("mode", ["brute", "cells"])
+def test_angle_cut_golden(oracle_mod, angle_golden, mode):
+    """PAPER.md:144 / Fig. 8(c): the hand-built view of tests/golden/angle_cut_tracks.json - a
+    horizontal 8-grain line the table removes, a steep one it keeps, two tracks just either side of a bin edge."""
+    G = angle_golden
+    g, off = _arr(G["grains"])
+    for case in G["cases"]:
+        p = dict(G["params"], angle_min_grains=case["angle_min_grains"])
+        r = oracle_mod.track_views(p, g, off, mode, 1)
+        assert r.counters["seeds"] == G["n_seeds"] and r.counters["candidates"] == G["n_candidates"]
+        _check_golden_tracks(r, [G["tracks"][name] for name in case["order"]])
+
+
+def _cos_bin_exact(points):
+    """bin of |cos theta| of the least-squares line, from the exact rational fit (cov/var form of exact_bruteforce)."""
+    f = fit_exact(points)
+    if f["degenerate"]:
+        return -1
+    u = f["axis"]
+    d = {u: Fraction(1)}
+    minor = {2: (0, 1), 0: (1, 2), 1: (0, 2)}[u]
+    d[minor[0]], d[minor[1]] = f["slope"]
+    cos2 = d[2] * d[2] / (d[0] * d[0] + d[1] * d[1] + d[2] * d[2])
+    return max(k for k in range(8) if Fraction(k * k, 64) <= cos2)
+
+
+def test_angle_cut_bins_against_exact_rationals(oracle_mod, config_oracle):
+    """On a generated view (config 0 and config 3: smeared tracks of every direction) the tracks a one-bin table
+    removes are exactly those whose exact-rational |cos theta| falls in that bin; the rest of the list, its order and
+    the grains of the removed tracks (left unassigned) do not change."""
+    for cfg in (0, 3):
+        b, p, ref = config_oracle(cfg)
+        xyz = b.grains[:, :3].astype(np.int64)
+        bins = []
+        for t in ref.tracks:
+            m = ref.members[t["member_off"]:t["member_off"] + t["n_members"]]
+            bins.append(_cos_bin_exact([tuple(int(v) for v in xyz[i]) for i in m]))
+        bins = np.asarray(bins)
+        assert len(set(bins.tolist())) >= 4
+        for k in range(8):
+            table = [0] * 8
+            table[k] = 8191
+            r = oracle_mod.track_views(dict(p, angle_min_grains=table), b.grains, b.view_off, "cells", 1)
+            keep = np.nonzero(bins != k)[0]
+            assert len(r.tracks) == len(keep)
+            assert _track_list(r) == [_track_list(ref)[i] for i in keep]
+        # a threshold between the member counts splits a bin
+        k = int(np.bincount(bins[bins >= 0]).argmax())
+        nm = np.sort(ref.tracks["n_members"][bins == k])
+        thr = int(nm[len(nm) // 2]) + 1
+        table = [0] * 8
+        table[k] = thr
+        r = oracle_mod.track_views(dict(p, angle_min_grains=table), b.grains, b.view_off, "cells", 1)
+        keep = np.nonzero((bins != k) | (ref.tracks["n_members"] >= thr))[0]
+        assert 0 < len(keep) < len(ref.tracks) and _track_list(r) == [_track_list(ref)[i] for i in keep]
+
+
+def test_angle_cut_all_equal_table_changes_nothing(oracle_mod, e1, config_oracle):
+    g, off = _arr(e1["grains"])
+    base = oracle_mod.track_views(e1["params"], g, off, "brute", 1)
+    for table in ([0] * 8, [8] * 8, [3] * 8):
+        assert _same(base, oracle_mod.track_views(dict(e1["params"], angle_min_grains=table), g, off, "brute", 1))
+    b, p, ref = config_oracle(2)
+    assert _same(ref, oracle_mod.track_views(dict(p, angle_min_grains=[p["min_grains"]] * 8), b.grains, b.view_off, "cells", 1))
