@@ -8,9 +8,9 @@ throughput batch of BASELINE.json configs[4]: 1,024 independent views of 350x300
 N > 1 is launched by torchrun, one rank per GPU; every rank processes its own V views (weak scaling, no
 data-path collective - the views are independent).  Rank 0 prints ONE JSON line.
 `--impl reference` times the CPU oracle (oracle/) on a bounded sample of the same workload instead.
-Optional extras (off by default, none changes the timed step): --latency-views (single views through the host
-call), --recognize-views (emu_recognize_grains on rendered voxel stacks), --tube-ext-um (the bounded tube of
-SURVEY 8(f) NEXT-1 instead of the contract's whole line).  DESIGN.md section 8 states every formula used here.
+Extras measured after the timed step (none changes it; 0 switches one off): --latency-views (single views through
+the host call, default 8), --recognize-views (emu_recognize_grains on rendered voxel stacks, default 4);
+--tube-ext-um runs the bounded tube of SURVEY 8(f) NEXT-1 instead of the contract's whole line.  DESIGN.md section 8 states every formula used here.
 """
 from __future__ import annotations
 
@@ -142,7 +142,31 @@ def oracle_sample(n_sample_views: int, threads: int):
     t0 = time.perf_counter()
     r = oracle.track_views(params_dict(), grains, off, "cells", threads)
     dt = time.perf_counter() - t0
-    return dt, int(off[-1]), r.counters
+    return dt, int(off[-1]), r.counters, r
+
+
+def first_views(out: dict, nv: int) -> dict:
+    """tracks / fits / members / track_off of views 0..nv-1 of a batch result (host arrays)."""
+    toff = np.asarray(out["track_off"])[:nv + 1].copy()
+    nt = int(toff[-1])
+    tr = np.asarray(out["tracks"])[:nt].copy()
+    nm = int(tr["member_off"][-1] + tr["n_members"][-1]) if nt else 0
+    return dict(track_off=toff, tracks=tr, fits=np.asarray(out["fits"])[:nt].copy(), members=np.asarray(out["members"])[:nm].copy())
+
+
+def same_as_oracle(got: dict, ref) -> bool:
+    """SURVEY 8(c) comparison rule: offsets, every track field and every member index bit-equal; fits: integer fields
+    equal, slopes / intercepts within 1e-5 relative (BASELINE.json north_star)."""
+    if not (np.array_equal(got["track_off"], ref.track_off) and got["tracks"].tobytes() == ref.tracks.tobytes()
+            and got["members"].tobytes() == ref.members.tobytes() and len(got["fits"]) == len(ref.fits)):
+        return False
+    f, r = got["fits"], ref.fits
+    for k in ("axis", "n", "u_min", "u_max"):
+        if not np.array_equal(f[k], r[k]):
+            return False
+    ok_s = np.abs(f["slope"] - r["slope"]) <= 1e-5 * np.maximum(np.abs(f["slope"]), np.abs(r["slope"])) + 1e-12
+    ok_i = np.abs(f["icpt"] - r["icpt"]) <= 1e-5 * np.maximum(np.abs(f["icpt"]), np.abs(r["icpt"])) + 1e-6
+    return bool(np.all(ok_s) and np.all(ok_i))
 
 
 def run_reference(args):
@@ -157,7 +181,7 @@ def run_reference(args):
     for _ in range(args.warmup if args.reference_warmup else 0):
         oracle_sample(nv, cores)
     for _ in range(max(1, min(args.steps, args.reference_steps))):
-        dt, ng, cnt = oracle_sample(nv, cores)
+        dt, ng, cnt, _ = oracle_sample(nv, cores)
         times.append(dt)
     t = float(np.mean(times))
     val = ng / t
@@ -199,10 +223,10 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cell-um", type=float, nargs=3, default=None, help="override the cell size of the 3D hash (um)")
-    ap.add_argument("--latency-views", type=int, default=0,
+    ap.add_argument("--latency-views", type=int, default=8,
                     help="also time single views one at a time through the host call (SURVEY 8(f) NEXT-3: the microscope "
                          "delivers one view every 0.2 s, P:102); adds the key single_view to the JSON line")
-    ap.add_argument("--recognize-views", type=int, default=0,
+    ap.add_argument("--recognize-views", type=int, default=4,
                     help="also time emu_recognize_grains (SURVEY 8(f) NEXT-4) on this many synthetic 1280 x 1024 x 40 voxel "
                          "stacks rendered from config-1 views; adds the key recognize to the JSON line")
     ap.add_argument("--tube-ext-um", type=float, default=None,
@@ -217,6 +241,12 @@ def main():
     if args.impl == "reference":
         run_reference(args)
         return
+
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # plain `python bench.py --gpus N`: start the N ranks ourselves (one process per GPU, rendezvous on 127.0.0.1)
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--standalone", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+               "--local-addr", "127.0.0.1", os.path.abspath(__file__)] + sys.argv[1:]
+        sys.exit(subprocess.call(cmd))
 
     import torch
     import torch.distributed as dist
@@ -275,9 +305,12 @@ def main():
     ms_total, (n_total,) = shard.reduce_step(ms_total, [n], device="cuda")    # max over ranks / sum over ranks
     ms_step = ms_total / args.steps
     counts = B.counts.cpu().numpy().copy()
+    cores = len(os.sched_getaffinity(0))
+    nv_s = args.sample_views if args.sample_views else max(1, min(cores, 16, V))      # views the oracle leg will check
+    dev_first = first_views(E.PathResult(B).host(), nv_s) if rank == 0 else None      # of the LAST timed step
 
     # end to end: ONE C-ABI call on pinned host buffers per step (H2D + path + D2H inside the call)
-    e2e = None
+    e2e, e2e_first = None, None
     if not args.no_e2e:
         del B                                               # one workspace at a time (each is sized for 180 GB of HBM)
         torch.cuda.empty_cache()
@@ -298,6 +331,7 @@ def main():
                "call": "emu_track_views_host (pinned host buffers; copies inside the timed call)"}
         assert int(H.h_counts[E.EMU_CNT["status"]]) == 0
         assert nt == int(counts[E.EMU_CNT["tracks"]]), "host path and device path disagree"
+        e2e_first = first_views(H.result(nt, nm), nv_s) if rank == 0 else None           # of the LAST timed call
         del H
 
     if rank != 0:
@@ -309,10 +343,16 @@ def main():
     seeds = int(counts[E.EMU_CNT["seeds"]])
     cpu = None
     alg = ALG_PER_SEED.get(tuple(CELL_UM))
+    parity = None
     if world == 1 and not args.no_cpu_baseline:
-        cores = len(os.sched_getaffinity(0))
-        nv_s = args.sample_views if args.sample_views else max(1, min(cores, 16, V))
-        dt, ng, cnt = oracle_sample(nv_s, cores)
+        dt, ng, cnt, ref = oracle_sample(nv_s, cores)
+        # parity of what was TIMED: views 0..nv_s-1 of the last timed device step and of the last timed host call
+        # against the oracle, element by element (SURVEY 8(c) comparison rule)
+        parity = {"views_checked": nv_s, "tracks_checked": int(len(ref.tracks)), "members_checked": int(len(ref.members)),
+                  "device_path": same_as_oracle(dev_first, ref),
+                  "e2e_host_call": same_as_oracle(e2e_first, ref) if e2e_first is not None else None,
+                  "rule": "track_off, tracks, members bit-equal; fits: integer fields equal, slope / icpt within 1e-5 relative"}
+        parity["identical"] = bool(parity["device_path"] and parity["e2e_host_call"] is not False)
         cpu = {"value": ng / dt, "unit": "grains/s", "cores": min(cores, nv_s), "kind": "oracle",
                "sample": f"views 0..{nv_s - 1} of the workload ({ng} grains), one OpenMP thread per view, oracle mode "
                          f"'cells' at cell {CELL_UM} um, {dt:.1f} s",
@@ -327,10 +367,14 @@ def main():
         alg_instr = seeds * (alg[0] * INSTR_PER_TEST + alg[1] * INSTR_PER_PAIR)   # per step, all vote launches
         achieved = alg_instr / (stage_ms["vote"] / args.steps * 1e-3) / 1e12
         views_per_launch = V * args.steps / stage_launches["vote"]
+        captured = tuple(CELL_UM) == (3.0, 4.0, 4.0) and TUBE_EXT_Q < 0     # the configuration of the committed ncu capture
+        gpu_tests = float(counts[E.EMU_CNT["tests"]]) / max(1, seeds)
         roofline = {"kernel": "k_brick<kVote> (A2 seeds are streamed in, A3 tube count + hit records, shared-memory bricks, "
                               "three frames)", "bound": "alu", "achieved": achieved, "peak": alu_peak,
                     "unit": "Tlane-instr/s", "frac": achieved / alu_peak,
-                    "traffic": VOTE_DRAM_BYTES_PER_VIEW * views_per_launch,
+                    "frac_on_kernel_tests": achieved / alu_peak * (gpu_tests * INSTR_PER_TEST + alg[1] * INSTR_PER_PAIR)
+                                            / (alg[0] * INSTR_PER_TEST + alg[1] * INSTR_PER_PAIR),
+                    "traffic": VOTE_DRAM_BYTES_PER_VIEW * views_per_launch if captured else None,
                     "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of profiles/r1e_k_brick_full.txt per view "
                                       "x views per launch",
                     "peak_source": f"148 SM x 4 schedulers x 32 lanes x {sm_max:.0f} MHz ({peaks['_source']} max SM clock)",
@@ -345,7 +389,7 @@ def main():
     bin_gbs = bin_bytes / (bin_ms * 1e-3) / 1e9 if bin_ms > 0 else 0.0
     roofline_bin = {"kernel": "emu_bin_grains: k_bin_split + k_bin_chunk (two passes: chunks of cells through a scratch array, then one chunk per block in shared memory)", "bound": "hbm",
                     "achieved": bin_gbs, "peak": hbm, "unit": "GB/s", "frac": bin_gbs / hbm,
-                    "traffic": BIN_DRAM_BYTES_PER_GRAIN * n, "traffic_source": "profiles/r1e_k_bin_full.txt, both passes, per grain x grains",
+                    "traffic": BIN_DRAM_BYTES_PER_GRAIN * n if tuple(CELL_UM) == (3.0, 4.0, 4.0) else None, "traffic_source": "profiles/r1e_k_bin_full.txt, both passes, per grain x grains",
                     "algorithmic_bytes": bin_bytes, "ms": bin_ms,
                     "algorithmic_bytes_per_grain": bin_bytes / max(1, n),
                     "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peaks['_source']})"}
@@ -431,11 +475,15 @@ def main():
         "gpu_launches": int(sum(stage_launches.values())),
         "stage_ms_per_step": {k: v / args.steps for k, v in stage_ms.items()},
         "roofline": roofline, "roofline_bin": roofline_bin, "cpu_baseline": cpu, "e2e": e2e, "clocks": clocks,
-        "single_view": single, "recognize": recog,
+        "single_view": single, "recognize": recog, "parity": parity,
+        "timing_note": "emu_profile is active inside the timed region: a pair of CUDA events around every launch of the "
+                       "library (the per-stage times and gpu_launches come from them); value is therefore conservative",
     }
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
+    if parity is not None and not parity["identical"]:
+        sys.exit("bench.py: the timed run is NOT identical to the oracle on the checked views: " + json.dumps(parity))
 
 
 if __name__ == "__main__":

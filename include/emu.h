@@ -55,6 +55,14 @@ typedef struct emu_params {
                                /* [0] = expected candidates per grain (0 = default 48; 48 B each),         */
                                /* [1] = expected seeds per grain (0 = default 192; 160 B each: geometry,   */
                                /*       counter and the hit record of the voting pass); [2], [3] must be 0 */
+  int32_t angle_min_grains[8]; /* angle-dependent cut on the number of grains (Fig. 8(c): "a cut on */
+                               /* the number of grains is applied according to the line drawn in the       */
+                               /* figure"; the line is not given, hence a table - reading Q17): entry k    */
+                               /* is the minimum n_members of a track whose FITTED direction has           */
+                               /* floor(8 |cos theta|) = k (7 for |cos theta| = 1), theta = angle to z,    */
+                               /* decided exactly in integers from the moments of emu_fit.  Applied after  */
+                               /* the exclusive association; a track that fails is dropped and its grains  */
+                               /* stay unassigned.  0 (or <= min_grains) = no cut in that bin; each 0..8191 */
 } emu_params;
 
 typedef struct emu_track {     /* 32 B */
@@ -107,7 +115,8 @@ int64_t emu_grid_cells(const emu_params* params, int32_t dims_out[3]);
  *       cell = cx + nx*(cy + ny*cz), c = clamp(floor(coord/cell_size), 0, n-1) (out-of-box grains are
  *       legal and land in the boundary cells, reading Q13);
  *       d_cell_start int32[n_views*n_cells+1]: first position in d_sorted of every (view, cell).
- *  d_status: int64[1], OR-ed with EMU_ST_COORD if a coordinate is out of range (may be d_counts+5).
+ *  d_status: int64[1], OR-ed with EMU_ST_COORD if a coordinate is out of range; never cleared here.  (Not
+ *       d_counts + EMU_CNT_STATUS: emu_find_tracks zeroes all of d_counts when it starts.)
  *  d_ws / ws_bytes: scratch of at least the size emu_workspace_bytes reports. */
 int emu_bin_grains(const emu_params* params, const int32_t* d_grains, const int32_t* d_view_off,
                    int64_t n_grains, int32_t n_views, int32_t* d_sorted, int32_t* d_cell_start,
@@ -138,7 +147,9 @@ int emu_count_seeds(const emu_params* params, const int32_t* d_sorted, const int
 /* A6 least-squares line per track (BASELINE.json north_star; reading Q9; not in the paper).
  *  in : d_grains in ORIGINAL order (members are rows of it); tracks / offsets / members from
  *       emu_find_tracks.  n_tracks is read on the device from d_track_off[n_views].
- *  out: d_fits emu_fit[same capacity as d_tracks], entry t for track t. */
+ *  out: d_fits emu_fit[same capacity as d_tracks], entry t for track t.
+ *  Safe after a device-side overflow of emu_find_tracks (status != 0): the tracks of a chunk that overflowed are
+ *  not emitted, and a track whose members did not fit members_capacity carries n_members = 0. */
 int emu_fit_tracks(const emu_params* params, const int32_t* d_grains, const emu_track* d_tracks,
                    const int32_t* d_track_off, const int32_t* d_members, int32_t n_views,
                    emu_fit* d_fits, void* stream);
@@ -181,6 +192,30 @@ int emu_track_views_host(const emu_params* params, const int32_t* h_grains, cons
                          int64_t members_capacity, int64_t* h_counts, void* d_arena, size_t arena_bytes,
                          void* stream);
 
+/* ---- streaming: batches of views through one GPU, copies overlapped with the kernels -------
+ * The microscope delivers a view every 0.2 s and the paper's run spends 0.04 of 0.14 s per view on I/O
+ * (P:136).  An emu_stream is a host-side object that owns three CUDA streams (copy-in, compute, copy-out), a few
+ * events and a small pinned staging buffer; the device memory is the CALLER's: one arena of emu_stream_arena_bytes()
+ * from which it carves TWO slots of inputs and outputs and ONE set of work buffers (the kernels of successive batches
+ * run one after the other on the compute stream, so they can share the workspace).
+ *   submit(k)   host->device copy of batch k on the copy-in stream, A1..A7 on the compute stream behind batch k-1;
+ *               returns at once.  At most two batches may be in flight; a third submit returns EMU_ERR_CAPACITY.
+ *               h_grains / h_view_off (HOST, pinned for a truly asynchronous copy) must stay untouched until collect.
+ *   collect()   waits for the OLDEST batch in flight, copies the valid part of its outputs to the host arrays on the
+ *               copy-out stream (while the next batch computes) and returns when they have arrived.  Outputs and
+ *               return codes as emu_track_views_host.
+ * With submit(k+1) called before collect(k), the input copy of k+1 and the output copy of k-1 hide behind the
+ * kernels of k.  Every batch must satisfy n_grains <= max_grains, n_views <= max_views. */
+typedef struct emu_stream emu_stream;
+int emu_stream_arena_bytes(const emu_params* params, int64_t max_grains, int32_t max_views, size_t* arena_bytes);
+emu_stream* emu_stream_create(const emu_params* params, int64_t max_grains, int32_t max_views, void* d_arena,
+                              size_t arena_bytes);                   /* NULL on failure */
+void emu_stream_destroy(emu_stream* s);                              /* s may be NULL; drains the streams first */
+int emu_stream_submit(emu_stream* s, const int32_t* h_grains, const int32_t* h_view_off, int64_t n_grains,
+                      int32_t n_views);
+int emu_stream_collect(emu_stream* s, emu_track* h_tracks, emu_fit* h_fits, int64_t tracks_capacity,
+                       int32_t* h_track_off, int32_t* h_members, int64_t members_capacity, int64_t* h_counts);
+
 /* ---- optional per-stage timing (measurement aid for bench.py) -------------
  * An emu_profile is a host-side object that owns CUDA events.  Between emu_profile_begin(p) and
  * emu_profile_end() every kernel the library launches FROM THE CALLING HOST THREAD is bracketed by
@@ -202,6 +237,8 @@ int emu_track_views_host(const emu_params* params, const int32_t* h_grains, cons
 #define EMU_STAGE_SEEDS 10       /* A2: seed pairs (count, offsets, fill)                           */
 #define EMU_STAGE_CANDS 11       /* A4: threshold -> candidate list                                 */
 #define EMU_STAGE_RECOG 12       /* A0: grain recognition (emu_recognize_grains)                    */
+#define EMU_STAGE_GENERIC 13     /* global-memory fallback of A2..A4 for chunks the bricks cannot hold
+                                    (launched for every chunk; returns at once when the bricks did the work) */
 #define EMU_STAGE_COUNT 16
 typedef struct emu_profile emu_profile;
 emu_profile* emu_profile_create(void);              /* NULL on failure                              */

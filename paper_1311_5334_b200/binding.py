@@ -33,14 +33,15 @@ class emu_params(C.Structure):
     _fields_ = [("struct_size", C.c_int32), ("view_size_q", C.c_int32 * 3), ("cell_size_q", C.c_int32 * 3),
                 ("sep_min_q", C.c_int32), ("sep_max_q", C.c_int32), ("tube_r2_q", C.c_int32),
                 ("tube_ext_q", C.c_int32), ("min_grains", C.c_int32), ("max_tracks_per_view", C.c_int32),
-                ("reserved", C.c_int32 * 4)]
+                ("reserved", C.c_int32 * 4), ("angle_min_grains", C.c_int32 * 8)]
 
 
 _SYMBOLS = ["emu_workspace_bytes", "emu_grid_cells", "emu_bin_grains", "emu_find_tracks", "emu_count_seeds",
             "emu_fit_tracks", "emu_host_arena_bytes", "emu_track_views_host", "emu_profile_create", "emu_profile_destroy", "emu_profile_begin", "emu_profile_end",
-            "emu_profile_read", "emu_recognize_ws_bytes", "emu_recognize_grains"]
+            "emu_profile_read", "emu_recognize_ws_bytes", "emu_recognize_grains", "emu_stream_arena_bytes", "emu_stream_create",
+            "emu_stream_destroy", "emu_stream_submit", "emu_stream_collect"]
 EMU_STAGE = dict(bin_count=0, bin_scan=1, bin_scatter=2, bin_place=3, prep=4, vote=5, assoc=6, select=7, emit=8, fit=9,
-                 seeds=10, cands=11, recog=12)
+                 seeds=10, cands=11, recog=12, generic=13)
 EMU_STAGE_COUNT = 16
 _lib = None
 
@@ -77,6 +78,16 @@ def _load():
         L.emu_recognize_ws_bytes.argtypes = [i32, i32, i32]
         L.emu_recognize_grains.restype = C.c_int
         L.emu_recognize_grains.argtypes = [vp, i32, i32, i32, i32, i32, C.POINTER(i32 * 3), vp, i64, vp, vp, vp, vp, sz, vp]
+        L.emu_stream_arena_bytes.restype = C.c_int
+        L.emu_stream_arena_bytes.argtypes = [vp, i64, i32, C.POINTER(sz)]
+        L.emu_stream_create.restype = vp
+        L.emu_stream_create.argtypes = [vp, i64, i32, vp, sz]
+        L.emu_stream_destroy.restype = None
+        L.emu_stream_destroy.argtypes = [vp]
+        L.emu_stream_submit.restype = C.c_int
+        L.emu_stream_submit.argtypes = [vp, vp, vp, i64, i32]
+        L.emu_stream_collect.restype = C.c_int
+        L.emu_stream_collect.argtypes = [vp, vp, vp, i64, vp, vp, i64, vp]
         L.emu_profile_create.restype = vp
         L.emu_profile_create.argtypes = []
         L.emu_profile_destroy.restype = None
@@ -100,7 +111,8 @@ def exported_symbols() -> list:
 
 
 def make_params(view_size_q, cell_size_q, sep_min_q, sep_max_q, tube_r2_q, min_grains,
-                max_tracks_per_view=4096, tube_ext_q=-1, cand_per_grain=0, seeds_per_grain=0) -> emu_params:
+                max_tracks_per_view=4096, tube_ext_q=-1, cand_per_grain=0, seeds_per_grain=0,
+                angle_min_grains=None) -> emu_params:
     p = emu_params()
     p.struct_size = C.sizeof(emu_params)
     p.view_size_q[:] = [int(x) for x in view_size_q]
@@ -109,6 +121,8 @@ def make_params(view_size_q, cell_size_q, sep_min_q, sep_max_q, tube_r2_q, min_g
     p.tube_ext_q, p.min_grains, p.max_tracks_per_view = int(tube_ext_q), int(min_grains), int(max_tracks_per_view)
     p.reserved[0] = int(cand_per_grain)
     p.reserved[1] = int(seeds_per_grain)
+    if angle_min_grains is not None:
+        p.angle_min_grains[:] = [int(x) for x in angle_min_grains]
     return p
 
 
@@ -256,10 +270,85 @@ class HostPath:
             self.h_grains[:self.n_grains].copy_(torch.from_numpy(np.ascontiguousarray(grains, np.int32).reshape(-1, 4)))
         self.h_view_off.copy_(torch.from_numpy(np.ascontiguousarray(view_off, np.int32)))
         nt, nm = self.call()
+        return self.result(nt, nm)
+
+    def result(self, nt: int, nm: int) -> dict:
+        """copies of the pinned outputs of the last call()"""
         return dict(tracks=self.h_tracks[:nt].numpy().view(TRACK_DTYPE).reshape(-1).copy(),
                     fits=self.h_fits[:nt * FIT_DTYPE.itemsize].numpy().view(FIT_DTYPE).reshape(-1).copy(),
                     members=self.h_members[:nm].numpy().copy(), track_off=self.h_track_off.numpy().copy(),
                     counts=self.h_counts.numpy().copy())
+
+
+class StreamPath:
+    """emu_stream_* of include/emu.h with its buffers: batches of views through one GPU, the host->device copy of the
+    next batch and the device->host copy of the previous one hidden behind the kernels of the current one.  Two pinned
+    input buffers (a submitted batch must stay untouched until it is collected), one set of pinned outputs, one device
+    arena.  submit() / collect() marshal only."""
+
+    def __init__(self, params: emu_params, max_grains: int, max_views: int):
+        import torch
+        self.params, self.max_grains, self.max_views = params, max_grains, max_views
+        b = C.c_size_t(0)
+        _check(_load().emu_stream_arena_bytes(C.byref(params), max_grains, max_views, C.byref(b)), "emu_stream_arena_bytes")
+        self.arena = torch.empty(int(b.value), dtype=torch.uint8, device="cuda")
+        self._h = _load().emu_stream_create(C.byref(params), max_grains, max_views, _ptr(self.arena), _nbytes(self.arena))
+        if not self._h:
+            raise EmuError("emu_stream_create failed")
+        tcap = max(max_views, 1) * params.max_tracks_per_view
+        self.tcap = tcap
+
+        def pin(shape, dt):
+            return torch.empty(shape, dtype=dt, pin_memory=True)
+        self.h_in = [(pin((max(max_grains, 1), 4), torch.int32), pin(max_views + 1, torch.int32)) for _ in range(2)]
+        self.h_tracks = pin((max(tcap, 1), 8), torch.int32)
+        self.h_fits = pin(max(tcap, 1) * FIT_DTYPE.itemsize, torch.uint8)
+        self.h_track_off = pin(max_views + 1, torch.int32)
+        self.h_members = pin(max(max_grains, 1), torch.int32)
+        self.h_counts = pin(8, torch.int64)
+        self._k = 0
+        self._shapes = []
+
+    def submit(self, grains: np.ndarray, view_off: np.ndarray) -> int:
+        import torch
+        hg, ho = self.h_in[self._k & 1]
+        n, nv = len(grains), len(view_off) - 1
+        if n:
+            hg[:n].copy_(torch.from_numpy(np.ascontiguousarray(grains, np.int32).reshape(-1, 4)))
+        ho[:nv + 1].copy_(torch.from_numpy(np.ascontiguousarray(view_off, np.int32)))
+        rc = _load().emu_stream_submit(self._h, C.c_void_p(hg.data_ptr()), C.c_void_p(ho.data_ptr()), n, nv)
+        if rc < 0:
+            _check(rc, "emu_stream_submit")
+        self._k += 1
+        self._shapes.append((n, nv))
+        return rc
+
+    def collect(self, copy: bool = True) -> dict:
+        n, nv = self._shapes.pop(0)
+        rc = _load().emu_stream_collect(self._h, C.c_void_p(self.h_tracks.data_ptr()), C.c_void_p(self.h_fits.data_ptr()),
+                                        self.tcap, C.c_void_p(self.h_track_off.data_ptr()),
+                                        C.c_void_p(self.h_members.data_ptr()), self.h_members.numel(),
+                                        C.c_void_p(self.h_counts.data_ptr()))
+        _check(rc, "emu_stream_collect")
+        c = self.h_counts.numpy()
+        nt, nm = int(c[EMU_CNT["tracks"]]), int(c[EMU_CNT["members"]])
+        if not copy:
+            return dict(n_tracks=nt, n_members=nm, counts=c.copy())
+        return dict(tracks=self.h_tracks[:nt].numpy().view(TRACK_DTYPE).reshape(-1).copy(),
+                    fits=self.h_fits[:nt * FIT_DTYPE.itemsize].numpy().view(FIT_DTYPE).reshape(-1).copy(),
+                    members=self.h_members[:nm].numpy().copy(), track_off=self.h_track_off[:nv + 1].numpy().copy(),
+                    counts=c.copy())
+
+    def close(self):
+        if self._h:
+            _load().emu_stream_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
 
 
 class Profile:

@@ -20,6 +20,7 @@ bool params_ok(const emu_params* p) {
   if (p->min_grains < 2 || p->min_grains > 8191) return false;
   if (p->max_tracks_per_view < 1 || p->max_tracks_per_view > 65536) return false;
   if (p->reserved[0] < 0 || p->reserved[1] < 0 || p->reserved[2] || p->reserved[3]) return false;
+  for (int k = 0; k < 8; ++k) if (p->angle_min_grains[k] < 0 || p->angle_min_grains[k] > 8191) return false;
   return true;
 }
 
@@ -58,6 +59,11 @@ EmuDev make_dev(const emu_params* p) {
     if ((int64_t)d.fr[f].n[0] * d.cs[0] > 65536) d.packed_ok = 0;
   }
   d.ext = p->tube_ext_q;
+  d.angle_cut = 0;
+  for (int k = 0; k < 8; ++k) {
+    d.angle_min[k] = p->angle_min_grains[k];
+    if (d.angle_min[k] > p->min_grains) d.angle_cut = 1;
+  }
   d.min_grains = p->min_grains;
   d.max_tracks = p->max_tracks_per_view;
   return d;
@@ -75,6 +81,12 @@ int cand_per_grain(const emu_params* p) { return p->reserved[0] > 0 ? p->reserve
 int seeds_per_grain(const emu_params* p) { return p->reserved[1] > 0 ? p->reserved[1] : 192; }
 
 }  // namespace
+
+int emu_sm_count() {
+  int dev = 0, v = 0;
+  if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && v > 0) return v;
+  return 148;                                     // B200
+}
 
 // ---- per-stage timing ---------------------------------------------------------------------------
 struct emu_profile {
@@ -271,6 +283,142 @@ int emu_track_views_host(const emu_params* params, const int32_t* h_grains, cons
   if (nm > 0 && cudaMemcpyAsync(h_members, A.members, (size_t)nm * 4, cudaMemcpyDeviceToHost, st) != cudaSuccess) return EMU_ERR_CUDA;
   if (cudaStreamSynchronize(st) != cudaSuccess) return EMU_ERR_CUDA;
   return EMU_OK;
+}
+
+// ---- streaming (include/emu.h): two slots of inputs / outputs, one workspace, three streams ----------------------
+struct emu_stream {
+  emu_params params; EmuDev dev;
+  int64_t max_grains; int32_t max_views;
+  cudaStream_t s_in, s_run, s_out;
+  struct Slot {
+    int32_t *grains, *view_off, *track_off, *members; emu_track* tracks; emu_fit* fits; int64_t *counts, *status;
+    cudaEvent_t in_done, run_done;
+    int64_t n_grains; int32_t n_views;
+    int64_t* h_small;                      // pinned: counts[8], status
+  } slot[2];
+  int32_t *sorted, *cell_start; void* ws; size_t ws_bytes;
+  unsigned long long submitted, collected;
+};
+
+namespace {
+size_t stream_carve(const emu_params* p, const EmuDev& d, int64_t n, int32_t nv, char* base, emu_stream* S) {
+  size_t off = 0;
+  auto take = [&](size_t bytes) { char* r = base ? base + off : nullptr; off += emu_align256(bytes ? bytes : 1); return r; };
+  const size_t tcap = (size_t)(nv > 0 ? nv : 1) * (size_t)p->max_tracks_per_view;
+  for (int k = 0; k < 2; ++k) {
+    int32_t* g = (int32_t*)take((size_t)n * 16); int32_t* vo = (int32_t*)take(((size_t)nv + 1) * 4);
+    emu_track* t = (emu_track*)take(tcap * sizeof(emu_track)); emu_fit* f = (emu_fit*)take(tcap * sizeof(emu_fit));
+    int32_t* to = (int32_t*)take(((size_t)nv + 1) * 4); int32_t* m = (int32_t*)take((size_t)n * 4);
+    int64_t* c = (int64_t*)take(64); int64_t* st = (int64_t*)take(8);
+    if (S) { auto& L = S->slot[k]; L.grains = g; L.view_off = vo; L.tracks = t; L.fits = f; L.track_off = to; L.members = m; L.counts = c; L.status = st; }
+  }
+  int32_t* srt = (int32_t*)take((size_t)n * 16);
+  int32_t* cs = (int32_t*)take(((size_t)nv * d.ncell + 1) * 4);
+  const size_t b = emu_bin_ws_bytes(d, n, nv), f = emu_find_ws_recommended_bytes(d, n, nv, seeds_per_grain(p), cand_per_grain(p));
+  const size_t wsb = b > f ? b : f;
+  void* ws = take(wsb);
+  if (S) { S->sorted = srt; S->cell_start = cs; S->ws = ws; S->ws_bytes = wsb; }
+  return off + 256;
+}
+}  // namespace
+
+int emu_stream_arena_bytes(const emu_params* params, int64_t max_grains, int32_t max_views, size_t* arena_bytes) {
+  if (!params_ok(params) || !arena_bytes) return EMU_ERR_INVALID;
+  EmuDev d = make_dev(params);
+  if (!shape_ok(d, max_grains, max_views)) return EMU_ERR_INVALID;
+  *arena_bytes = stream_carve(params, d, max_grains, max_views, nullptr, nullptr);
+  return EMU_OK;
+}
+
+emu_stream* emu_stream_create(const emu_params* params, int64_t max_grains, int32_t max_views, void* d_arena, size_t arena_bytes) {
+  if (!params_ok(params) || !d_arena) return nullptr;
+  EmuDev d = make_dev(params);
+  if (!shape_ok(d, max_grains, max_views)) return nullptr;
+  if (arena_bytes < stream_carve(params, d, max_grains, max_views, nullptr, nullptr)) return nullptr;
+  emu_stream* S = new (std::nothrow) emu_stream();
+  if (!S) return nullptr;
+  S->params = *params; S->dev = d; S->max_grains = max_grains; S->max_views = max_views;
+  S->submitted = S->collected = 0;
+  S->s_in = S->s_run = S->s_out = nullptr;
+  for (int k = 0; k < 2; ++k) { S->slot[k].in_done = S->slot[k].run_done = nullptr; S->slot[k].h_small = nullptr; }
+  stream_carve(params, d, max_grains, max_views, (char*)emu_align_ptr(d_arena), S);
+  bool ok = cudaStreamCreateWithFlags(&S->s_in, cudaStreamNonBlocking) == cudaSuccess &&
+            cudaStreamCreateWithFlags(&S->s_run, cudaStreamNonBlocking) == cudaSuccess &&
+            cudaStreamCreateWithFlags(&S->s_out, cudaStreamNonBlocking) == cudaSuccess;
+  for (int k = 0; k < 2 && ok; ++k)
+    ok = cudaEventCreateWithFlags(&S->slot[k].in_done, cudaEventDisableTiming) == cudaSuccess &&
+         cudaEventCreateWithFlags(&S->slot[k].run_done, cudaEventDisableTiming) == cudaSuccess &&
+         cudaMallocHost((void**)&S->slot[k].h_small, 16 * sizeof(int64_t)) == cudaSuccess;
+  if (!ok) { emu_stream_destroy(S); return nullptr; }
+  return S;
+}
+
+void emu_stream_destroy(emu_stream* S) {
+  if (!S) return;
+  if (S->s_in) { cudaStreamSynchronize(S->s_in); cudaStreamDestroy(S->s_in); }
+  if (S->s_run) { cudaStreamSynchronize(S->s_run); cudaStreamDestroy(S->s_run); }
+  if (S->s_out) { cudaStreamSynchronize(S->s_out); cudaStreamDestroy(S->s_out); }
+  for (int k = 0; k < 2; ++k) {
+    if (S->slot[k].in_done) cudaEventDestroy(S->slot[k].in_done);
+    if (S->slot[k].run_done) cudaEventDestroy(S->slot[k].run_done);
+    if (S->slot[k].h_small) cudaFreeHost(S->slot[k].h_small);
+  }
+  delete S;
+}
+
+int emu_stream_submit(emu_stream* S, const int32_t* h_grains, const int32_t* h_view_off, int64_t n_grains, int32_t n_views) {
+  if (!S || !h_view_off || n_grains < 0 || n_views < 0 || (n_grains > 0 && !h_grains)) return EMU_ERR_INVALID;
+  if (n_grains > S->max_grains || n_views > S->max_views) return EMU_ERR_INVALID;
+  if (S->submitted - S->collected >= 2) return EMU_ERR_CAPACITY;            // both slots are in flight
+  auto& L = S->slot[S->submitted & 1];
+  const EmuDev& d = S->dev;
+  // the slot's buffers are free: its previous batch was collected (collect waits for the kernels and the output copy)
+  if (n_grains > 0 && cudaMemcpyAsync(L.grains, h_grains, (size_t)n_grains * 16, cudaMemcpyHostToDevice, S->s_in) != cudaSuccess) return EMU_ERR_CUDA;
+  if (cudaMemcpyAsync(L.view_off, h_view_off, ((size_t)n_views + 1) * 4, cudaMemcpyHostToDevice, S->s_in) != cudaSuccess) return EMU_ERR_CUDA;
+  if (cudaEventRecord(L.in_done, S->s_in) != cudaSuccess) return EMU_ERR_CUDA;
+  if (cudaStreamWaitEvent(S->s_run, L.in_done, 0) != cudaSuccess) return EMU_ERR_CUDA;
+  cudaStream_t st = S->s_run;
+  if (cudaMemsetAsync(L.status, 0, 8, st) != cudaSuccess) return EMU_ERR_CUDA;
+  int rc = emu_bin_launch(d, 0, L.grains, L.view_off, n_grains, n_views, S->sorted, S->cell_start, L.status, S->ws, S->ws_bytes, st);
+  if (rc != EMU_OK) return rc;
+  rc = emu_find_launch(d, seeds_per_grain(&S->params), cand_per_grain(&S->params), S->sorted, S->cell_start, L.view_off, n_grains, n_views,
+                       L.tracks, L.track_off, L.members, n_grains, L.counts, S->ws, S->ws_bytes, st);
+  if (rc != EMU_OK) return rc;
+  rc = emu_fit_launch(L.grains, L.tracks, L.track_off, L.members, n_views, L.fits, st);
+  if (rc != EMU_OK) return rc;
+  if (cudaMemcpyAsync(L.h_small, L.counts, 64, cudaMemcpyDeviceToHost, st) != cudaSuccess) return EMU_ERR_CUDA;
+  if (cudaMemcpyAsync(L.h_small + 8, L.status, 8, cudaMemcpyDeviceToHost, st) != cudaSuccess) return EMU_ERR_CUDA;
+  if (cudaEventRecord(L.run_done, st) != cudaSuccess) return EMU_ERR_CUDA;
+  L.n_grains = n_grains; L.n_views = n_views;
+  return (int)(S->submitted++ & 0x3fffffff);
+}
+
+int emu_stream_collect(emu_stream* S, emu_track* h_tracks, emu_fit* h_fits, int64_t tracks_capacity, int32_t* h_track_off,
+                       int32_t* h_members, int64_t members_capacity, int64_t* h_counts) {
+  if (!S || !h_track_off || !h_counts || tracks_capacity < 0 || members_capacity < 0) return EMU_ERR_INVALID;
+  if (S->collected == S->submitted) return EMU_ERR_INVALID;                 // nothing in flight
+  auto& L = S->slot[S->collected & 1];
+  S->collected++;                                                          // the slot is given back whatever happens
+  if (cudaEventSynchronize(L.run_done) != cudaSuccess) return EMU_ERR_CUDA;
+  for (int k = 0; k < 8; ++k) h_counts[k] = L.h_small[k];
+  h_counts[EMU_CNT_STATUS] |= L.h_small[8];
+  cudaStream_t so = S->s_out;
+  if (cudaMemcpyAsync(h_track_off, L.track_off, ((size_t)L.n_views + 1) * 4, cudaMemcpyDeviceToHost, so) != cudaSuccess) return EMU_ERR_CUDA;
+  const int64_t nt = h_counts[EMU_CNT_TRACKS], nm = h_counts[EMU_CNT_MEMBERS];
+  int rc = EMU_OK;
+  if (h_counts[EMU_CNT_STATUS] == 0) {
+    if (nt > tracks_capacity || nm > members_capacity) rc = EMU_ERR_CAPACITY;
+    else if ((nt > 0 && (!h_tracks || !h_fits)) || (nm > 0 && !h_members)) rc = EMU_ERR_INVALID;
+    else {
+      if (nt > 0) {
+        if (cudaMemcpyAsync(h_tracks, L.tracks, (size_t)nt * sizeof(emu_track), cudaMemcpyDeviceToHost, so) != cudaSuccess) rc = EMU_ERR_CUDA;
+        if (cudaMemcpyAsync(h_fits, L.fits, (size_t)nt * sizeof(emu_fit), cudaMemcpyDeviceToHost, so) != cudaSuccess) rc = EMU_ERR_CUDA;
+      }
+      if (nm > 0 && cudaMemcpyAsync(h_members, L.members, (size_t)nm * 4, cudaMemcpyDeviceToHost, so) != cudaSuccess) rc = EMU_ERR_CUDA;
+    }
+  }
+  if (cudaStreamSynchronize(so) != cudaSuccess) return EMU_ERR_CUDA;
+  return rc;
 }
 
 int emu_recognize_grains(const uint8_t* d_vox, int32_t n_views, int32_t nx, int32_t ny, int32_t nz, int32_t threshold,

@@ -553,7 +553,7 @@ int emu_bin_launch(const EmuDev& P, int frame, const int32_t* d_grains, const in
     if (cudaFuncSetAttribute(k_bin_chunk, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return EMU_ERR_CUDA;
     if (cudaMemsetAsync(redo, 0, ((size_t)n_views + 1) * sizeof(int), st) != cudaSuccess) return EMU_ERR_CUDA;
     if (cudaMemsetAsync(cur, 0, (size_t)n_views * S.K * sizeof(int), st) != cudaSuccess) return EMU_ERR_CUDA;
-    const int blocks = (int)emu_max64(1, emu_min64(n_views, 148 * 8));
+    const int blocks = (int)emu_max64(1, emu_min64(n_views, emu_sm_count() * 8));
     const int tile = kSplitThreads * kSplitPer;
     const int tiles = (int)emu_min64(65535, 2 * ((n_grains / n_views + tile - 1) / tile) + 2);   // per view; larger views are redone
     EMU_LAUNCH(frame == 0 ? EMU_STAGE_BIN_COUNT : EMU_STAGE_PREP, st, k_bin_split<<<dim3(tiles, n_views), kSplitThreads, 0, st>>>(
@@ -570,7 +570,7 @@ int emu_bin_launch(const EmuDev& P, int frame, const int32_t* d_grains, const in
     const size_t smem = (size_t)((ncell + 3) / 4) * 4;
     if (cudaFuncSetAttribute(k_bin_view<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return EMU_ERR_CUDA;
     if (cudaMemsetAsync(redo, 0, ((size_t)n_views + 1) * sizeof(int), st) != cudaSuccess) return EMU_ERR_CUDA;
-    const int blocks = (int)emu_max64(1, emu_min64(n_views, 148 * 8));
+    const int blocks = (int)emu_max64(1, emu_min64(n_views, emu_sm_count() * 8));
     EMU_LAUNCH(frame == 0 ? EMU_STAGE_BIN_SCATTER : EMU_STAGE_PREP, st, k_bin_view<true><<<blocks, kViewThreads, smem, st>>>(
         P, frame, (const int4*)d_grains, d_view_off, n_views, n, (int4*)d_sorted, d_cell_start, count, tmp, redo,
         (unsigned long long*)d_status));
@@ -580,11 +580,11 @@ int emu_bin_launch(const EmuDev& P, int frame, const int32_t* d_grains, const in
     return cudaGetLastError() == cudaSuccess ? EMU_OK : EMU_ERR_CUDA;
   }
   if (cudaMemsetAsync(count, 0, (size_t)n_views * ncell * sizeof(int), st) != cudaSuccess) return EMU_ERR_CUDA;
-  int blocks = (int)emu_min64((n_grains + kBinThreads - 1) / kBinThreads, 148 * 16);
+  int blocks = (int)emu_min64((n_grains + kBinThreads - 1) / kBinThreads, emu_sm_count() * 16);
   if (blocks < 1) blocks = 1;
   EMU_LAUNCH(EMU_STAGE_BIN_COUNT, st, k_bin_count<<<blocks, kBinThreads, 0, st>>>(P, frame, (const int4*)d_grains, d_view_off, n_views, n, count,
                                               (unsigned long long*)d_status));
-  EMU_LAUNCH(EMU_STAGE_BIN_SCAN, st, k_bin_scan<<<(int)emu_min64(n_views > 0 ? n_views : 1, 148 * 2), 1024, 0, st>>>(ncell, d_view_off, n_views, n, count, d_cell_start));
+  EMU_LAUNCH(EMU_STAGE_BIN_SCAN, st, k_bin_scan<<<(int)emu_min64(n_views > 0 ? n_views : 1, emu_sm_count() * 2), 1024, 0, st>>>(ncell, d_view_off, n_views, n, count, d_cell_start));
   EMU_LAUNCH(EMU_STAGE_BIN_SCATTER, st, k_bin_scatter<<<blocks, kBinThreads, 0, st>>>(P, frame, (const int4*)d_grains, d_view_off, n_views, n, count, d_cell_start, tmp));
   EMU_LAUNCH(EMU_STAGE_BIN_PLACE, st, k_bin_place<<<blocks, kBinThreads, 0, st>>>(P, frame, tmp, d_view_off, n_views, n, d_cell_start, (int4*)d_sorted));
   return cudaGetLastError() == cudaSuccess ? EMU_OK : EMU_ERR_CUDA;

@@ -11,8 +11,9 @@
 #define EMU_FULL 0xffffffffu
 
 // Frames.  The tube walk of emu_find.cu wants the line's dominant axis to be the axis the rows of cells
-// run along, so every view is binned three times, once per cyclic permutation of the axes:
-//   frame 0: (u,v,w) = (x,y,z)   frame 1: (u,v,w) = (y,z,x)   frame 2: (u,v,w) = (z,x,y)
+// run along, so every view is binned three times, once per choice of the first axis:
+//   frame 0: (u,v,w) = (x,y,z)   frame 1: (u,v,w) = (y,x,z)   frame 2: (u,v,w) = (z,x,y)
+// (w = z wherever possible: a view is flat, a line crosses few z layers, and w is the outer loop of the walk)
 // The cell size triple cs[] applies to (u,v,w) in every frame; frame 0 is the binning the C ABI defines.
 struct EmuFrame { int n[3]; int ncell; };
 
@@ -35,6 +36,8 @@ struct EmuDev {           // passed by value to every kernel
   float csf[3];           // cell size as float
   float Rup;              // ceil(sqrt(r2)) as float (error band of the float tube test)
   int packed_ok;          // 1: the 4-byte grain format of the brick kernels can hold a view of this grid
+  int angle_min[8];       // angle-dependent cut: minimum members per bin of |cos theta|, 0 = none
+  int angle_cut;          // 1: some entry of angle_min exceeds min_grains (the cut can remove a track)
 };
 
 // lab axis of coordinate i of frame f

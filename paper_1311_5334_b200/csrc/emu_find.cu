@@ -390,28 +390,28 @@ __global__ void __launch_bounds__(1024)
 k_chunk_offsets(int nv, const unsigned* __restrict__ tot, unsigned* __restrict__ off, unsigned* __restrict__ total_out,
                 unsigned cap, unsigned status_bit, FindCtl* __restrict__ ctl, unsigned long long* __restrict__ counts,
                 int count_slot) {
-  __shared__ unsigned warp_sum[32];
+  __shared__ unsigned long long warp_sum[32];
   __shared__ unsigned long long carry_s;
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   if (threadIdx.x == 0) carry_s = 0;
   __syncthreads();
   for (int b = 0; b < nv; b += blockDim.x) {
     const int v = b + threadIdx.x;
-    unsigned x = (v < nv) ? tot[v] : 0u;
-    unsigned incl = x;
+    const unsigned long long x = (v < nv) ? tot[v] : 0ull;
+    unsigned long long incl = x;                       // 64-bit throughout: 1 024 entries of up to 2^32 - 1 seeds
 #pragma unroll
-    for (int o = 1; o < 32; o <<= 1) { unsigned y = __shfl_up_sync(EMU_FULL, incl, o); if (lane >= o) incl += y; }
+    for (int o = 1; o < 32; o <<= 1) { unsigned long long y = __shfl_up_sync(EMU_FULL, incl, o); if (lane >= o) incl += y; }
     if (lane == 31) warp_sum[wid] = incl;
     __syncthreads();
     if (wid == 0) {
-      unsigned w = warp_sum[lane], wi = w;
+      unsigned long long w = warp_sum[lane], wi = w;
 #pragma unroll
-      for (int o = 1; o < 32; o <<= 1) { unsigned y = __shfl_up_sync(EMU_FULL, wi, o); if (lane >= o) wi += y; }
+      for (int o = 1; o < 32; o <<= 1) { unsigned long long y = __shfl_up_sync(EMU_FULL, wi, o); if (lane >= o) wi += y; }
       warp_sum[lane] = wi - w;
     }
     __syncthreads();
     const unsigned long long carry = carry_s;
-    const unsigned long long mine = carry + warp_sum[wid] + incl;   // (a 1024-view tile of the scan stays below 2^32 when it fits)
+    const unsigned long long mine = carry + warp_sum[wid] + incl;
     if (v < nv) off[v] = (unsigned)min(mine - x, 0xffffffffull);
     __syncthreads();
     if (threadIdx.x == blockDim.x - 1) carry_s = mine;
@@ -430,6 +430,15 @@ k_chunk_offsets(int nv, const unsigned* __restrict__ tot, unsigned* __restrict__
       *total_out = (unsigned)total;
     }
   }
+}
+
+// the 64-bit counters of the seeds this chunk has (the count is on the device)
+__global__ void __launch_bounds__(256)
+k_clear_seed_cnt(const FindCtl* __restrict__ ctl, unsigned long long* __restrict__ seed_cnt) {
+  const size_t n = ctl->seed_count;
+  ulonglong2* p2 = reinterpret_cast<ulonglong2*>(seed_cnt);
+  const size_t stride = (size_t)gridDim.x * blockDim.x;
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; 2 * i < n; i += stride) p2[i] = make_ulonglong2(0ull, 0ull);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -1270,16 +1279,138 @@ k_wins(const int* __restrict__ view_off, int v0, int v1, const FindCtl* __restri
 // A5 part 3: "again the threshold on number of grains is applied to all tracks"
 __global__ void __launch_bounds__(256)
 k_select(EmuDev P, const Cand* __restrict__ cands, const FindCtl* __restrict__ ctl, const int* __restrict__ wins,
-         int* __restrict__ view_ntracks, unsigned* __restrict__ view_tracks, unsigned long long* __restrict__ counts) {
+         int* __restrict__ view_ntracks, unsigned* __restrict__ view_tracks, unsigned* __restrict__ cand_slot,
+         unsigned long long* __restrict__ counts) {
   if (ctl->skip) return;
   const unsigned n = ctl->cand_count;
   for (unsigned ci = blockIdx.x * blockDim.x + threadIdx.x; ci < n; ci += gridDim.x * blockDim.x) {
     if (wins[ci] >= P.min_grains) {
       int vl = cands[ci].n_tube_view >> 16;
       int slot = atomicAdd(view_ntracks + vl, 1);
-      if (slot < P.max_tracks) view_tracks[(size_t)vl * P.max_tracks + slot] = ci;
-      else atomicOr(counts + EMU_CNT_STATUS, (unsigned long long)EMU_ST_TRACK_OVERFLOW);
+      if (slot < P.max_tracks) {
+        view_tracks[(size_t)vl * P.max_tracks + slot] = ci;
+        if (P.angle_cut) cand_slot[ci] = (unsigned)slot;           // for k_cut_acc (cand_track is free until k_track_emit)
+      } else {
+        atomicOr(counts + EMU_CNT_STATUS, (unsigned long long)EMU_ST_TRACK_OVERFLOW);
+      }
     }
+  }
+}
+
+// ---- A5b: angle-dependent cut on the number of grains (Fig. 8(c); emu.h angle_min_grains; reading Q17) ----
+// The members of the surviving candidates are not listed yet, so every grain adds itself to the moment sums of its
+// owner (slot = place of the owner in its view's track list): extents and the nine sums S(x), S(y), S(z), S(xx), ...,
+// from which the direction of the least-squares line of emu_fit follows exactly: it is proportional to the integers
+// (den, num_v, num_w) along (u, v, w).  bin = largest k with (k/8)^2 <= cos^2 = c_z^2 / (den^2 + num_v^2 + num_w^2),
+// decided in 128-bit integers (|den|, |num| <= 2^60: n < 2^13, |coord| < 2^17).  A track with fewer members than
+// angle_min[bin] leaves the list; its grains stay unassigned.
+struct CutAcc { int lo[3], hi[3]; long long s[9]; };   // 96 B: sums x, y, z, xx, yy, zz, xy, xz, yz
+
+__global__ void __launch_bounds__(256)
+k_cut_init(EmuDev P, int nv, const FindCtl* __restrict__ ctl, const int* __restrict__ view_ntracks, CutAcc* __restrict__ acc) {
+  if (ctl->skip) return;
+  const int vl = blockIdx.y;
+  if (vl >= nv) return;
+  const int nt = min(view_ntracks[vl], P.max_tracks);
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < nt; i += gridDim.x * blockDim.x) {
+    CutAcc a;
+    for (int k = 0; k < 3; ++k) { a.lo[k] = 0x7fffffff; a.hi[k] = (int)0x80000000; }
+    for (int k = 0; k < 9; ++k) a.s[k] = 0;
+    acc[(size_t)vl * P.max_tracks + i] = a;
+  }
+}
+
+__global__ void __launch_bounds__(256)
+k_cut_acc(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ view_off, int v0, int v1,
+          const FindCtl* __restrict__ ctl, const unsigned long long* __restrict__ keyA,
+          const unsigned long long* __restrict__ keyB, const unsigned* __restrict__ owner, const Cand* __restrict__ cands,
+          const unsigned* __restrict__ cand_slot, CutAcc* __restrict__ acc) {
+  if (ctl->skip) return;
+  const int g0 = __ldg(view_off + v0), g1 = __ldg(view_off + v1);
+  for (int j = g0 + blockIdx.x * blockDim.x + threadIdx.x; j < g1; j += gridDim.x * blockDim.x) {
+    const int4 g = __ldg(sorted + j);
+    const unsigned ci = owner_of(g.w, ctl, keyA, keyB, owner);
+    if (ci == kNone) continue;
+    const unsigned slot = cand_slot[ci];
+    if (slot == kNone) continue;
+    CutAcc* a = acc + ((size_t)(cands[ci].n_tube_view >> 16) * P.max_tracks + slot);
+    const int c[3] = {g.x, g.y, g.z};
+#pragma unroll
+    for (int k = 0; k < 3; ++k) { atomicMin(&a->lo[k], c[k]); atomicMax(&a->hi[k], c[k]); }
+    const long long x = g.x, y = g.y, z = g.z;
+    const long long v[9] = {x, y, z, x * x, y * y, z * z, x * y, x * z, y * z};
+#pragma unroll
+    for (int k = 0; k < 9; ++k) atomicAdd(reinterpret_cast<unsigned long long*>(&a->s[k]), (unsigned long long)v[k]);
+  }
+}
+
+__device__ __forceinline__ unsigned __int128 sq128(long long a) {
+  const unsigned __int128 m = (unsigned __int128)(unsigned long long)(a < 0 ? -a : a);
+  return m * m;
+}
+
+__global__ void __launch_bounds__(256)
+k_cut_decide(EmuDev P, int nv, const FindCtl* __restrict__ ctl, const int* __restrict__ view_ntracks,
+             unsigned* __restrict__ view_tracks, const int* __restrict__ wins, const CutAcc* __restrict__ acc,
+             unsigned* __restrict__ cand_slot) {
+  if (ctl->skip) return;
+  const int vl = blockIdx.y;
+  if (vl >= nv) return;
+  const int nt = min(view_ntracks[vl], P.max_tracks);
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < nt; i += gridDim.x * blockDim.x) {
+    const size_t at = (size_t)vl * P.max_tracks + i;
+    const unsigned ci = view_tracks[at];
+    cand_slot[ci] = kNone;                                     // back to "no track yet" for k_track_emit
+    const CutAcc a = acc[at];
+    const long long ex = (long long)a.hi[0] - a.lo[0], ey = (long long)a.hi[1] - a.lo[1], ez = (long long)a.hi[2] - a.lo[2];
+    // dominant axis by member extent, ties z, x, y (emu_fit); s: 0 x, 1 y, 2 z, 3 xx, 4 yy, 5 zz, 6 xy, 7 xz, 8 yz
+    long long Su, Sv, Sw, Suu, Suv, Suw;
+    bool u_is_z = false;
+    if (ez >= ex && ez >= ey) { u_is_z = true; Su = a.s[2]; Sv = a.s[0]; Sw = a.s[1]; Suu = a.s[5]; Suv = a.s[7]; Suw = a.s[8]; }
+    else if (ex >= ey)        { Su = a.s[0]; Sv = a.s[1]; Sw = a.s[2]; Suu = a.s[3]; Suv = a.s[6]; Suw = a.s[7]; }
+    else                      { Su = a.s[1]; Sv = a.s[0]; Sw = a.s[2]; Suu = a.s[4]; Suv = a.s[6]; Suw = a.s[8]; }
+    const long long N = wins[ci];
+    const long long den = N * Suu - Su * Su, nvv = N * Suv - Su * Sv, nww = N * Suw - Su * Sw;
+    if (den == 0) continue;                                    // all members coincide: no direction, never cut
+    const unsigned __int128 S = sq128(den) + sq128(nvv) + sq128(nww);
+    const unsigned __int128 cz2 = u_is_z ? sq128(den) : sq128(nww);
+    int bin = 0;
+#pragma unroll
+    for (int k = 1; k <= 7; ++k) if ((unsigned __int128)(k * k) * S <= (unsigned __int128)64 * cz2) bin = k;
+    if ((int)N < P.angle_min[bin]) view_tracks[at] = kNone;
+  }
+}
+
+// the per-view track lists without the tracks the cut removed (one block per view; in place: a tile is read, the
+// block synchronises, and its survivors land at or before the places just read)
+__global__ void __launch_bounds__(256)
+k_cut_compact(EmuDev P, int nv, const FindCtl* __restrict__ ctl, int* __restrict__ view_ntracks, unsigned* __restrict__ view_tracks) {
+  __shared__ int warp_sum[8];
+  __shared__ int base_s;
+  if (ctl->skip) return;
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  for (int vl = blockIdx.x; vl < nv; vl += gridDim.x) {
+    const int nt = min(view_ntracks[vl], P.max_tracks);
+    unsigned* list = view_tracks + (size_t)vl * P.max_tracks;
+    if (threadIdx.x == 0) base_s = 0;
+    __syncthreads();
+    for (int i0 = 0; i0 < nt; i0 += blockDim.x) {
+      const int i = i0 + threadIdx.x;
+      const unsigned ci = i < nt ? list[i] : kNone;
+      const bool keep = ci != kNone;
+      const unsigned m = __ballot_sync(EMU_FULL, keep);
+      if (lane == 0) warp_sum[wid] = __popc(m);
+      __syncthreads();
+      int before = 0, total = 0;
+      for (int w = 0; w < 8; ++w) { if (w < wid) before += warp_sum[w]; total += warp_sum[w]; }
+      const int base = base_s;
+      __syncthreads();
+      if (keep) list[base + before + __popc(m & ((1u << lane) - 1u))] = ci;
+      if (threadIdx.x == 0) base_s = base + total;
+      __syncthreads();
+    }
+    if (threadIdx.x == 0) view_ntracks[vl] = base_s;    // (<= max_tracks: k_track_scan's clamp changes nothing)
+    __syncthreads();
   }
 }
 
@@ -1372,9 +1503,14 @@ k_member_scan(int v0, int v1, const int* __restrict__ track_off, emu_track* __re
     long long carry = carry_s;
     if (t < t1) {
       long long off = carry + warp_sum[wid] + incl - x;
-      tracks[t].member_off = (int)off;
+      tracks[t].member_off = (int)min(off, (long long)0x7fffffff);
       cursor[t - t0] = 0;
-      if (off + x > members_capacity) atomicOr(counts + EMU_CNT_STATUS, (unsigned long long)EMU_ST_MEMBER_OVERFLOW);
+      if (off + x > members_capacity) {
+        // the list does not fit: the track carries no members (emu_fit_tracks then reads nothing); the total needed
+        // still goes to counts[EMU_CNT_MEMBERS]
+        atomicOr(counts + EMU_CNT_STATUS, (unsigned long long)EMU_ST_MEMBER_OVERFLOW);
+        tracks[t].n_members = 0; tracks[t].member_off = 0;
+      }
     }
     __syncthreads();
     if (threadIdx.x == blockDim.x - 1) carry_s = carry + warp_sum[wid] + incl;
@@ -1400,7 +1536,7 @@ k_member_scatter(const int4* __restrict__ sorted, const int* __restrict__ view_o
     unsigned ci = owner_of(g, ctl, keyA, keyB, owner);
     if (ci == kNone) continue;
     unsigned t = cand_track[ci];
-    if (t == kNone) continue;
+    if (t == kNone || tracks[t].n_members == 0) continue;     // (no members: the list did not fit, k_member_scan)
     int k = atomicAdd(cursor + (t - t0), 1);
     long long pos = (long long)tracks[t].member_off + k;
     if (pos < members_capacity) members[pos] = g;                // g is a row
@@ -1460,6 +1596,7 @@ struct FindWs {
   int* slot_row; int* vf_brick_base; unsigned* view_ovf_cnt; unsigned* view_ovf_off;
   int4* geo; int2* ab; unsigned long long* seed_cnt; unsigned short* recs;
   Cand* cands; unsigned* cand_seed; int4* ovf_geo; unsigned* ovf_ci; int* wins; unsigned* cand_track;
+  CutAcc* cut_acc;                                                                // only with the angle cut
   size_t seed_cap, cand_cap, brick_cap; int views_per_chunk;
 };
 
@@ -1486,6 +1623,7 @@ size_t fixed_bytes(const EmuDev& P, const Tilings& TT, int64_t n_grains, int32_t
   b += emu_align256(3 * (size_t)n_grains * sizeof(int));                    // slot_row: every grain once per frame
   b += emu_align256((size_t)vpc * sizeof(int));
   b += emu_align256((size_t)vpc * P.max_tracks * sizeof(unsigned));
+  if (P.angle_cut) b += emu_align256((size_t)vpc * P.max_tracks * sizeof(CutAcc));
   b += emu_align256((size_t)vpc * bricks_per_view(P, TT) * sizeof(Brick));
   for (int f = 1; f < 3; ++f) {                                             // the binnings of frames 1 and 2
     b += emu_align256((size_t)n_grains * sizeof(int4));
@@ -1575,6 +1713,8 @@ static int carve(const EmuDev& P, const Tilings& TT, Hints hints, int64_t n_grai
     // what is available is split between seeds and candidates in the proportion of the hints
     const double ws_seed = (double)spv * kSeedBytes, ws_cand = (double)cpv * kCandBytes;
     seed_cap = (size_t)((double)avail * ws_seed / (ws_seed + ws_cand) / kSeedBytes);
+    const size_t seed_max = (avail - kMinCandCap * kCandBytes) / kSeedBytes;     // leave the candidates their minimum
+    if (seed_cap > seed_max) seed_cap = seed_max;
     if (seed_cap < kMinSeedCap) seed_cap = kMinSeedCap;
     cand_cap = (avail - seed_cap * kSeedBytes) / kCandBytes;
     return cand_cap >= kMinCandCap && ((int64_t)seed_cap >= spv * vpc || relaxed);
@@ -1609,6 +1749,7 @@ static int carve(const EmuDev& P, const Tilings& TT, Hints hints, int64_t n_grai
   W.slot_row = (int*)take(3 * (size_t)n_grains * sizeof(int));
   W.view_ntracks = (int*)take((size_t)vpc * sizeof(int));
   W.view_tracks = (unsigned*)take((size_t)vpc * P.max_tracks * sizeof(unsigned));
+  W.cut_acc = P.angle_cut ? (CutAcc*)take((size_t)vpc * P.max_tracks * sizeof(CutAcc)) : nullptr;
   W.brick_cap = (size_t)vpc * bricks_per_view(P, TT);
   W.bricks = (Brick*)take(W.brick_cap * sizeof(Brick));
   W.sortedF[0] = nullptr; W.cell_startF[0] = nullptr;
@@ -1638,11 +1779,6 @@ static int grid_for(int64_t n, int threads, int max_blocks) {
   return (int)emu_min64(b, max_blocks);
 }
 
-static int sm_count() {
-  int dev = 0, v = 0;
-  if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && v > 0) return v;
-  return 148;
-}
 
 #define EMU_CK(x) do { if ((x) != cudaSuccess) return EMU_ERR_CUDA; } while (0)
 
@@ -1693,9 +1829,8 @@ static int vote_chunk(const EmuDev& P, const Tilings& TT, FindWs& W, const Frame
       W.ctl, counts, EMU_CNT_SEEDS));
   EMU_LAUNCH(EMU_STAGE_SEEDS, st, k_seed_pairs<1><<<kSM * 16, kVoteThreads, 0, st>>>(
       P, sorted, d_cell_start, d_view_off, v0, v1, W.seed_off, plane, W.view_seed_off, W.ctl, W.geo, W.ab, counts));
-  // only the counters of the seeds this chunk has are cleared (the count is on the device: clear the capacity
-  // when the chunk is the size the workspace was cut for, else what its views can hold by the hint)
-  EMU_CK(cudaMemsetAsync(W.seed_cnt, 0, W.seed_cap * sizeof(unsigned long long), st));
+  // only the counters of the seeds this chunk has are cleared (the count is on the device)
+  EMU_LAUNCH(EMU_STAGE_PREP, st, k_clear_seed_cnt<<<kSM * 8, 256, 0, st>>>(W.ctl, W.seed_cnt));
   EMU_LAUNCH(EMU_STAGE_PREP, st, k_plan<<<grid_for(3 * nv, 4, 1 << 20), 128, 0, st>>>(
       P, TT, F, W.bbox, v0, v1, W.bricks, (unsigned)W.brick_cap, W.vf_brick_base, W.ctl));
   EMU_LAUNCH(EMU_STAGE_PREP, st, k_plan_finish<<<1, 1, 0, st>>>(W.ctl, (unsigned)W.brick_cap));
@@ -1718,7 +1853,7 @@ int emu_find_launch(const EmuDev& P, int seeds_per_grain, int cand_per_grain, co
   if (rc != EMU_OK) return rc;
   const int4* sorted = (const int4*)d_sorted;
   unsigned long long* counts = (unsigned long long*)d_counts;
-  const int kSM = sm_count();
+  const int kSM = emu_sm_count();
   EMU_CK(cudaMemsetAsync(d_counts, 0, 8 * sizeof(int64_t), st));
   EMU_CK(cudaMemsetAsync(d_track_off, 0, ((size_t)n_views + 1) * sizeof(int32_t), st));
   EMU_CK(cudaMemsetAsync(W.keyA, 0, (size_t)n_grains * sizeof(unsigned long long), st));
@@ -1754,7 +1889,7 @@ int emu_find_launch(const EmuDev& P, int seeds_per_grain, int cand_per_grain, co
         P, v0, W.ctl, W.view_seed_off, W.seed_cnt, W.geo, W.ab, W.view_cand_cnt, W.view_cand_off, W.view_ovf_cnt,
         W.view_ovf_off, W.cands, W.cand_seed, W.ovf_geo, W.ovf_ci, counts));
     // generic fallback for the whole chunk (returns at once unless the brick plan failed)
-    EMU_LAUNCH(EMU_STAGE_VOTE, st, k_vote_generic<false><<<kSM * 16, kVoteThreads, 0, st>>>(
+    EMU_LAUNCH(EMU_STAGE_GENERIC, st, k_vote_generic<false><<<kSM * 16, kVoteThreads, 0, st>>>(
         P, sorted, d_cell_start, d_view_off, W.bbox, v0, v1, W.cands, (unsigned)W.cand_cap, W.ctl, nullptr, 0, nullptr,
         counts));
     EMU_LAUNCH(EMU_STAGE_PREP, st, k_cands_finish<<<1, 1, 0, st>>>(W.ctl, (unsigned)W.cand_cap, counts));
@@ -1773,7 +1908,15 @@ int emu_find_launch(const EmuDev& P, int seeds_per_grain, int cand_per_grain, co
     EMU_LAUNCH(EMU_STAGE_ASSOC, st, k_assoc_generic<1><<<kSM * 16, kVoteThreads, 0, st>>>(
         P, sorted, d_cell_start, W.bbox, v0, W.cands, W.ctl, W.tie_bits, W.keyA, W.keyB, W.owner));
     EMU_LAUNCH(EMU_STAGE_SELECT, st, k_wins<<<kSM * 4, 256, 0, st>>>(d_view_off, v0, v1, W.ctl, W.keyA, W.keyB, W.owner, W.wins));
-    EMU_LAUNCH(EMU_STAGE_SELECT, st, k_select<<<kSM * 8, 256, 0, st>>>(P, W.cands, W.ctl, W.wins, W.view_ntracks, W.view_tracks, counts));
+    EMU_LAUNCH(EMU_STAGE_SELECT, st, k_select<<<kSM * 8, 256, 0, st>>>(P, W.cands, W.ctl, W.wins, W.view_ntracks, W.view_tracks, W.cand_track, counts));
+    if (P.angle_cut) {                                           // A5b: angle-dependent cut on the number of grains
+      const dim3 gv(4, nv);
+      EMU_LAUNCH(EMU_STAGE_SELECT, st, k_cut_init<<<gv, 256, 0, st>>>(P, nv, W.ctl, W.view_ntracks, W.cut_acc));
+      EMU_LAUNCH(EMU_STAGE_SELECT, st, k_cut_acc<<<kSM * 4, 256, 0, st>>>(
+          P, sorted, d_view_off, v0, v1, W.ctl, W.keyA, W.keyB, W.owner, W.cands, W.cand_track, W.cut_acc));
+      EMU_LAUNCH(EMU_STAGE_SELECT, st, k_cut_decide<<<gv, 256, 0, st>>>(P, nv, W.ctl, W.view_ntracks, W.view_tracks, W.wins, W.cut_acc, W.cand_track));
+      EMU_LAUNCH(EMU_STAGE_SELECT, st, k_cut_compact<<<grid_for(nv, 1, kSM * 8), 256, 0, st>>>(P, nv, W.ctl, W.view_ntracks, W.view_tracks));
+    }
     EMU_LAUNCH(EMU_STAGE_EMIT, st, k_track_scan<<<1, 1024, 0, st>>>(P, v0, v1, W.view_ntracks, d_track_off));
     EMU_LAUNCH(EMU_STAGE_EMIT, st, k_track_emit<<<grid_for(nv, 1, kSM * 8), 256, 0, st>>>(
         P, sorted, v0, v1, W.cands, W.wins, W.view_ntracks, W.view_tracks, d_track_off, d_tracks, W.cand_track));
@@ -1799,7 +1942,7 @@ int emu_count_seeds_launch(const EmuDev& P, int seeds_per_grain, int cand_per_gr
   if (W.views_per_chunk < n_views) return EMU_ERR_CAPACITY;      // the per-seed dump is a one-chunk test aid
   const int4* sorted = (const int4*)d_sorted;
   unsigned long long* counts = (unsigned long long*)d_counts;
-  const int kSM = sm_count();
+  const int kSM = emu_sm_count();
   EMU_CK(cudaMemsetAsync(d_counts, 0, 8 * sizeof(int64_t), st));
   EMU_CK(cudaMemsetAsync(W.dump_cursor, 0, 256, st));
   FramePtrs F;
@@ -1810,7 +1953,7 @@ int emu_count_seeds_launch(const EmuDev& P, int seeds_per_grain, int cand_per_gr
     if (rc != EMU_OK) return rc;
     EMU_LAUNCH(EMU_STAGE_CANDS, st, k_seed_dump<<<dim3(64, 3 * n_views), 256, 0, st>>>(
         0, W.ctl, sorted, W.view_seed_off, W.seed_cnt, W.ab, (int4*)d_seed_dump, dump_capacity));
-    EMU_LAUNCH(EMU_STAGE_VOTE, st, k_vote_generic<true><<<kSM * 16, kVoteThreads, 0, st>>>(
+    EMU_LAUNCH(EMU_STAGE_GENERIC, st, k_vote_generic<true><<<kSM * 16, kVoteThreads, 0, st>>>(
         P, sorted, d_cell_start, d_view_off, W.bbox, 0, n_views, nullptr, 0, W.ctl, (int4*)d_seed_dump, dump_capacity,
         W.dump_cursor, counts));
   }

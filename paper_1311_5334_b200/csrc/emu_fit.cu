@@ -70,6 +70,6 @@ k_fit(const int4* __restrict__ grains, const emu_track* __restrict__ tracks, con
 
 int emu_fit_launch(const int32_t* d_grains, const emu_track* d_tracks, const int32_t* d_track_off,
                    const int32_t* d_members, int32_t n_views, emu_fit* d_fits, cudaStream_t st) {
-  EMU_LAUNCH(EMU_STAGE_FIT, st, k_fit<<<148 * 4, 256, 0, st>>>((const int4*)d_grains, d_tracks, d_track_off, d_members, n_views, d_fits));
+  EMU_LAUNCH(EMU_STAGE_FIT, st, k_fit<<<emu_sm_count() * 4, 256, 0, st>>>((const int4*)d_grains, d_tracks, d_track_off, d_members, n_views, d_fits));
   return cudaGetLastError() == cudaSuccess ? EMU_OK : EMU_ERR_CUDA;
 }

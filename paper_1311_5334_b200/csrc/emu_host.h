@@ -11,6 +11,8 @@ static inline void* emu_align_ptr(void* p) { return (void*)(((uintptr_t)p + 255)
 static inline int64_t emu_min64(int64_t a, int64_t b) { return a < b ? a : b; }
 static inline int64_t emu_max64(int64_t a, int64_t b) { return a > b ? a : b; }
 
+int emu_sm_count();     // multiprocessors of the current device (grids are sized in multiples of it)
+
 // ---- optional per-stage timing (emu_profile_* of include/emu.h) -------------------------------
 // While a profile is active on the calling host thread, every kernel launch of the library is
 // bracketed by a pair of CUDA events on the launch stream and counted.  Without one, EMU_LAUNCH

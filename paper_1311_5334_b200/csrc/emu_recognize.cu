@@ -224,12 +224,12 @@ int emu_recognize_launch(const uint8_t* d_vox, int32_t n_views, int32_t nx, int3
   int* view_tot = (int*)(ws + emu_align256((size_t)n_views * ny * nz * sizeof(int)));
   const int rows_per_view = ny * nz;
   const long long n_rows = (long long)rows_per_view * n_views;
-  const int blocks = (int)emu_max64(1, emu_min64((n_rows + 7) / 8, 148 * 32));
+  const int blocks = (int)emu_max64(1, emu_min64((n_rows + 7) / 8, emu_sm_count() * 32));
   EMU_LAUNCH(EMU_STAGE_RECOG, st, k_recog<0><<<blocks, kRecogThreads, 0, st>>>(R, d_vox, n_views, row, nullptr, nullptr, 0,
                                                                                 (unsigned long long*)d_status));
-  EMU_LAUNCH(EMU_STAGE_RECOG, st, k_row_scan<<<(int)emu_max64(1, emu_min64(n_views, 148 * 2)), 1024, 0, st>>>(rows_per_view, n_views, row, view_tot));
+  EMU_LAUNCH(EMU_STAGE_RECOG, st, k_row_scan<<<(int)emu_max64(1, emu_min64(n_views, emu_sm_count() * 2)), 1024, 0, st>>>(rows_per_view, n_views, row, view_tot));
   EMU_LAUNCH(EMU_STAGE_RECOG, st, k_view_offsets<<<1, 1, 0, st>>>(n_views, view_tot, d_view_off, (long long*)d_count));
-  EMU_LAUNCH(EMU_STAGE_RECOG, st, k_row_rebase<<<(int)emu_max64(1, emu_min64((n_rows + 255) / 256, 148 * 8)), 256, 0, st>>>(rows_per_view, n_views, row, d_view_off));
+  EMU_LAUNCH(EMU_STAGE_RECOG, st, k_row_rebase<<<(int)emu_max64(1, emu_min64((n_rows + 255) / 256, emu_sm_count() * 8)), 256, 0, st>>>(rows_per_view, n_views, row, d_view_off));
   EMU_LAUNCH(EMU_STAGE_RECOG, st, k_recog<1><<<blocks, kRecogThreads, 0, st>>>(R, d_vox, n_views, row, row, (int4*)d_grains, capacity,
                                                                                 (unsigned long long*)d_status));
   return cudaGetLastError() == cudaSuccess ? EMU_OK : EMU_ERR_CUDA;

@@ -5,7 +5,8 @@ import numpy as np
 def gpu_params(E, p: dict, **kw):
     d = dict(view_size_q=p["view_size_q"], cell_size_q=p["cell_size_q"], sep_min_q=p["sep_min_q"],
              sep_max_q=p["sep_max_q"], tube_r2_q=p["tube_r2_q"], min_grains=p["min_grains"],
-             max_tracks_per_view=p.get("max_tracks_per_view", 4096), tube_ext_q=p.get("tube_ext_q", -1))
+             max_tracks_per_view=p.get("max_tracks_per_view", 4096), tube_ext_q=p.get("tube_ext_q", -1),
+             angle_min_grains=p.get("angle_min_grains"))
     d.update(kw)
     return E.make_params(**d)
 

@@ -35,7 +35,7 @@ def test_every_declared_symbol_is_exported(E):
 
 def test_struct_sizes_match_the_header(E):
     from paper_1311_5334_b200.binding import emu_params
-    assert C.sizeof(emu_params) == 4 * (1 + 3 + 3 + 6 + 4)
+    assert C.sizeof(emu_params) == 4 * (1 + 3 + 3 + 6 + 4 + 8)
     assert E.TRACK_DTYPE.itemsize == 32 and E.FIT_DTYPE.itemsize == 48
 
 

@@ -185,16 +185,33 @@ def test_capacity_and_range_errors_are_reported(E):
         E.emu_workspace_bytes(prm, 10, 1)
 
 
-def test_bench_workload_sampled_views(E, oracle_mod):
-    """BASELINE.json configs[4] as bench.py runs it (same generator, parameters, 3x4x4 um cells, recommended workspace,
-    hence the same kernels, frames, three bricks per frame and several internal chunks): 20 views through the CUDA
-    path; views 0, 9 and 19 are compared with the oracle element by element, and the properties that hold at any
-    size are checked on all of them."""
-    import bench
-    V = 20
-    grains, off = bench.make_workload(0, V)
-    p = bench.params_dict()
-    got = run_gpu(E, p, grains, off)
+def _compare_sampled_views(E, got, oracle_mod, p, grains, off, sample, min_tracks=500):
+    """views `sample` of a batch result against the oracle run on those views alone, element by element"""
+    toff, tr, mem = got["track_off"], got["tracks"], got["members"]
+    sub = np.concatenate([grains[off[v]:off[v + 1]] for v in sample])
+    soff = np.zeros(len(sample) + 1, np.int32)
+    soff[1:] = np.cumsum([off[v + 1] - off[v] for v in sample])
+    ref = oracle_mod.track_views(p, sub, soff, "cells", 0)
+    for k, v in enumerate(sample):
+        shift = int(off[v]) - int(soff[k])
+        g = tr[toff[v]:toff[v + 1]]
+        r = ref.tracks[ref.track_off[k]:ref.track_off[k + 1]]
+        assert len(g) == len(r) and len(g) > min_tracks, (v, len(g), len(r))
+        for f in ("n_tube", "n_members", "seed_d2"):
+            assert np.array_equal(g[f], r[f]), (v, f)
+        assert np.array_equal(g["seed_a"] - shift, r["seed_a"]) and np.array_equal(g["seed_b"] - shift, r["seed_b"])
+        assert np.all(g["view"] == v)
+        gm = mem[g["member_off"][0]:g["member_off"][-1] + g["n_members"][-1]] - shift
+        rm = ref.members[r["member_off"][0]:r["member_off"][-1] + r["n_members"][-1]]
+        assert np.array_equal(gm, rm)
+        gf, rf = got["fits"][toff[v]:toff[v + 1]], ref.fits[ref.track_off[k]:ref.track_off[k + 1]]
+        for f in ("axis", "n", "u_min", "u_max"):
+            assert np.array_equal(gf[f], rf[f])
+        assert np.all(np.abs(gf["slope"] - rf["slope"]) <= 1e-5 * np.maximum(np.abs(gf["slope"]), np.abs(rf["slope"])) + 1e-12)
+        assert np.all(np.abs(gf["icpt"] - rf["icpt"]) <= 1e-5 * np.maximum(np.abs(gf["icpt"]), np.abs(rf["icpt"])) + 1e-6)
+
+
+def _check_batch_properties(E, got, p, off, V):
     counts = got["counts"]
     assert int(counts[E.EMU_CNT["status"]]) == 0
     toff, tr, mem = got["track_off"], got["tracks"], got["members"]
@@ -205,27 +222,149 @@ def test_bench_workload_sampled_views(E, oracle_mod):
     assert len(mem) == int(tr["n_members"].sum()) and len(np.unique(mem)) == len(mem)        # exclusive association
     mview = np.searchsorted(off, mem, side="right") - 1
     assert np.array_equal(mview, np.repeat(tr["view"], tr["n_members"]))                     # members stay in their view
-    sample = [0, 9, 19]
-    sub = np.concatenate([grains[off[v]:off[v + 1]] for v in sample])
-    soff = np.zeros(len(sample) + 1, np.int32)
-    soff[1:] = np.cumsum([off[v + 1] - off[v] for v in sample])
-    ref = oracle_mod.track_views(p, sub, soff, "cells", len(sample))
-    for k, v in enumerate(sample):
-        shift = int(off[v]) - int(soff[k])
-        g = tr[toff[v]:toff[v + 1]]
-        r = ref.tracks[ref.track_off[k]:ref.track_off[k + 1]]
-        assert len(g) == len(r) and len(g) > 500
-        for f in ("n_tube", "n_members", "seed_d2"):
-            assert np.array_equal(g[f], r[f]), (v, f)
-        assert np.array_equal(g["seed_a"] - shift, r["seed_a"]) and np.array_equal(g["seed_b"] - shift, r["seed_b"])
-        gm = mem[g["member_off"][0]:g["member_off"][-1] + g["n_members"][-1]] - shift
-        rm = ref.members[r["member_off"][0]:r["member_off"][-1] + r["n_members"][-1]]
-        assert np.array_equal(gm, rm)
-        gf, rf = got["fits"][toff[v]:toff[v + 1]], ref.fits[ref.track_off[k]:ref.track_off[k + 1]]
-        for f in ("axis", "n", "u_min", "u_max"):
-            assert np.array_equal(gf[f], rf[f])
-        assert np.all(np.abs(gf["slope"] - rf["slope"]) <= 1e-5 * np.maximum(np.abs(gf["slope"]), np.abs(rf["slope"])) + 1e-12)
-        assert np.all(np.abs(gf["icpt"] - rf["icpt"]) <= 1e-5 * np.maximum(np.abs(gf["icpt"]), np.abs(rf["icpt"])) + 1e-6)
+
+
+def test_bench_workload_sampled_views(E, oracle_mod):
+    """BASELINE.json configs[4] as bench.py runs it (same generator, parameters, 3x4x4 um cells, hence the same kernels,
+    frames and three bricks per frame): 20 views through the CUDA path, once with the recommended workspace (one
+    internal chunk) and once with a workspace that holds about 8 views per chunk (three chunks, as the 1 024-view
+    bench run has 22).  The views either side of both chunk borders (7 | 8, 15 | 16) and the first and last view are
+    compared with the oracle element by element; the properties that hold at any size are checked on all views."""
+    import bench
+    V = 20
+    grains, off = bench.make_workload(0, V)
+    p = bench.params_dict()
+    got = run_gpu(E, p, grains, off)
+    _check_batch_properties(E, got, p, off, V)
+    # about 2.1 GB of seed / candidate storage per view at the default hints (192 seeds per grain of 160 B, 48
+    # candidates of 48 B): 18 GiB hold 8 views per chunk beside the fixed part
+    got8 = run_gpu(E, p, grains, off, find_ws_bytes=18 << 30)
+    _check_batch_properties(E, got8, p, off, V)
+    for k in ("tracks", "members", "track_off"):
+        assert got[k].tobytes() == got8[k].tobytes(), k                   # the chunking may not be visible
+    _compare_sampled_views(E, got8, oracle_mod, p, grains, off, [0, 7, 8, 15, 16, 19])
+
+
+def test_host_call_bit_exact(E, oracle_mod, config_oracle):
+    """emu_track_views_host (the call bench.py's e2e figure is measured through: H2D, A1..A7, D2H inside) against the
+    oracle: configs 0-3 whole, and a config-4 sample as the bench runs it."""
+    import torch
+    from gpu_helpers import gpu_params
+    for cfg in (0, 1, 2, 3):
+        b, p, ref = config_oracle(cfg)
+        p = dict(p, cell_size_q=default_params(cfg, cell_um=(3.0, 4.0, 4.0))["cell_size_q"])
+        H = E.HostPath(gpu_params(E, p), b.n_grains, b.n_views)
+        out = H.run(b.grains, b.view_off)
+        assert_same_tracks(E, out, ref)
+        out2 = H.run(b.grains, b.view_off)                               # the buffers are reusable
+        assert out2["tracks"].tobytes() == out["tracks"].tobytes() and out2["members"].tobytes() == out["members"].tobytes()
+        del H
+    import bench
+    torch.cuda.empty_cache()
+    V = 6
+    grains, off = bench.make_workload(100, V)                            # views 100..105 of the batch
+    p = bench.params_dict()
+    H = E.HostPath(gpu_params(E, p), len(grains), V)
+    out = H.run(grains, off)
+    _check_batch_properties(E, out, p, off, V)
+    _compare_sampled_views(E, out, oracle_mod, p, grains, off, [0, 3, 5])
+
+
+def test_rank_shard_with_first_view_not_zero(E, oracle_mod):
+    """What rank 1 of a 2-GPU bench.py run does (shard.view_range): its own views of the batch, first_view != 0,
+    through the kernels, against the oracle on the same grains."""
+    import bench
+    from paper_1311_5334_b200 import shard
+    first, n = shard.view_range(1, 2, 3)
+    assert first == 3
+    grains, off = bench.make_workload(first, n)
+    g0, _ = bench.make_workload(0, 1)
+    assert not np.array_equal(grains[:1000], g0[:1000])                  # really other views than rank 0's
+    p = bench.params_dict()
+    got = run_gpu(E, p, grains, off)
+    _check_batch_properties(E, got, p, off, n)
+    _compare_sampled_views(E, got, oracle_mod, p, grains, off, [0, 2])
+
+
+def test_tie_break_keys_golden_on_gpu(E, oracle_mod):
+    """tests/golden/tie_break_keys.json (hand-derived: min(x,y), x, row of kmin and kmax decide): the CUDA path must
+    give the golden tracks, at 8 um cells (generic kernels) and at 3x4x4 um (bricks, hit records, tie settlement)."""
+    with open(os.path.join(HERE, "golden", "tie_break_keys.json")) as f:
+        G = json.load(f)
+    for cell in ((512, 512, 512), (192, 256, 256)):
+        for c in G["cases"]:
+            g = np.zeros((len(c["grains"]), 4), np.int32); g[:, :3] = c["grains"]
+            off = np.asarray([0, len(g)], np.int32)
+            p = dict(G["params"], cell_size_q=cell)
+            got = run_gpu(E, p, g, off)
+            assert int(got["counts"][E.EMU_CNT["seeds"]]) == c["n_seeds"]
+            assert int(got["counts"][E.EMU_CNT["candidates"]]) == c["n_candidates"]
+            assert len(got["tracks"]) == len(c["tracks"]), c["name"]
+            for t, e in zip(got["tracks"], c["tracks"]):
+                for k in ("seed_a", "seed_b", "n_tube", "n_members", "seed_d2"):
+                    assert int(t[k]) == e[k], (c["name"], k)
+                assert [int(x) for x in got["members"][t["member_off"]:t["member_off"] + t["n_members"]]] == e["members"]
+            assert_same_tracks(E, got, oracle_mod.track_views(p, g, off, "brute", 1))
+
+
+@pytest.mark.parametrize("cell_um", [(8.0, 8.0, 8.0), (3.0, 4.0, 4.0)])
+def test_angle_cut_bit_exact(E, oracle_mod, config_oracle, cell_um):
+    """the angle-dependent cut on the number of grains.  The hand-built golden view
+    (every case of its table) and generated views of configs 0-3 with a sloping table, against the oracle; 128-bit
+    exact decision on both sides, so the lists are bit-identical."""
+    with open(os.path.join(HERE, "golden", "angle_cut_tracks.json")) as f:
+        G = json.load(f)
+    g = np.zeros((len(G["grains"]), 4), np.int32); g[:, :3] = G["grains"]
+    off = np.asarray([0, len(g)], np.int32)
+    cell = default_params(0, cell_um=cell_um)["cell_size_q"]
+    for case in G["cases"]:
+        p = dict(G["params"], cell_size_q=cell, angle_min_grains=case["angle_min_grains"])
+        got = run_gpu(E, p, g, off)
+        assert [(int(t["seed_a"]), int(t["seed_b"])) for t in got["tracks"]] == \
+               [(G["tracks"][n]["seed_a"], G["tracks"][n]["seed_b"]) for n in case["order"]]
+        assert_same_tracks(E, got, oracle_mod.track_views(p, g, off, "brute", 1))
+    table = [14, 13, 12, 11, 10, 9, 9, 8]                               # more grains asked of the nearly level tracks
+    for cfg in (0, 1, 2, 3):
+        b, p0, ref0 = config_oracle(cfg)
+        p = dict(p0, cell_size_q=default_params(cfg, cell_um=cell_um)["cell_size_q"], angle_min_grains=table)
+        ref = oracle_mod.track_views(p, b.grains, b.view_off, "cells", 0)
+        assert len(ref.tracks) < len(ref0.tracks)
+        assert_same_tracks(E, run_gpu(E, p, b.grains, b.view_off), ref)
+    # several views, several chunks (the lists are compacted per view)
+    b = make_batch(CONFIGS[0], 0, n_views=7)
+    p = dict(default_params(0, cell_um=cell_um), angle_min_grains=table)
+    ref = oracle_mod.track_views(p, b.grains, b.view_off, "cells", 0)
+    for ws in (None, 200 << 20):
+        assert_same_tracks(E, run_gpu(E, p, b.grains, b.view_off, find_ws_bytes=ws), ref)
+
+
+def test_device_side_overflows_are_reported_and_harmless(E, oracle_mod):
+    """EMU_ST_MEMBER_OVERFLOW, EMU_ST_SEED_OVERFLOW, EMU_ST_CAND_OVERFLOW: the status bit is set, no CUDA error is
+    raised (the fit runs straight after the search, as run_path does), and the next, properly sized call is exact."""
+    import torch
+    from gpu_helpers import gpu_params
+    b = make_config(1)
+    p = default_params(1, cell_um=(3.0, 4.0, 4.0))
+    ref = oracle_mod.track_views(p, b.grains, b.view_off, "cells", 1)
+    d_grains = torch.from_numpy(b.grains).cuda(); d_off = torch.from_numpy(b.view_off).cuda()
+
+    def status_of(prm, **kw):
+        B = E.PathBuffers(prm, b.n_grains, b.n_views, **kw)
+        res = E.run_path(prm, d_grains, d_off, b.n_views, B)
+        torch.cuda.synchronize()                                           # raises if a kernel faulted
+        return res.host()
+    out = status_of(gpu_params(E, p), members_capacity=100)                # 7 020 members do not fit
+    st = int(out["counts"][E.EMU_CNT["status"]])
+    assert st & E.EMU_ST["member_overflow"] and int(out["counts"][E.EMU_CNT["members"]]) == len(ref.members)
+    # hints far below the truth (63 seeds, 3.4 candidates per grain) with the workspace recommended for them
+    prm = gpu_params(E, p, seeds_per_grain=8)                              # 1 476 854 seeds against 1 Mi places
+    out = status_of(prm, find_ws_bytes=E.emu_workspace_bytes(prm, b.n_grains, b.n_views)[1])
+    assert int(out["counts"][E.EMU_CNT["status"]]) & E.EMU_ST["seed_overflow"]
+    assert int(out["counts"][E.EMU_CNT["need"]]) == ref.counters["seeds"]
+    prm = gpu_params(E, p, cand_per_grain=1)                               # 80 930 candidates against 65 536 places
+    out = status_of(prm, find_ws_bytes=E.emu_workspace_bytes(prm, b.n_grains, b.n_views)[1])
+    assert int(out["counts"][E.EMU_CNT["status"]]) & E.EMU_ST["cand_overflow"]
+    assert_same_tracks(E, run_gpu(E, p, b.grains, b.view_off), ref)
 
 
 @pytest.mark.parametrize("cell_um", [(8.0, 8.0, 8.0), (4.0, 4.0, 4.0), (3.0, 4.0, 2.5)])
