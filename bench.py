@@ -229,6 +229,10 @@ def main():
     ap.add_argument("--recognize-views", type=int, default=4,
                     help="also time emu_recognize_grains (SURVEY 8(f) NEXT-4) on this many synthetic 1280 x 1024 x 40 voxel "
                          "stacks rendered from config-1 views; adds the key recognize to the JSON line")
+    ap.add_argument("--stream-views", type=int, default=1024,
+                    help="also run this many views of the workload in batches through emu_stream_* (copies overlapped with "
+                         "the kernels, SURVEY 8(f) NEXT-3) and 32 config-1 views one per batch; adds the key stream; 0 = off")
+    ap.add_argument("--stream-batch", type=int, default=48, help="views per streamed batch")
     ap.add_argument("--tube-ext-um", type=float, default=None,
                     help="bounded tube (SURVEY 8(f) NEXT-1): axial extent beyond the seed grains in um; default: whole line")
     args = ap.parse_args()
@@ -423,6 +427,58 @@ def main():
             del H1
             torch.cuda.empty_cache()
 
+    stream = None
+    if args.stream_views > 0 and world == 1:
+        # the same workload in batches through emu_stream_* (H2D of batch k+1 and D2H of batch k-1
+        # behind the kernels of batch k), and config-1 views one per batch as a microscope would deliver them
+        from emu_synth import CONFIGS, default_params, make_view
+        stream = {}
+        torch.cuda.empty_cache()
+        SV, BV = min(args.stream_views, V), args.stream_batch
+        nb = (SV + BV - 1) // BV
+        bounds = [(b * BV, min(SV, (b + 1) * BV)) for b in range(nb)]
+        S = E.StreamPath(prm, max(int(off[b1] - off[b0]) for b0, b1 in bounds), BV)
+
+        def batch(b):
+            b0, b1 = bounds[b]
+            return grains[off[b0]:off[b1]], (off[b0:b1 + 1] - off[b0]).astype(np.int32)
+        for rep_i in range(2):                                             # the first round warms up
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            nt_s = 0
+            S.submit(*batch(0))
+            for b in range(1, nb):
+                S.submit(*batch(b))
+                nt_s += S.collect(copy=False)["n_tracks"]
+            nt_s += S.collect(copy=False)["n_tracks"]
+            dt = time.perf_counter() - t0
+        assert SV < V or nt_s == int(counts[E.EMU_CNT["tracks"]]), "the streamed batches and the one-call path disagree"
+        stream["config4"] = {"views": SV, "views_per_batch": BV, "grains_per_s": float(off[SV]) / dt, "views_per_s": SV / dt,
+                             "ms_per_view": dt / SV * 1e3, "tracks": nt_s,
+                             "call": "emu_stream_submit / emu_stream_collect, two batches in flight, pinned host buffers"}
+        S.close(); del S
+        torch.cuda.empty_cache()
+        pp = default_params(1, cell_um=CELL_UM, max_tracks_per_view=4096)
+        pp["tube_ext_q"] = TUBE_EXT_Q
+        pr1 = E.make_params(**{k: pp[k] for k in ("view_size_q", "cell_size_q", "sep_min_q", "sep_max_q", "tube_r2_q",
+                                                   "min_grains", "max_tracks_per_view", "tube_ext_q")})
+        views = [make_view(CONFIGS[1], 1, v)[0] for v in range(32)]
+        offs = [np.asarray([0, len(g)], np.int32) for g in views]
+        S = E.StreamPath(pr1, max(len(g) for g in views), 1)
+        for rep_i in range(2):
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            S.submit(views[0], offs[0])
+            for b in range(1, len(views)):
+                S.submit(views[b], offs[b])
+                S.collect(copy=False)
+            S.collect(copy=False)
+            dt = time.perf_counter() - t0
+        stream["config1"] = {"views": len(views), "views_per_batch": 1, "views_per_s": len(views) / dt,
+                             "ms_per_view": dt / len(views) * 1e3, "microscope_rate_hz": 5.0}
+        S.close(); del S
+        torch.cuda.empty_cache()
+
     recog = None
     if args.recognize_views > 0:
         from emu_synth import CONFIGS, make_view
@@ -475,7 +531,7 @@ def main():
         "gpu_launches": int(sum(stage_launches.values())),
         "stage_ms_per_step": {k: v / args.steps for k, v in stage_ms.items()},
         "roofline": roofline, "roofline_bin": roofline_bin, "cpu_baseline": cpu, "e2e": e2e, "clocks": clocks,
-        "single_view": single, "recognize": recog, "parity": parity,
+        "single_view": single, "stream": stream, "recognize": recog, "parity": parity,
         "timing_note": "emu_profile is active inside the timed region: a pair of CUDA events around every launch of the "
                        "library (the per-stage times and gpu_launches come from them); value is therefore conservative",
     }

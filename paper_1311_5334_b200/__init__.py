@@ -5,11 +5,11 @@ the thin Python binding: the same entry points by the same names, argument marsh
 PyTorch supplies device memory and streams, nothing else.  There is no CPU fallback: without the
 built library, or without a CUDA device for the compute calls, everything here raises.
 """
-from .binding import (EMU_CNT, EMU_ST, EMU_STAGE, HostPath, Profile, emu_host_arena_bytes, FIT_DTYPE, TRACK_DTYPE, EmuError, PathBuffers, PathResult, emu_bin_grains,
+from .binding import (EMU_CNT, EMU_ST, EMU_STAGE, HostPath, StreamPath, Profile, emu_host_arena_bytes, FIT_DTYPE, TRACK_DTYPE, EmuError, PathBuffers, PathResult, emu_bin_grains,
                       emu_count_seeds, emu_find_tracks, emu_fit_tracks, emu_grid_cells, emu_workspace_bytes,
                       emu_recognize_grains, emu_recognize_ws_bytes,
                       exported_symbols, library_path, make_params, run_path)
 
-__all__ = ["EMU_CNT", "EMU_ST", "EMU_STAGE", "HostPath", "Profile", "emu_host_arena_bytes", "FIT_DTYPE", "TRACK_DTYPE", "EmuError", "PathBuffers", "PathResult",
+__all__ = ["EMU_CNT", "EMU_ST", "EMU_STAGE", "HostPath", "StreamPath", "Profile", "emu_host_arena_bytes", "FIT_DTYPE", "TRACK_DTYPE", "EmuError", "PathBuffers", "PathResult",
            "emu_bin_grains", "emu_count_seeds", "emu_find_tracks", "emu_fit_tracks", "emu_grid_cells",
            "emu_workspace_bytes", "emu_recognize_grains", "emu_recognize_ws_bytes", "exported_symbols", "library_path", "make_params", "run_path"]

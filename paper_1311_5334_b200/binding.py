@@ -311,6 +311,8 @@ class StreamPath:
 
     def submit(self, grains: np.ndarray, view_off: np.ndarray) -> int:
         import torch
+        if len(self._shapes) >= 2:                   # both pinned input buffers hold batches that are still in flight
+            raise EmuError("StreamPath.submit: two batches are in flight, collect one first")
         hg, ho = self.h_in[self._k & 1]
         n, nv = len(grains), len(view_off) - 1
         if n:

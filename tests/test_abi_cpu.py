@@ -20,7 +20,7 @@ def E():
 def _declared_functions():
     src = open(os.path.join(ROOT, "include", "emu.h")).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-    names = re.findall(r"^\s*(?:size_t|int64_t|int|void|emu_profile\s*\*)\s+\**\s*(emu_\w+)\s*\(", src, flags=re.M)
+    names = re.findall(r"^\s*(?:size_t|int64_t|int|void|emu_profile\s*\*|emu_stream\s*\*)\s+\**\s*(emu_\w+)\s*\(", src, flags=re.M)
     return sorted(set(names))
 
 

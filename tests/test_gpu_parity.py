@@ -270,6 +270,29 @@ def test_host_call_bit_exact(E, oracle_mod, config_oracle):
     _compare_sampled_views(E, out, oracle_mod, p, grains, off, [0, 3, 5])
 
 
+def test_stream_batches_bit_exact(E, oracle_mod):
+    """emu_stream_* (SURVEY 8(f) NEXT-3): seven batches of one to three config-0 views through the double-buffered
+    path, two in flight at any time; every batch against the oracle, and a third submit is refused."""
+    from gpu_helpers import gpu_params
+    p = default_params(0, cell_um=(3.0, 4.0, 4.0))
+    batches = [make_batch(CONFIGS[0], 0, n_views=1 + (k % 3), first_view=10 * k) for k in range(7)]
+    S = E.StreamPath(gpu_params(E, p), max(b.n_grains for b in batches), 3)
+    refs = [oracle_mod.track_views(p, b.grains, b.view_off, "cells", 0) for b in batches]
+    S.submit(batches[0].grains, batches[0].view_off)
+    for k in range(1, len(batches)):
+        S.submit(batches[k].grains, batches[k].view_off)                  # k-1 and k are in flight
+        if k == 1:
+            with pytest.raises(E.EmuError):
+                S.submit(batches[2].grains, batches[2].view_off)          # both slots taken: the binding refuses ...
+            import ctypes as C
+            from paper_1311_5334_b200 import binding
+            hg, ho = S.h_in[0]                                            # ... and so does the library (EMU_ERR_CAPACITY)
+            assert binding._load().emu_stream_submit(S._h, C.c_void_p(hg.data_ptr()), C.c_void_p(ho.data_ptr()), 1, 1) == -2
+        assert_same_tracks(E, S.collect(), refs[k - 1])
+    assert_same_tracks(E, S.collect(), refs[-1])
+    S.close()
+
+
 def test_rank_shard_with_first_view_not_zero(E, oracle_mod):
     """What rank 1 of a 2-GPU bench.py run does (shard.view_range): its own views of the batch, first_view != 0,
     through the kernels, against the oracle on the same grains."""
