@@ -1,6 +1,8 @@
 // emu_bin.cu - A1: attribute every grain to its 3D cell as a counting sort.
 //   count (per-(view,cell) histogram) -> per-view exclusive scan -> scatter -> rank inside the cell.
 // Output order is (view, cell, row): the canonical order SURVEY 8(c) O1 defines.
+#include <stdlib.h>
+
 #include "emu_dev.cuh"
 #include "emu_host.h"
 
@@ -350,12 +352,14 @@ __device__ __forceinline__ int chunk_of(int cell, const SplitPlan& S) {
 
 __global__ void __launch_bounds__(kSplitThreads)
 k_bin_split(EmuDev P, int frame, SplitPlan S, const int4* __restrict__ grains, const int* __restrict__ view_off,
-            int n_views, int4* __restrict__ tmp, int* __restrict__ cur, int* __restrict__ redo,
+            int v_first, int4* __restrict__ tmp, int* __restrict__ cur, int* __restrict__ redo,
             unsigned long long* __restrict__ status) {
-  // grid = (tiles, views): block (t, v) takes tile t of view v; a view with more tiles than the grid has is flagged
+  // grid = (tiles, views of the group): block (t, y) takes tile t of view v_first + y; a view with more tiles than the
+  // grid has is flagged.  The scratch regions are those of the GROUP (indexed by y): every group reuses the same
+  // addresses, so the round trip through the scratch stays in the L2.
   __shared__ int hist_s[kMaxChunks], base_s[kMaxChunks];
   const int tid = threadIdx.x;
-  const int v = blockIdx.y;
+  const int v = v_first + (int)blockIdx.y;
   const int g0 = __ldg(view_off + v), g1 = __ldg(view_off + v + 1);
   const int t0 = g0 + (int)blockIdx.x * (kSplitThreads * kSplitPer);
   if (blockIdx.x == 0 && tid == 0 && (long long)(g1 - g0) > (long long)gridDim.x * (kSplitThreads * kSplitPer)) redo[v] = 1;
@@ -401,19 +405,19 @@ k_bin_split(EmuDev P, int frame, SplitPlan S, const int4* __restrict__ grains, c
   for (int u = 0; u < kSplitPer; ++u) {
     if (kk[u] < 0) continue;
     const int slot = base_s[kk[u]] + rr[u];
-    if (slot < S.cap) tmp[((size_t)v * S.K + kk[u]) * S.cap + slot] = gg[u];
+    if (slot < S.cap) tmp[((size_t)blockIdx.y * S.K + kk[u]) * S.cap + slot] = gg[u];
   }
   if (status && __any_sync(EMU_FULL, bad) && (tid & 31) == 0) atomicOr(status, (unsigned long long)EMU_ST_COORD);
 }
 
 __global__ void __launch_bounds__(kChunkThreads)
-k_bin_chunk(EmuDev P, int frame, SplitPlan S, const int* __restrict__ view_off, int n_views, int n_grains,
+k_bin_chunk(EmuDev P, int frame, SplitPlan S, const int* __restrict__ view_off, int n_views, int n_grains, int v_first,
             const int4* __restrict__ tmp, const int* __restrict__ cur, const int* __restrict__ redo,
             int4* __restrict__ sorted, int* __restrict__ cell_start) {
   extern __shared__ __align__(16) unsigned char chunk_smem[];
   __shared__ int warp_sum[kChunkThreads / 32];
   __shared__ int base_s;
-  const int k = blockIdx.x, v = blockIdx.y;
+  const int k = blockIdx.x, v = v_first + (int)blockIdx.y;
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   const int ncell = P.fr[frame].ncell;
   if (k == 0 && v == 0 && tid == 0) cell_start[(size_t)n_views * ncell] = n_grains;
@@ -425,7 +429,7 @@ k_bin_chunk(EmuDev P, int frame, SplitPlan S, const int* __restrict__ view_off, 
   unsigned short* pre = cnt + ((S.cpc + 1) & ~1);                                    // [cpc] exclusive prefix
   unsigned* cntw = reinterpret_cast<unsigned*>(cnt);
   int* wbuf = reinterpret_cast<int*>(pre + ((S.cpc + 1) & ~1));                      // [cap] rows in arrival order
-  const int4* src = tmp + ((size_t)v * S.K + k) * S.cap;
+  const int4* src = tmp + ((size_t)blockIdx.y * S.K + k) * S.cap;
   const int n = min(cur[(size_t)v * S.K + k], S.cap);
   int4 gg[kChunkPer];                                  // the chunk's grains stay in registers: one batch of independent loads
 #pragma unroll
@@ -512,11 +516,27 @@ SplitPlan split_plan(const EmuDev& P, int frame, int64_t n_grains, int32_t n_vie
   return S;
 }
 
+// views per group of the two-pass path.  A group's scratch regions (K x cap grains per view) are reused by the next
+// group; with groups that fit the L2 the round trip through the scratch could stay on chip.  Measured on the bench
+// (1 024 views): one group 1.14 ms; groups of 128 / 96 / 64 / 48 / 32 / 16 MB: 1.34 / 1.40 / 1.50 / 1.56 / 1.71 / 2.31 ms -
+// the tail of every small launch costs more than the traffic saves, so the default is ONE group (the hook stays for
+// the record; gpurun_out/r2b_bin_sweep.txt).
+#ifndef EMU_BIN_GROUP_MB
+#define EMU_BIN_GROUP_MB (1 << 20)
+#endif
+int split_group_views(const SplitPlan& S, int32_t n_views) {
+  static int mb = 0;
+  if (!mb) { const char* e = getenv("EMU_BIN_GROUP_MB"); mb = e ? atoi(e) : EMU_BIN_GROUP_MB; if (mb < 1) mb = EMU_BIN_GROUP_MB; }   // (tuning hook)
+  const int64_t per_view = (int64_t)S.K * S.cap * 16;
+  const int64_t g = emu_max64(1, ((int64_t)mb << 20) / emu_max64(1, per_view));
+  return (int)emu_min64(emu_min64(g, 65535), emu_max64(1, n_views));
+}
+
 size_t split_tmp_grains(const EmuDev& P, int64_t n_grains, int32_t n_views) {
-  size_t m = (size_t)n_grains;
+  size_t m = (size_t)n_grains;                       // (the one-kernel paths sort big cells through it)
   for (int f = 0; f < 3; ++f) {
     const SplitPlan S = split_plan(P, f, n_grains, n_views);
-    if (S.K) m = emu_max64((int64_t)m, (int64_t)n_views * S.K * S.cap);
+    if (S.K) m = emu_max64((int64_t)m, (int64_t)split_group_views(S, n_views) * S.K * S.cap);
   }
   return m;
 }
@@ -547,7 +567,7 @@ int emu_bin_launch(const EmuDev& P, int frame, const int32_t* d_grains, const in
   int* cur = (int*)((char*)redo + emu_align256(((size_t)n_views + 1) * sizeof(int)));
   const int n = (int)n_grains;
   const SplitPlan S = split_plan(P, frame, n_grains, n_views);
-  if (S.K > 0 && n_views <= 65535) {
+  if (S.K > 0) {
     // two passes: split into chunks of cells, then one chunk per block in shared memory
     const size_t smem = (size_t)S.cap * 16 + 2 * (size_t)((S.cpc + 1) & ~1) * sizeof(unsigned short) + (size_t)S.cap * 4;
     if (cudaFuncSetAttribute(k_bin_chunk, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return EMU_ERR_CUDA;
@@ -556,10 +576,14 @@ int emu_bin_launch(const EmuDev& P, int frame, const int32_t* d_grains, const in
     const int blocks = (int)emu_max64(1, emu_min64(n_views, emu_sm_count() * 8));
     const int tile = kSplitThreads * kSplitPer;
     const int tiles = (int)emu_min64(65535, 2 * ((n_grains / n_views + tile - 1) / tile) + 2);   // per view; larger views are redone
-    EMU_LAUNCH(frame == 0 ? EMU_STAGE_BIN_COUNT : EMU_STAGE_PREP, st, k_bin_split<<<dim3(tiles, n_views), kSplitThreads, 0, st>>>(
-        P, frame, S, (const int4*)d_grains, d_view_off, n_views, tmp, cur, redo, (unsigned long long*)d_status));
-    EMU_LAUNCH(frame == 0 ? EMU_STAGE_BIN_SCATTER : EMU_STAGE_PREP, st, k_bin_chunk<<<dim3(S.K, n_views), kChunkThreads, smem, st>>>(
-        P, frame, S, d_view_off, n_views, n, tmp, cur, redo, (int4*)d_sorted, d_cell_start));
+    const int G = split_group_views(S, n_views);
+    for (int v0 = 0; v0 < n_views; v0 += G) {
+      const int gv = (int)emu_min64(G, n_views - v0);
+      EMU_LAUNCH(frame == 0 ? EMU_STAGE_BIN_COUNT : EMU_STAGE_PREP, st, k_bin_split<<<dim3(tiles, gv), kSplitThreads, 0, st>>>(
+          P, frame, S, (const int4*)d_grains, d_view_off, v0, tmp, cur, redo, (unsigned long long*)d_status));
+      EMU_LAUNCH(frame == 0 ? EMU_STAGE_BIN_SCATTER : EMU_STAGE_PREP, st, k_bin_chunk<<<dim3(S.K, gv), kChunkThreads, smem, st>>>(
+          P, frame, S, d_view_off, n_views, n, v0, tmp, cur, redo, (int4*)d_sorted, d_cell_start));
+    }
     EMU_LAUNCH(frame == 0 ? EMU_STAGE_BIN_PLACE : EMU_STAGE_PREP, st, k_bin_view<false><<<blocks, kViewThreads, 0, st>>>(
         P, frame, (const int4*)d_grains, d_view_off, n_views, n, (int4*)d_sorted, d_cell_start, count, tmp, redo,
         (unsigned long long*)d_status));
