@@ -856,6 +856,8 @@ k_brick(EmuDev P, FramePtrs F, int v0, const Brick* __restrict__ bricks, FindCtl
       unsigned mS = __ballot_sync(EMU_FULL, idle);
       if (!exhausted && __popc(mS) >= kRefill) {
         bool fresh = false;
+        // the counts of the lanes that finished since the last refill leave together (count != 0: not yet flushed)
+        if (kMode == kVote && idle && count) { atomicAdd(seed_cnt + sidx, (unsigned long long)min(count, 0xffff) << ord_shift); count = 0; }
         if (kMode == kVote) {
           // the brick's own list: every record is a hit with its clip stored (k_prep), one pass serves the idle lanes
           if (wcur == wend) {
@@ -995,8 +997,7 @@ k_brick(EmuDev P, FramePtrs F, int v0, const Brick* __restrict__ bricks, FindCtl
       if (!idle && j >= e) {
         const bool nl = cyf >= cyhf;                        // the rows of the layer are used up
         if (nl) { czf += 1.0f; ozm -= P.csf[2]; layp += lay_b; }
-        if (czf > czhf) {                                   // the seed is finished
-          if (kMode == kVote && count) atomicAdd(seed_cnt + sidx, (unsigned long long)min(count, 0xffff) << ord_shift);
+        if (czf > czhf) {                                   // the seed is finished (its count is flushed by the next refill)
           idle = true;
         } else {
           const float tl0 = fmaxf(t0, __fmaf_rn(czf, dtz, tzl)), tl1 = fminf(t1, __fmaf_rn(czf, dtz, tzh));
@@ -1070,6 +1071,7 @@ k_brick(EmuDev P, FramePtrs F, int v0, const Brick* __restrict__ bricks, FindCtl
       }
       }   // body
     }
+    if (kMode == kVote && count) atomicAdd(seed_cnt + sidx, (unsigned long long)min(count, 0xffff) << ord_shift);
     n_tests += item_tests;
   }
 
