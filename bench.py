@@ -495,7 +495,7 @@ def main():
         cap = 1 << 20
         d_g = torch.empty((cap, 4), dtype=torch.int32, device="cuda"); d_o = torch.empty(NV + 1, dtype=torch.int32, device="cuda")
         d_c = torch.zeros(1, dtype=torch.int64, device="cuda"); d_s = torch.zeros(1, dtype=torch.int64, device="cuda")
-        ws = torch.empty(E.emu_recognize_ws_bytes(NV, shape[1], shape[0]), dtype=torch.uint8, device="cuda")
+        ws = torch.empty(E.emu_recognize_ws_bytes(NV, shape[1], shape[0], cap), dtype=torch.uint8, device="cuda")
         for _ in range(3):
             E.emu_recognize_grains(d_vox, THRESHOLD, PITCH_Q, d_g, d_o, d_c, d_s, ws)
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)

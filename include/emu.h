@@ -167,8 +167,9 @@ int emu_fit_tracks(const emu_params* params, const int32_t* d_grains, const emu_
  *       a view in raster order of the defining voxel - the layout emu_bin_grains takes (its w is payload);
  *       d_view_off int32[n_views+1]; d_count int64[1] = grains found (may exceed capacity: then d_status gets
  *       EMU_ST_GRAIN_OVERFLOW and the excess is not written); d_status int64[1], OR-ed, never cleared here.
- *  d_ws: scratch of emu_recognize_ws_bytes(n_views, ny, nz) bytes. */
-size_t emu_recognize_ws_bytes(int32_t n_views, int32_t ny, int32_t nz);
+ *  d_ws: scratch of emu_recognize_ws_bytes(n_views, ny, nz, capacity) bytes (a counter per row of voxels and a 32-byte
+ *       staging record per grain d_grains can hold).  n_views, ny, nz <= 65535. */
+size_t emu_recognize_ws_bytes(int32_t n_views, int32_t ny, int32_t nz, int64_t capacity);
 int emu_recognize_grains(const uint8_t* d_vox, int32_t n_views, int32_t nx, int32_t ny, int32_t nz, int32_t threshold,
                          const int32_t* pitch_q, int32_t* d_grains, int64_t capacity, int32_t* d_view_off,
                          int64_t* d_count, int64_t* d_status, void* d_ws, size_t ws_bytes, void* stream);

@@ -75,7 +75,7 @@ def _load():
         L.emu_track_views_host.restype = C.c_int
         L.emu_track_views_host.argtypes = [vp, vp, vp, i64, i32, vp, vp, i64, vp, vp, i64, vp, vp, sz, vp]
         L.emu_recognize_ws_bytes.restype = sz
-        L.emu_recognize_ws_bytes.argtypes = [i32, i32, i32]
+        L.emu_recognize_ws_bytes.argtypes = [i32, i32, i32, i64]
         L.emu_recognize_grains.restype = C.c_int
         L.emu_recognize_grains.argtypes = [vp, i32, i32, i32, i32, i32, C.POINTER(i32 * 3), vp, i64, vp, vp, vp, vp, sz, vp]
         L.emu_stream_arena_bytes.restype = C.c_int
@@ -212,8 +212,8 @@ def emu_recognize_grains(d_vox, threshold: int, pitch_q, d_grains, d_view_off, d
                                         _nbytes(d_ws), _stream()), "emu_recognize_grains")
 
 
-def emu_recognize_ws_bytes(n_views: int, ny: int, nz: int) -> int:
-    return int(_load().emu_recognize_ws_bytes(int(n_views), int(ny), int(nz)))
+def emu_recognize_ws_bytes(n_views: int, ny: int, nz: int, capacity: int) -> int:
+    return int(_load().emu_recognize_ws_bytes(int(n_views), int(ny), int(nz), int(capacity)))
 
 
 def emu_host_arena_bytes(params: emu_params, n_grains: int, n_views: int) -> int:

@@ -546,35 +546,44 @@ __device__ __forceinline__ float rcp_fast(float x) {
 struct PrepRec { int4 geo; unsigned sidx; float t0, t1; unsigned layers; };   // 32 B; layers = first | last << 16
 constexpr int kPrepSub = 32;            // sub-lists per brick = blocks per (view, frame) of k_prep
 
+// the line of a seed as the clip needs it (computed once per seed, used for every brick of its (view, frame))
+struct ClipLine { float ax, ay, az, dx, a, bz, y0, z0, inv_a, inv_b, eu; bool has_y, has_z; };
+
 template <bool kBounded>
-__device__ __forceinline__ bool clip_to_brick(const EmuDev& P, const Brick& B, const int4& q, float& t0, float& t1,
-                                              unsigned& layers) {
-  const float R = P.Rw;
-  const float ax = (float)(q.x & 0xffff), ay = (float)((unsigned)q.x >> 16), az = (float)(q.y & 0xffff);
+__device__ __forceinline__ ClipLine clip_line(const EmuDev& P, const int4& q) {
+  ClipLine L;
+  L.ax = (float)(q.x & 0xffff); L.ay = (float)((unsigned)q.x >> 16); L.az = (float)(q.y & 0xffff);
   int idx, idy, idz;
   geo_d(q, idx, idy, idz);
   const float dx = (float)idx, dy = (float)idy, dz = (float)idz;
   const float inv_dx = rcp_fast(dx);                                  // du >= 1
-  const float a = dy * inv_dx, bz = dz * inv_dx;
-  const float y0 = __fmaf_rn(-a, ax, ay), z0 = __fmaf_rn(-bz, ax, az);
-  const float inv_a = dy != 0.f ? dx * rcp_fast(dy) : 0.0f;
-  const float inv_b = dz != 0.f ? dx * rcp_fast(dz) : 0.0f;
+  L.dx = dx;
+  L.a = dy * inv_dx; L.bz = dz * inv_dx;
+  L.y0 = __fmaf_rn(-L.a, L.ax, L.ay); L.z0 = __fmaf_rn(-L.bz, L.ax, L.az);
+  L.has_y = dy != 0.f; L.has_z = dz != 0.f;
+  L.inv_a = L.has_y ? dx * rcp_fast(dy) : 0.0f;
+  L.inv_b = L.has_z ? dx * rcp_fast(dz) : 0.0f;
+  // bounded tube: the feet of the grains that can count lie between u(A) - E du/|d| and u(B) + E du/|d| (2 q of slack)
+  L.eu = kBounded ? __fmaf_rn((float)P.ext * dx, rsqrtf(__fmaf_rn(dx, dx, __fmaf_rn(dy, dy, dz * dz))) * 1.0001f, 2.0f) : 0.0f;
+  return L;
+}
+
+template <bool kBounded>
+__device__ __forceinline__ bool clip_to_brick(const EmuDev& P, const Brick& B, const ClipLine& L, float& t0, float& t1,
+                                              unsigned& layers) {
+  const float R = P.Rw;
   const float blo0 = (float)(B.cx0 * P.cs[0]) - R, bhi0 = (float)((B.cx1 + 1) * P.cs[0] - 1) + R;
   const float blo1 = (float)(B.cy0 * P.cs[1]) - R, bhi1 = (float)((B.cy1 + 1) * P.cs[1] - 1) + R;
   const float blo2 = (float)(B.cz0 * P.cs[2]) - R, bhi2 = (float)((B.cz1 + 1) * P.cs[2] - 1) + R;
   t0 = blo0; t1 = bhi0;
   bool hit = true;
-  if (dy != 0.f) { const float p = (blo1 - y0) * inv_a, r = (bhi1 - y0) * inv_a; t0 = fmaxf(t0, fminf(p, r)); t1 = fminf(t1, fmaxf(p, r)); }
-  else hit = hit && (ay >= blo1) && (ay <= bhi1);
-  if (dz != 0.f) { const float p = (blo2 - z0) * inv_b, r = (bhi2 - z0) * inv_b; t0 = fmaxf(t0, fminf(p, r)); t1 = fminf(t1, fmaxf(p, r)); }
-  else hit = hit && (az >= blo2) && (az <= bhi2);
-  if (kBounded) {
-    // the feet of the grains that can count lie between u(A) - E du/|d| and u(B) + E du/|d| (2 q of slack)
-    const float eu = __fmaf_rn((float)P.ext * dx, rsqrtf(__fmaf_rn(dx, dx, __fmaf_rn(dy, dy, dz * dz))) * 1.0001f, 2.0f);
-    t0 = fmaxf(t0, ax - eu); t1 = fminf(t1, ax + dx + eu);
-  }
+  if (L.has_y) { const float p = (blo1 - L.y0) * L.inv_a, r = (bhi1 - L.y0) * L.inv_a; t0 = fmaxf(t0, fminf(p, r)); t1 = fminf(t1, fmaxf(p, r)); }
+  else hit = hit && (L.ay >= blo1) && (L.ay <= bhi1);
+  if (L.has_z) { const float p = (blo2 - L.z0) * L.inv_b, r = (bhi2 - L.z0) * L.inv_b; t0 = fmaxf(t0, fminf(p, r)); t1 = fminf(t1, fmaxf(p, r)); }
+  else hit = hit && (L.az >= blo2) && (L.az <= bhi2);
+  if (kBounded) { t0 = fmaxf(t0, L.ax - L.eu); t1 = fminf(t1, L.ax + L.dx + L.eu); }
   if (!(hit && t0 <= t1)) return false;
-  const float za = __fmaf_rn(bz, t0, z0), zb = __fmaf_rn(bz, t1, z0);
+  const float za = __fmaf_rn(L.bz, t0, L.z0), zb = __fmaf_rn(L.bz, t1, L.z0);
   const int c_lo = max(B.cz0, rn_int(__fmaf_rn(fminf(za, zb), P.inv_cs[2], P.klo[2])));
   const int c_hi = min(B.cz1, rn_int(__fmaf_rn(fmaxf(za, zb), P.inv_cs[2], P.khi[2])));
   if (c_lo > c_hi) return false;
@@ -595,11 +604,12 @@ k_prep(EmuDev P, const FindCtl* __restrict__ ctl, const unsigned* __restrict__ v
     const unsigned i = i0 + (unsigned)lane;
     const bool on = i < hi;
     const int4 q = on ? __ldg(geo + i) : make_int4(0, 0, 0x08010801, 0x0800);   // (an idle lane: d = (1, 1, 0))
+    const ClipLine L = clip_line<kBounded>(P, q);
     for (int k = 0; k < vb.y; ++k) {
       const Brick B = bricks[vb.x + k];
       float t0, t1;
       unsigned layers = 0;
-      const bool hit = on && clip_to_brick<kBounded>(P, B, q, t0, t1, layers);
+      const bool hit = on && clip_to_brick<kBounded>(P, B, L, t0, t1, layers);
       const unsigned m = __ballot_sync(EMU_FULL, hit);
       if (!m) continue;
       // every brick's list is cut into kPrepSub sub-lists, one per blockIdx.x, each with its own counter: the eight

@@ -112,7 +112,7 @@ def test_batch_of_views_in_several_chunks(E, oracle_mod):
     _, rec = E.emu_workspace_bytes(prm, b.n_grains, b.n_views)
     # the recommendation holds all 7 views at once; the minimum seed / candidate capacity (1 Mi seeds of 160 B:
     # geometry, counter and hit records) holds about 3 views of this shape at the default hint of 192 seeds per grain
-    for ws in (None, 200 << 20):
+    for ws in (None, 300 << 20):
         got = run_gpu(E, p, b.grains, b.view_off, find_ws_bytes=ws)
         assert_same_tracks(E, got, ref)
 
@@ -357,7 +357,7 @@ def test_angle_cut_bit_exact(E, oracle_mod, config_oracle, cell_um):
     b = make_batch(CONFIGS[0], 0, n_views=7)
     p = dict(default_params(0, cell_um=cell_um), angle_min_grains=table)
     ref = oracle_mod.track_views(p, b.grains, b.view_off, "cells", 0)
-    for ws in (None, 200 << 20):
+    for ws in (None, 300 << 20):
         assert_same_tracks(E, run_gpu(E, p, b.grains, b.view_off, find_ws_bytes=ws), ref)
 
 

@@ -26,7 +26,7 @@ def _gpu(E, vox, thr, pitch, capacity=None):
     d_off = torch.zeros(nv + 1, dtype=torch.int32, device="cuda")
     d_cnt = torch.zeros(1, dtype=torch.int64, device="cuda")
     d_st = torch.zeros(1, dtype=torch.int64, device="cuda")
-    ws = torch.empty(E.emu_recognize_ws_bytes(nv, ny, nz), dtype=torch.uint8, device="cuda")
+    ws = torch.empty(E.emu_recognize_ws_bytes(nv, ny, nz, cap), dtype=torch.uint8, device="cuda")
     E.emu_recognize_grains(d_vox, thr, pitch, d_g, d_off, d_cnt, d_st, ws)
     torch.cuda.synchronize()
     n = int(d_cnt.cpu()[0])
