@@ -229,6 +229,9 @@ def main():
     ap.add_argument("--recognize-views", type=int, default=4,
                     help="also time emu_recognize_grains (SURVEY 8(f) NEXT-4) on this many synthetic 1280 x 1024 x 40 voxel "
                          "stacks rendered from config-1 views; adds the key recognize to the JSON line")
+    ap.add_argument("--find-ws-gib", type=float, default=None,
+                    help="workspace given to emu_find_tracks in GiB (default: what emu_workspace_bytes recommends, about "
+                         "100 GiB for the full batch); the views are then processed in smaller internal chunks")
     ap.add_argument("--stream-views", type=int, default=1024,
                     help="also run this many views of the workload in batches through emu_stream_* (copies overlapped with "
                          "the kernels, SURVEY 8(f) NEXT-3) and 32 config-1 views one per batch; adds the key stream; 0 = off")
@@ -276,7 +279,8 @@ def main():
                                              "min_grains", "max_tracks_per_view", "tube_ext_q")})
     d_grains = torch.from_numpy(grains).cuda()
     d_off = torch.from_numpy(off).cuda()
-    B = E.PathBuffers(prm, n, V)
+    find_ws = int(args.find_ws_gib * (1 << 30)) if args.find_ws_gib else None
+    B = E.PathBuffers(prm, n, V, find_ws_bytes=find_ws)
 
     def barrier():
         torch.cuda.synchronize()
@@ -284,6 +288,7 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
+    B_ws_bytes = B.ws.numel()
     for _ in range(args.warmup):
         E.run_path(prm, d_grains, d_off, V, B)
     barrier()
@@ -525,6 +530,7 @@ def main():
         "vs_baseline": None, "dtype": "int32", "data": "synthetic", "config": workload_config(V, world),
         "views_per_s": V * world / (ms_step * 1e-3),
         "cm2_per_hour": V * world / (ms_step * 1e-3) * 3600 * VIEW_AREA_CM2,
+        "find_workspace_gib": float(B_ws_bytes) / (1 << 30),
         "grains_per_gpu": n, "seeds": seeds, "candidates": int(counts[E.EMU_CNT["candidates"]]),
         "tracks": int(counts[E.EMU_CNT["tracks"]]),
         "tests_per_seed_gpu": float(counts[E.EMU_CNT["tests"]]) / max(1, seeds),

@@ -32,6 +32,7 @@
 // Everything is a max / min / sum over a total order, so the result does not depend on the order in
 // which threads run (reading Q7: "one-shot, order-free").
 #include <math.h>
+#include <stdlib.h>
 
 #include "emu_dev.cuh"
 #include "emu_host.h"
@@ -484,14 +485,27 @@ k_plan(EmuDev P, Tilings TT, FramePtrs F, const EmuBox* __restrict__ bbox, int v
       if (cx0 > cx1 || cy0 > cy1) continue;
       const int W = cx1 - cx0 + 1, H = cy1 - cy0 + 1;
       int z_first = 0, acc = 0;
+      int batch = 0;                                        // grains of layer (cz & ~31) + lane, 32 layers at a time
       for (int cz = 0; cz <= nz; ++cz) {
+        if ((cz & 31) == 0) {
+          // the counts of the next 32 layers, one per lane (a layer at a time made every step wait for its own loads:
+          // 0.2 ms for the 75 layers of frame 2 when a single view is processed)
+          const int mz = cz + lane;
+          batch = 0;
+          if (mz < nz) {
+            if (W == nx) {                                  // full rows: the cells of rows cy0..cy1 are consecutive
+              batch = __ldg(cell_start + vbase + (mz * ny + cy1) * nx + nx) - __ldg(cell_start + vbase + (mz * ny + cy0) * nx);
+            } else {
+              for (int cy = cy0; cy <= cy1; ++cy) {
+                const int rb = vbase + (mz * ny + cy) * nx;
+                batch += __ldg(cell_start + rb + cx1 + 1) - __ldg(cell_start + rb + cx0);
+              }
+            }
+          }
+        }
         int cnt = 0;
         if (cz < nz) {
-          for (int cy = cy0 + lane; cy <= cy1; cy += 32) {
-            const int rb = vbase + (cz * ny + cy) * nx;
-            cnt += __ldg(cell_start + rb + cx1 + 1) - __ldg(cell_start + rb + cx0);
-          }
-          cnt = __reduce_add_sync(EMU_FULL, cnt);
+          cnt = __shfl_sync(EMU_FULL, batch, cz & 31);
           if (brick_bytes(cnt, H, W) > kPoolBytes) { if (lane == 0) ctl->generic = 1; return; }
         }
         const bool flush = (cz == nz) || brick_bytes(acc + cnt, (long long)(cz - z_first + 1) * H, W) > kPoolBytes;
@@ -544,7 +558,8 @@ __device__ __forceinline__ float rcp_fast(float x) {
 }
 
 struct PrepRec { int4 geo; unsigned sidx; float t0, t1; unsigned layers; };   // 32 B; layers = first | last << 16
-constexpr int kPrepSub = 32;            // sub-lists per brick = blocks per (view, frame) of k_prep
+constexpr int kPrepSubMin = 32, kPrepSubMax = 512;   // sub-lists per brick = blocks per (view, frame) of k_prep: more when
+                                                     // the chunk holds few views, so that a single view still fills the GPU
 
 // the line of a seed as the clip needs it (computed once per seed, used for every brick of its (view, frame))
 struct ClipLine { float ax, ay, az, dx, a, bz, y0, z0, inv_a, inv_b, eu; bool has_y, has_z; };
@@ -612,9 +627,9 @@ k_prep(EmuDev P, const FindCtl* __restrict__ ctl, const unsigned* __restrict__ v
       const bool hit = on && clip_to_brick<kBounded>(P, B, L, t0, t1, layers);
       const unsigned m = __ballot_sync(EMU_FULL, hit);
       if (!m) continue;
-      // every brick's list is cut into kPrepSub sub-lists, one per blockIdx.x, each with its own counter: the eight
+      // every brick's list is cut into gridDim.x sub-lists, one per blockIdx.x, each with its own counter: the eight
       // warps of a block are all that ever meet on one address (a single counter per brick cost 0.9 ms per view)
-      const unsigned slot = (unsigned)(vb.x + k) * (unsigned)kPrepSub + blockIdx.x;
+      const unsigned slot = (unsigned)(vb.x + k) * gridDim.x + blockIdx.x;
       unsigned base = 0;
       if (lane == 0) base = atomicAdd(brick_cnt + slot, (unsigned)__popc(m));
       if (!kFill) continue;
@@ -693,7 +708,7 @@ template <int kMode, bool kBounded>
 __global__ void __launch_bounds__(kBrickThreads, 1)
 k_brick(EmuDev P, FramePtrs F, int v0, const Brick* __restrict__ bricks, FindCtl* __restrict__ ctl,
         int slices, const int4* __restrict__ geo, const unsigned* __restrict__ item_ci,
-        const unsigned* __restrict__ view_item_off, const PrepRec* __restrict__ prec, const unsigned* __restrict__ brick_off, unsigned long long* __restrict__ seed_cnt, unsigned short* __restrict__ recs, int* __restrict__ slot_row,
+        const unsigned* __restrict__ view_item_off, const PrepRec* __restrict__ prec, const unsigned* __restrict__ brick_off, int prep_sub, unsigned long long* __restrict__ seed_cnt, unsigned short* __restrict__ recs, int* __restrict__ slot_row,
         unsigned long long* __restrict__ keyA, unsigned long long* __restrict__ keyB,
         unsigned long long* __restrict__ counts) {
   extern __shared__ __align__(16) unsigned char pool[];
@@ -724,7 +739,7 @@ k_brick(EmuDev P, FramePtrs F, int v0, const Brick* __restrict__ bricks, FindCtl
     if (w >= n_items) break;
     const int b = (int)(w / (unsigned)slices), sl = (int)(w % (unsigned)slices);
     if (kMode == kVote) {                                // an item whose slice of the brick's list is empty: nothing to stage
-      const unsigned lo = brick_off[b * kPrepSub], hi = brick_off[(b + 1) * kPrepSub];
+      const unsigned lo = brick_off[b * prep_sub], hi = brick_off[(b + 1) * prep_sub];
       const unsigned per = (hi - lo + (unsigned)slices - 1u) / (unsigned)slices;
       if (min(hi, lo + per * (unsigned)sl) >= hi) continue;
     }
@@ -799,8 +814,8 @@ k_brick(EmuDev P, FramePtrs F, int v0, const Brick* __restrict__ bricks, FindCtl
     {
       // VOTE: the brick's own list of prepared seeds (k_prep); ASSOC: the walk list of the brick's (view, frame)
       const int vf = (B.view - v0) * 3 + B.frame;
-      const unsigned lo = kMode == kVote ? brick_off[b * kPrepSub] : view_item_off[vf];
-      const unsigned hi = kMode == kVote ? brick_off[(b + 1) * kPrepSub] : view_item_off[vf + 1];
+      const unsigned lo = kMode == kVote ? brick_off[b * prep_sub] : view_item_off[vf];
+      const unsigned hi = kMode == kVote ? brick_off[(b + 1) * prep_sub] : view_item_off[vf + 1];
       const unsigned per = (hi - lo + (unsigned)slices - 1u) / (unsigned)slices;
       const unsigned s0 = min(hi, lo + per * (unsigned)sl), s1 = min(hi, s0 + per);
       if (tid == 0) { sh.next = s0; sh.end = s1; }
@@ -1609,11 +1624,13 @@ k_track_emit(EmuDev P, const int4* __restrict__ sorted, int v0, int v1, const Ca
              const int* __restrict__ wins, const int* __restrict__ view_ntracks,
              const unsigned* __restrict__ view_tracks, const int* __restrict__ track_off,
              emu_track* __restrict__ tracks, unsigned* __restrict__ cand_track) {
-  for (int v = v0 + blockIdx.x; v < v1; v += gridDim.x) {
+  // grid = (parts, views): the tracks of a view are dealt to gridDim.x blocks (one view alone would otherwise rank its
+  // 1 400 tracks against one another in a single block: 1.9 ms for a config-4 view)
+  for (int v = v0 + blockIdx.y; v < v1; v += gridDim.y) {
     const int nt = view_ntracks[v - v0];
     const unsigned* list = view_tracks + (size_t)(v - v0) * P.max_tracks;
     const int t0 = track_off[v];
-    for (int i = threadIdx.x; i < nt; i += blockDim.x) {
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < nt; i += gridDim.x * blockDim.x) {
       const unsigned ci = list[i];
       const Cand c = cands[ci];
       int rank = 0;
@@ -1752,7 +1769,7 @@ struct FindWs {
   int4* sortedF[3]; int* cell_startF[3]; void* bin_ws; size_t bin_ws_bytes;     // frames 1, 2 (0 = the caller's)
   int* slot_row; int* vf_brick_base; unsigned* view_ovf_cnt; unsigned* view_ovf_off;
   int4* geo; int2* ab; unsigned long long* seed_cnt; unsigned short* recs;
-  PrepRec* prec; size_t prep_cap; int2* vf_bricks; unsigned* brick_cnt; unsigned* brick_off;
+  PrepRec* prec; size_t prep_cap; int2* vf_bricks; unsigned* brick_cnt; unsigned* brick_off; int prep_sub;
   Cand* cands; unsigned* cand_seed; int4* ovf_geo; unsigned* ovf_ci; int* wins; unsigned* cand_track;
   CutAcc* cut_acc;                                                                // only with the angle cut
   size_t seed_cap, cand_cap, brick_cap; int views_per_chunk;
@@ -1770,6 +1787,12 @@ size_t bricks_per_view(const EmuDev& P, const Tilings& TT) {
   return n;
 }
 
+// sub-lists per brick for chunks of up to vpc views: about 8 blocks of k_prep per SM of a 148-SM part
+int prep_sub_for(int vpc) {
+  const int s = (8 * 148 + 3 * vpc - 1) / (3 * (vpc > 0 ? vpc : 1));
+  return s < kPrepSubMin ? kPrepSubMin : (s > kPrepSubMax ? kPrepSubMax : s);
+}
+
 size_t fixed_bytes(const EmuDev& P, const Tilings& TT, int64_t n_grains, int32_t n_views, int vpc) {
   size_t b = 0;
   b += emu_align256((size_t)n_views * sizeof(EmuBox));
@@ -1785,7 +1808,7 @@ size_t fixed_bytes(const EmuDev& P, const Tilings& TT, int64_t n_grains, int32_t
   if (P.angle_cut) b += emu_align256((size_t)vpc * P.max_tracks * sizeof(CutAcc));
   b += emu_align256((size_t)vpc * bricks_per_view(P, TT) * sizeof(Brick));
   b += emu_align256(3 * (size_t)vpc * sizeof(int2));                        // vf_bricks
-  b += 2 * emu_align256(((size_t)vpc * bricks_per_view(P, TT) * kPrepSub + 1) * sizeof(unsigned));   // brick_cnt, brick_off
+  b += 2 * emu_align256(((size_t)vpc * bricks_per_view(P, TT) * prep_sub_for(vpc) + 1) * sizeof(unsigned));   // brick_cnt, brick_off
   for (int f = 1; f < 3; ++f) {                                             // the binnings of frames 1 and 2
     b += emu_align256((size_t)n_grains * sizeof(int4));
     b += emu_align256(((size_t)n_views * P.fr[f].ncell + 1) * sizeof(int));
@@ -1914,8 +1937,9 @@ static int carve(const EmuDev& P, const Tilings& TT, Hints hints, int64_t n_grai
   W.brick_cap = (size_t)vpc * bricks_per_view(P, TT);
   W.bricks = (Brick*)take(W.brick_cap * sizeof(Brick));
   W.vf_bricks = (int2*)take(3 * (size_t)vpc * sizeof(int2));
-  W.brick_cnt = (unsigned*)take((W.brick_cap * kPrepSub + 1) * sizeof(unsigned));
-  W.brick_off = (unsigned*)take((W.brick_cap * kPrepSub + 1) * sizeof(unsigned));
+  W.prep_sub = prep_sub_for(vpc);
+  W.brick_cnt = (unsigned*)take((W.brick_cap * W.prep_sub + 1) * sizeof(unsigned));
+  W.brick_off = (unsigned*)take((W.brick_cap * W.prep_sub + 1) * sizeof(unsigned));
   W.sortedF[0] = nullptr; W.cell_startF[0] = nullptr;
   for (int f = 1; f < 3; ++f) {
     W.sortedF[f] = (int4*)take((size_t)n_grains * sizeof(int4));
@@ -1948,12 +1972,21 @@ static int grid_for(int64_t n, int threads, int max_blocks) {
 
 #define EMU_CK(x) do { if ((x) != cudaSuccess) return EMU_ERR_CUDA; } while (0)
 
-static int choose_slices(const Tilings& TT, int nv, int n_sm, int per_sm) {
-  // enough work items that every SM gets several even when the chunk holds few views
+static int choose_slices(const Tilings& TT, int nv, int n_sm, int per_sm, int64_t chunk_grains, int entries_per_grain,
+                         int min_entries = 2048) {
+  // Work items = bricks x slices of a brick's list.  A big chunk wants fine items (per_sm of them per SM: short tail);
+  // a small one must not be cut finer than its work pays for - an item stages its brick and drains its lanes once:
+  // at least one item per SM if that leaves about min_entries list entries per item, items of 16 Ki entries beyond
+  // that.  (A single config-1 view: 768 items of 1 900 seeds took 1.02 ms, 150 items of 10 k take 0.52; config 0:
+  // 0.31 -> 0.09 ms.)  The lists are counted on the device; the host plans with entries_per_grain per grain.
   int64_t bricks = 0;
   for (int f = 0; f < 3; ++f) bricks += (int64_t)nv * TT.t[f].tx * TT.t[f].ty;
   bricks = emu_max64(1, bricks);
-  int64_t s = (per_sm * (int64_t)n_sm + bricks - 1) / bricks;
+  const int64_t fine = (per_sm * (int64_t)n_sm + bricks - 1) / bricks;
+  const int64_t wave = ((int64_t)n_sm + bricks - 1) / bricks;
+  const int64_t per_brick = chunk_grains * entries_per_grain / bricks;
+  int64_t s = emu_min64(fine, emu_max64(wave, per_brick / 16384));
+  s = emu_min64(s, emu_max64(1, per_brick / min_entries));
   if (s < 1) s = 1;
   if (s > 256) s = 256;
   return (int)s;
@@ -2001,20 +2034,20 @@ static int vote_chunk(const EmuDev& P, const Tilings& TT, FindWs& W, const Frame
       P, TT, F, W.bbox, v0, v1, W.bricks, (unsigned)W.brick_cap, W.vf_brick_base, W.vf_bricks, W.ctl));
   EMU_LAUNCH(EMU_STAGE_PREP, st, k_plan_finish<<<1, 1, 0, st>>>(W.ctl, (unsigned)W.brick_cap));
   // per-brick lists of prepared seeds: count, scan over the bricks, fill
-  const dim3 gp(kPrepSub, 3 * nv);
-  EMU_CK(cudaMemsetAsync(W.brick_cnt, 0, (W.brick_cap * kPrepSub + 1) * sizeof(unsigned), st));
+  const dim3 gp(W.prep_sub, 3 * nv);
+  EMU_CK(cudaMemsetAsync(W.brick_cnt, 0, (W.brick_cap * W.prep_sub + 1) * sizeof(unsigned), st));
   if (P.ext >= 0) EMU_LAUNCH(EMU_STAGE_SEEDS, st, k_prep<0, true><<<gp, 256, 0, st>>>(P, W.ctl, W.view_seed_off, W.geo, W.bricks, W.vf_bricks, W.brick_cnt, nullptr, nullptr));
   else EMU_LAUNCH(EMU_STAGE_SEEDS, st, k_prep<0, false><<<gp, 256, 0, st>>>(P, W.ctl, W.view_seed_off, W.geo, W.bricks, W.vf_bricks, W.brick_cnt, nullptr, nullptr));
   EMU_LAUNCH(EMU_STAGE_SEEDS, st, k_chunk_offsets<<<1, 1024, 0, st>>>(
-      (int)(W.brick_cap * kPrepSub), W.brick_cnt, W.brick_off, &W.ctl->prep_count, (unsigned)W.prep_cap, (unsigned)EMU_ST_SEED_OVERFLOW,
+      (int)(W.brick_cap * W.prep_sub), W.brick_cnt, W.brick_off, &W.ctl->prep_count, (unsigned)W.prep_cap, (unsigned)EMU_ST_SEED_OVERFLOW,
       W.ctl, counts, -1, -1));
-  EMU_CK(cudaMemsetAsync(W.brick_cnt, 0, (W.brick_cap * kPrepSub + 1) * sizeof(unsigned), st));
+  EMU_CK(cudaMemsetAsync(W.brick_cnt, 0, (W.brick_cap * W.prep_sub + 1) * sizeof(unsigned), st));
   if (P.ext >= 0) EMU_LAUNCH(EMU_STAGE_SEEDS, st, k_prep<1, true><<<gp, 256, 0, st>>>(P, W.ctl, W.view_seed_off, W.geo, W.bricks, W.vf_bricks, W.brick_cnt, W.brick_off, W.prec));
   else EMU_LAUNCH(EMU_STAGE_SEEDS, st, k_prep<1, false><<<gp, 256, 0, st>>>(P, W.ctl, W.view_seed_off, W.geo, W.bricks, W.vf_bricks, W.brick_cnt, W.brick_off, W.prec));
   auto vote_kernel = P.ext >= 0 ? k_brick<kVote, true> : k_brick<kVote, false>;
   EMU_CK(cudaFuncSetAttribute(vote_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kPoolBytes));
   EMU_LAUNCH(EMU_STAGE_VOTE, st, vote_kernel<<<kSM, kBrickThreads, kPoolBytes, st>>>(
-      P, F, v0, W.bricks, W.ctl, slices, W.geo, nullptr, W.view_seed_off, W.prec, W.brick_off, W.seed_cnt, W.recs, W.slot_row, nullptr,
+      P, F, v0, W.bricks, W.ctl, slices, W.geo, nullptr, W.view_seed_off, W.prec, W.brick_off, W.prep_sub, W.seed_cnt, W.recs, W.slot_row, nullptr,
       nullptr, counts));
   return EMU_OK;
 }
@@ -2043,15 +2076,18 @@ int emu_find_launch(const EmuDev& P, int seeds_per_grain, int cand_per_grain, co
   for (int v0 = 0; v0 < n_views; v0 += W.views_per_chunk) {
     const int v1 = (int)emu_min64(n_views, (int64_t)v0 + W.views_per_chunk);
     const int nv = v1 - v0;
-    const int slices = choose_slices(TT, nv, kSM, EMU_ITEMS_PER_SM);      // the voting pass: fine items, short tail
-    const int slices_walk = choose_slices(TT, nv, kSM, 4);                // the walk list is short: staging would dominate
+    // (host copies of view_off are not available: the chunk's grains are taken as its share of the batch)
+    const int64_t chunk_grains = n_views > 0 ? n_grains * nv / n_views : 0;
+    const int slices = choose_slices(TT, nv, kSM, EMU_ITEMS_PER_SM, chunk_grains, 64);   // the voting pass: fine items, short tail
+    const int slices_walk = choose_slices(TT, nv, kSM, 4, chunk_grains, 1);              // the walk list is short: staging would dominate
     EMU_CK(cudaMemsetAsync(W.view_ntracks, 0, (size_t)nv * sizeof(int), st));
     EMU_CK(cudaMemsetAsync(W.tie_bits, 0, kTieBits / 8, st));
     rc = vote_chunk(P, TT, W, F, d_view_off, n_grains, v0, v1, slices, kSM, counts, st);
     if (rc != EMU_OK) return rc;
     // A4: candidates grouped by (view, frame)
     EMU_CK(cudaMemsetAsync(W.view_ovf_cnt, 0, (3 * (size_t)nv + 1) * sizeof(unsigned), st));
-    EMU_LAUNCH(EMU_STAGE_CANDS, st, k_cands<0><<<dim3(16, 3 * nv), 256, 0, st>>>(
+    const int gx = (int)emu_max64(16, emu_min64(512, (4 * kSM + 3 * nv - 1) / (3 * nv)));   // blocks per (view, frame): few views still fill the GPU
+    EMU_LAUNCH(EMU_STAGE_CANDS, st, k_cands<0><<<dim3(gx, 3 * nv), 256, 0, st>>>(
         P, v0, W.ctl, W.view_seed_off, W.seed_cnt, W.geo, W.ab, W.view_cand_cnt, nullptr, W.view_ovf_cnt, nullptr,
         nullptr, nullptr, nullptr, nullptr, counts));
     EMU_LAUNCH(EMU_STAGE_CANDS, st, k_chunk_offsets<<<1, 1024, 0, st>>>(
@@ -2062,7 +2098,7 @@ int emu_find_launch(const EmuDev& P, int seeds_per_grain, int cand_per_grain, co
         W.ctl, counts, -1, -1));
     EMU_CK(cudaMemsetAsync(W.view_cand_cnt, 0, (3 * (size_t)nv + 1) * sizeof(unsigned), st));
     EMU_CK(cudaMemsetAsync(W.view_ovf_cnt, 0, (3 * (size_t)nv + 1) * sizeof(unsigned), st));
-    EMU_LAUNCH(EMU_STAGE_CANDS, st, k_cands<1><<<dim3(16, 3 * nv), 256, 0, st>>>(
+    EMU_LAUNCH(EMU_STAGE_CANDS, st, k_cands<1><<<dim3(gx, 3 * nv), 256, 0, st>>>(
         P, v0, W.ctl, W.view_seed_off, W.seed_cnt, W.geo, W.ab, W.view_cand_cnt, W.view_cand_off, W.view_ovf_cnt,
         W.view_ovf_off, W.cands, W.cand_seed, W.ovf_geo, W.ovf_ci, counts));
     // generic fallback for the whole chunk (returns at once unless the brick plan failed)
@@ -2074,10 +2110,10 @@ int emu_find_launch(const EmuDev& P, int seeds_per_grain, int cand_per_grain, co
     // A5
     auto walk_kernel = P.ext >= 0 ? k_brick<kAssoc, true> : k_brick<kAssoc, false>;
     EMU_CK(cudaFuncSetAttribute(walk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kPoolBytes));
-    EMU_LAUNCH(EMU_STAGE_ASSOC, st, k_assoc_hits<<<dim3(48, 3 * nv), 256, 0, st>>>(
+    EMU_LAUNCH(EMU_STAGE_ASSOC, st, k_assoc_hits<<<dim3(emu_max64(48, gx), 3 * nv), 256, 0, st>>>(
         v0, W.ctl, W.view_cand_off, W.cands, W.cand_seed, W.seed_cnt, W.recs, W.slot_row, W.vf_brick_base, W.keyA, W.keyB));
     EMU_LAUNCH(EMU_STAGE_ASSOC, st, walk_kernel<<<kSM, kBrickThreads, kPoolBytes, st>>>(
-        P, F, v0, W.bricks, W.ctl, slices_walk, W.ovf_geo, W.ovf_ci, W.view_ovf_off, nullptr, nullptr, nullptr, nullptr, nullptr, W.keyA, W.keyB,
+        P, F, v0, W.bricks, W.ctl, slices_walk, W.ovf_geo, W.ovf_ci, W.view_ovf_off, nullptr, nullptr, 1, nullptr, nullptr, nullptr, W.keyA, W.keyB,
         counts));
     EMU_LAUNCH(EMU_STAGE_ASSOC, st, k_assoc_generic<0><<<kSM * 16, kVoteThreads, 0, st>>>(
         P, sorted, d_cell_start, W.bbox, v0, W.cands, W.ctl, W.tie_bits, W.keyA, W.keyB, W.owner));
@@ -2095,7 +2131,7 @@ int emu_find_launch(const EmuDev& P, int seeds_per_grain, int cand_per_grain, co
       EMU_LAUNCH(EMU_STAGE_SELECT, st, k_cut_compact<<<grid_for(nv, 1, kSM * 8), 256, 0, st>>>(P, nv, W.ctl, W.view_ntracks, W.view_tracks));
     }
     EMU_LAUNCH(EMU_STAGE_EMIT, st, k_track_scan<<<1, 1024, 0, st>>>(P, v0, v1, W.view_ntracks, d_track_off));
-    EMU_LAUNCH(EMU_STAGE_EMIT, st, k_track_emit<<<grid_for(nv, 1, kSM * 8), 256, 0, st>>>(
+    EMU_LAUNCH(EMU_STAGE_EMIT, st, k_track_emit<<<dim3((unsigned)emu_max64(1, emu_min64(16, (2 * kSM + nv - 1) / nv)), (unsigned)emu_min64(nv, 65535)), 256, 0, st>>>(
         P, sorted, v0, v1, W.cands, W.wins, W.view_ntracks, W.view_tracks, d_track_off, d_tracks, W.cand_track));
     // the per-track fill cursors reuse view_tracks (its contents are dead after k_track_emit)
     EMU_LAUNCH(EMU_STAGE_EMIT, st, k_member_scan<<<1, 1024, 0, st>>>(v0, v1, d_track_off, d_tracks, (int*)W.view_tracks, counts, members_capacity));
@@ -2126,7 +2162,7 @@ int emu_count_seeds_launch(const EmuDev& P, int seeds_per_grain, int cand_per_gr
   rc = prepare_frames(P, W, F, d_sorted, d_cell_start, d_view_off, n_grains, n_views, kSM, st);
   if (rc != EMU_OK) return rc;
   if (n_views > 0) {
-    rc = vote_chunk(P, TT, W, F, d_view_off, n_grains, 0, n_views, choose_slices(TT, n_views, kSM, EMU_ITEMS_PER_SM), kSM, counts, st);
+    rc = vote_chunk(P, TT, W, F, d_view_off, n_grains, 0, n_views, choose_slices(TT, n_views, kSM, EMU_ITEMS_PER_SM, n_grains, 64), kSM, counts, st);
     if (rc != EMU_OK) return rc;
     EMU_LAUNCH(EMU_STAGE_CANDS, st, k_seed_dump<<<dim3(64, 3 * n_views), 256, 0, st>>>(
         0, W.ctl, sorted, W.view_seed_off, W.seed_cnt, W.ab, (int4*)d_seed_dump, dump_capacity));

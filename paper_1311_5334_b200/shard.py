@@ -16,18 +16,37 @@ def view_range(rank: int, world: int, views_per_rank: int):
     return rank * views_per_rank, views_per_rank
 
 
-def split_views(n_views: int, world: int):
-    """Strong-scaling split of n_views over `world` ranks: contiguous ranges whose sizes differ by at most one.
-    Returns the list of (first, n) per rank."""
+def split_views(n_views: int, world: int, grains_per_view=None):
+    """Strong-scaling split of n_views over `world` ranks: contiguous ranges, returned as the list of (first, n) per
+    rank.  Without grain counts the sizes differ by at most one.  With `grains_per_view` (length n_views) the ranges
+    are balanced by sum N^2 instead (the work of a view goes with its seeds, i.e. with N times the grain
+    density): the cut after rank r is placed where the running sum of N^2 comes closest to (r + 1) / world of the total,
+    every rank keeping at least one view while views are left."""
     if world < 1 or n_views < 0:
         raise ValueError("bad world / n_views")
-    base, extra = divmod(n_views, world)
-    out, first = [], 0
-    for r in range(world):
-        n = base + (1 if r < extra else 0)
-        out.append((first, n))
-        first += n
-    return out
+    if grains_per_view is None:
+        base, extra = divmod(n_views, world)
+        out, first = [], 0
+        for r in range(world):
+            n = base + (1 if r < extra else 0)
+            out.append((first, n))
+            first += n
+        return out
+    w = np.asarray(grains_per_view, np.float64) ** 2
+    if len(w) != n_views:
+        raise ValueError("grains_per_view must have one entry per view")
+    cum = np.concatenate(([0.0], np.cumsum(w)))
+    cuts = [0]
+    for r in range(1, world):
+        lo = min(n_views, cuts[-1] + 1) if n_views - cuts[-1] > world - r else cuts[-1] + (1 if cuts[-1] < n_views else 0)
+        hi = max(lo, n_views - (world - r)) if n_views >= world else n_views
+        target = cum[-1] * r / world
+        k = int(np.searchsorted(cum, target))
+        if k > 0 and abs(cum[k - 1] - target) <= abs(cum[min(k, n_views)] - target):
+            k -= 1
+        cuts.append(int(min(max(k, lo), hi)))
+    cuts.append(n_views)
+    return [(cuts[r], cuts[r + 1] - cuts[r]) for r in range(world)]
 
 
 def _dist():

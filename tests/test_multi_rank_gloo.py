@@ -55,6 +55,21 @@ def test_split_views_covers_everything():
         assert sum(k for _, k in parts) == n
         assert all(parts[i][0] + parts[i][1] == parts[i + 1][0] for i in range(w - 1))
         assert max(k for _, k in parts) - min(k for _, k in parts) <= 1
+    # balanced by sum N^2: one dense view weighs as much as four views of half its grains
+    n = [100] * 8 + [200] * 2
+    parts = shard.split_views(10, 2, n)
+    assert parts == [(0, 8), (8, 2)]
+    assert sum(k for _, k in parts) == 10
+    for nv, w in ((7, 3), (3, 5), (64, 8)):
+        rng = np.random.default_rng(nv)
+        g = rng.integers(1000, 70000, nv)
+        parts = shard.split_views(nv, w, g)
+        assert len(parts) == w and parts[0][0] == 0 and sum(k for _, k in parts) == nv
+        assert all(parts[i][0] + parts[i][1] == parts[i + 1][0] for i in range(w - 1))
+        if nv >= w:
+            assert all(k >= 1 for _, k in parts)
+            loads = [float((g[a:a + k].astype(float) ** 2).sum()) for a, k in parts]
+            assert max(loads) <= sum(loads) / w + float(g.max()) ** 2          # within one view of the ideal share
     assert shard.view_range(3, 8, 128) == (384, 128)
     with pytest.raises(ValueError):
         shard.view_range(8, 8, 1)
