@@ -282,6 +282,9 @@ k_seed_pairs(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ 
     const int czb = emu_cell_axis(A.z + P.sep_max, P.cs[2], P.inv_cs[2], P.n[2]);
     const int ny = cyb - cya + 1, n_rows = ny * (czb - czA + 1);
     const float inv_ny = 1.0f / (float)ny;
+    // the rows of A's own layer that lie before A's row hold only grains before A in sorted order: not dealt out
+    // (66 rows -> 61 on the bench grid: two rounds of 32 lanes instead of three)
+    const int r_first = emu_cell_axis(A.y, P.cs[1], P.inv_cs[1], P.n[1]) - cya;
     unsigned n[3] = {0u, 0u, 0u};
     unsigned base[3] = {0u, 0u, 0u};
     if (kFill) {
@@ -290,7 +293,7 @@ k_seed_pairs(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ 
       if (lane < 3) cur_s[wib][lane] = 0u;
       __syncwarp();
     }
-    for (int r = lane; r < n_rows; r += 32) {
+    for (int r = r_first + lane; r < n_rows; r += 32) {
       const int lz = (int)(((float)r + 0.5f) * inv_ny);              // r / ny (small integers: exact)
       const int cz = czA + lz, cy = cya + (r - lz * ny);
       const int rb = vbase + (cz * P.n[1] + cy) * P.n[0];
