@@ -32,15 +32,16 @@ CFG = 4                          # BASELINE.json configs[4] "throughput batch"
 CELL_UM = (3.0, 4.0, 4.0)        # cell size of the 3D hash (a pure speed knob: no effect on the track list)
 VIEW_AREA_CM2 = 350e-4 * 300e-4  # 350 x 300 um = 1.05e-3 cm^2 per view
 # Algorithmic work of the voting kernel: lane-instructions per seed
-#   = tests/seed * 18 + pair-tests/seed * 9, with tests/seed and pair-tests/seed the ORACLE's own counters
+#   = tests/seed * 18 + pair-tests/seed * 10, with tests/seed and pair-tests/seed the ORACLE's own counters
 # (oracle mode "cells", same cell size) on views 0..7 of this workload.  The cpu_baseline leg re-measures
 # them live; the constants serve the runs that have no such leg (N > 1).
 ALG_PER_SEED = {(8.0, 8.0, 8.0): (317.7, 2.88), (3.0, 4.0, 4.0): (102.1, 2.26)}
-INSTR_PER_TEST, INSTR_PER_PAIR = 18, 9
+INSTR_PER_TEST, INSTR_PER_PAIR = 18, 10    # read off the SASS: profiles/r2_sass_counts.md
+MIX_PEAK_SHARE = 99.3 / 128.0    # measured issue rate of the tube-test instruction mix / nominal issue rate (mb_pipes.cu)
 BIN_BYTES_PER_GRAIN = 32.0       # 16 B read + 16 B written per grain; + 4 B per cell of the grid
 # DRAM bytes (read + write) of one k_brick<kVote> launch per view of the launch, from the committed ncu --set full
-# capture profiles/r1e_k_brick_full.txt (16 views: 20.98 GB read + 13.90 GB written)
-VOTE_DRAM_BYTES_PER_VIEW = (20.978974e9 + 13.904418e9) / 16
+# capture profiles/r2_k_brick_full.txt (33 views: 50.48 GB read + 28.71 GB written)
+VOTE_DRAM_BYTES_PER_VIEW = (50.480965e9 + 28.710393e9) / 33
 # DRAM bytes of the two binning kernels per grain, from profiles/r1e_k_bin_full.txt (65 792 077 grains:
 # k_bin_split 1.053 + 1.006 GB, k_bin_chunk 1.055 + 1.457 GB)
 BIN_DRAM_BYTES_PER_GRAIN = (1.053481e9 + 1.005627e9 + 1.055078e9 + 1.456763e9) / 65792077
@@ -378,13 +379,16 @@ def main():
         views_per_launch = V * args.steps / stage_launches["vote"]
         captured = tuple(CELL_UM) == (3.0, 4.0, 4.0) and TUBE_EXT_Q < 0     # the configuration of the committed ncu capture
         gpu_tests = float(counts[E.EMU_CNT["tests"]]) / max(1, seeds)
-        roofline = {"kernel": "k_brick<kVote> (A2 seeds are streamed in, A3 tube count + hit records, shared-memory bricks, "
-                              "three frames)", "bound": "alu", "achieved": achieved, "peak": alu_peak,
+        roofline = {"kernel": "k_brick<kVote> (A3 tube count + hit records on shared-memory bricks, three frames; the seeds of "
+                              "A2 arrive as per-brick lists of prepared records)", "bound": "alu", "achieved": achieved, "peak": alu_peak,
                     "unit": "Tlane-instr/s", "frac": achieved / alu_peak,
+                    "frac_of_mix_peak": achieved / (alu_peak * MIX_PEAK_SHARE),
+                    "mix_peak_source": "profiles/r2_mb_pipes.md: the tube-test instruction mix sustains 99.3 of 128 "
+                                       "lane-instr per clock and SM",
                     "frac_on_kernel_tests": achieved / alu_peak * (gpu_tests * INSTR_PER_TEST + alg[1] * INSTR_PER_PAIR)
                                             / (alg[0] * INSTR_PER_TEST + alg[1] * INSTR_PER_PAIR),
                     "traffic": VOTE_DRAM_BYTES_PER_VIEW * views_per_launch if captured else None,
-                    "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of profiles/r1e_k_brick_full.txt per view "
+                    "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of profiles/r2_k_brick_full.txt per view "
                                       "x views per launch",
                     "peak_source": f"148 SM x 4 schedulers x 32 lanes x {sm_max:.0f} MHz ({peaks['_source']} max SM clock)",
                     "algorithmic": f"{seeds} seeds x ({alg[0]:.1f} tests x {INSTR_PER_TEST} + {alg[1]:.2f} pair tests x "
