@@ -337,7 +337,7 @@ constexpr int kSplitPer = EMU_SPLIT_PER;                         // grains per t
 #endif
 constexpr int kChunkThreads = EMU_CHUNK_THREADS;
 constexpr int kChunkPer = EMU_CHUNK_PER;                         // grains per thread of a chunk block (held in registers)
-constexpr int kChunkCap = kChunkThreads * kChunkPer; // grains of a chunk: 1 536 = 24 KB of shared memory
+constexpr int kChunkCap = kChunkThreads * kChunkPer; // grains of a chunk: 2 560 = 40 KB of shared memory
 constexpr int kMaxChunks = 128;
 constexpr int kMaxChunkCells = 12288;                // cells of a chunk: 2 x 16 bits each in shared memory
 
@@ -410,7 +410,12 @@ k_bin_split(EmuDev P, int frame, SplitPlan S, const int4* __restrict__ grains, c
   if (status && __any_sync(EMU_FULL, bad) && (tid & 31) == 0) atomicOr(status, (unsigned long long)EMU_ST_COORD);
 }
 
-__global__ void __launch_bounds__(kChunkThreads)
+// 1: pass 2 stores every grain straight to its place instead of staging the chunk in shared memory and streaming it
+// out (one barrier and 39 KB of shared memory less; 1.154 -> 1.126 ms on the bench; more blocks per SM only spill)
+#ifndef EMU_BIN_DIRECT
+#define EMU_BIN_DIRECT 1
+#endif
+__global__ void __launch_bounds__(kChunkThreads, EMU_CHUNK_MINB)
 k_bin_chunk(EmuDev P, int frame, SplitPlan S, const int* __restrict__ view_off, int n_views, int n_grains, int v_first,
             const int4* __restrict__ tmp, const int* __restrict__ cur, const int* __restrict__ redo,
             int4* __restrict__ sorted, int* __restrict__ cell_start) {
@@ -424,8 +429,12 @@ k_bin_chunk(EmuDev P, int frame, SplitPlan S, const int* __restrict__ view_off, 
   if (redo[v]) return;
   const int c_lo = k * S.cpc, nc = min(ncell, c_lo + S.cpc) - c_lo;
   if (nc <= 0) return;
+#if EMU_BIN_DIRECT
+  unsigned short* cnt = reinterpret_cast<unsigned short*>(chunk_smem);                // [cpc] counts
+#else
   int4* buf = reinterpret_cast<int4*>(chunk_smem);                                   // [cap]
   unsigned short* cnt = reinterpret_cast<unsigned short*>(chunk_smem + (size_t)S.cap * 16);   // [cpc] counts
+#endif
   unsigned short* pre = cnt + ((S.cpc + 1) & ~1);                                    // [cpc] exclusive prefix
   unsigned* cntw = reinterpret_cast<unsigned*>(cnt);
   int* wbuf = reinterpret_cast<int*>(pre + ((S.cpc + 1) & ~1));                      // [cap] rows in arrival order
@@ -493,10 +502,16 @@ k_bin_chunk(EmuDev P, int frame, SplitPlan S, const int* __restrict__ view_off, 
     const int m = cnt[cc[u]], p0 = pre[cc[u]];
     int r = 0;
     if (m >= 2) for (int t = 0; t < m; ++t) r += (wbuf[p0 + t] < gg[u].w);
+#if EMU_BIN_DIRECT
+    sorted[base + p0 + r] = gg[u];                     // straight to its place (the L2 merges the 16-byte stores of a chunk)
+#else
     buf[p0 + r] = gg[u];
+#endif
   }
+#if !EMU_BIN_DIRECT
   __syncthreads();
   for (int i = tid; i < n; i += kChunkThreads) sorted[base + i] = buf[i];
+#endif
 }
 
 // plan of the two-pass path for one frame; K = 0: not applicable (the one-kernel paths take over)
@@ -505,7 +520,7 @@ SplitPlan split_plan(const EmuDev& P, int frame, int64_t n_grains, int32_t n_vie
   const int ncell = P.fr[frame].ncell;
   if (n_views < 1 || n_grains < 1 || ncell >= (1 << 24)) return S;
   const double avg = (double)n_grains / n_views;
-  // the fewest chunks whose scratch region (1.6 x the average chunk + 256) fits the shared-memory buffer
+  // the fewest chunks whose scratch region (EMU_CHUNK_SLACK = 1.3 x the average chunk + 256) fits the shared-memory buffer
   int K = (int)emu_max64(1, (int64_t)(avg * EMU_CHUNK_SLACK / (double)(kChunkCap - 256 - 64)) + 1);
   K = (int)emu_max64(K, ((int64_t)ncell + kMaxChunkCells - 1) / kMaxChunkCells);
   if (K > kMaxChunks) return S;
@@ -569,7 +584,7 @@ int emu_bin_launch(const EmuDev& P, int frame, const int32_t* d_grains, const in
   const SplitPlan S = split_plan(P, frame, n_grains, n_views);
   if (S.K > 0) {
     // two passes: split into chunks of cells, then one chunk per block in shared memory
-    const size_t smem = (size_t)S.cap * 16 + 2 * (size_t)((S.cpc + 1) & ~1) * sizeof(unsigned short) + (size_t)S.cap * 4;
+    const size_t smem = (EMU_BIN_DIRECT ? 0 : (size_t)S.cap * 16) + 2 * (size_t)((S.cpc + 1) & ~1) * sizeof(unsigned short) + (size_t)S.cap * 4;
     if (cudaFuncSetAttribute(k_bin_chunk, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return EMU_ERR_CUDA;
     if (cudaMemsetAsync(redo, 0, ((size_t)n_views + 1) * sizeof(int), st) != cudaSuccess) return EMU_ERR_CUDA;
     if (cudaMemsetAsync(cur, 0, (size_t)n_views * S.K * sizeof(int), st) != cudaSuccess) return EMU_ERR_CUDA;

@@ -375,9 +375,10 @@ k_view_scan(const int* __restrict__ view_off, int v0, int v1, unsigned* __restri
       }
       __syncthreads();
       const unsigned carry = carry_s;
-      const unsigned mine = carry + warp_sum[wid] + incl;
+      const unsigned long long mine64 = (unsigned long long)carry + warp_sum[wid] + incl;   // (a tile of 1 024 grains stays far below 2^32)
+      const unsigned mine = (unsigned)mine64;
       if (g < g1) {
-        if (mine < carry) atomicOr(counts + EMU_CNT_STATUS, (unsigned long long)EMU_ST_SEED_OVERFLOW);  // >= 2^32 seeds in a view
+        if (mine64 > 0xffffffffull) atomicOr(counts + EMU_CNT_STATUS, (unsigned long long)EMU_ST_SEED_OVERFLOW);  // >= 2^32 seeds in a (view, frame)
         seed_off[g] = mine - x;
       }
       __syncthreads();

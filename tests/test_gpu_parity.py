@@ -38,7 +38,10 @@ def _mess_up(g, size_q):
 @pytest.mark.parametrize("cfg,cell_um,messy", [(0, (8.0, 8.0, 8.0), False), (0, (3.0, 17.0, 5.5), True),
                                                (1, (8.0, 8.0, 8.0), False), (1, (4.0, 4.0, 4.0), True),
                                                (3, (40.0, 2.0, 60.0), False), (0, (200.0, 200.0, 100.0), False),
-                                               (1, (3.0, 4.0, 4.0), False)])
+                                               (1, (3.0, 4.0, 4.0), False),
+                                               # 400 x 400 x 200 = 32 M cells per view (>= 2^24): neither the two-pass plan nor the
+                                               # shared-memory counters can hold the grid: the four-kernel counting sort
+                                               (0, (0.25, 0.25, 0.25), True)])
 def test_binning_bit_exact(E, oracle_mod, cfg, cell_um, messy):
     b = make_batch(CONFIGS[cfg], cfg, n_views=3 if cfg == 0 else 1)
     p = default_params(cfg, cell_um=cell_um)
