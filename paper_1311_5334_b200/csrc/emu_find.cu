@@ -58,10 +58,10 @@ constexpr int kMaxTube = 8191;                    // n_tube field of the packed 
 #define EMU_BODY_REPS 2
 #endif
 #ifndef EMU_REFILL
-#define EMU_REFILL 10
+#define EMU_REFILL 8
 #endif
 #ifndef EMU_REFILL_STOP
-#define EMU_REFILL_STOP 6
+#define EMU_REFILL_STOP 4
 #endif
 constexpr int kBrickThreads = EMU_BRICK_THREADS;  // one persistent block per SM
 constexpr int kPoolBytes = 222 * 1024;            // dynamic shared memory of a brick: grains | row table | cell table
