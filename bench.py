@@ -40,8 +40,8 @@ INSTR_PER_TEST, INSTR_PER_PAIR = 18, 10    # read off the SASS: profiles/r2_sass
 MIX_PEAK_SHARE = 99.3 / 128.0    # measured issue rate of the tube-test instruction mix / nominal issue rate (mb_pipes.cu)
 BIN_BYTES_PER_GRAIN = 32.0       # 16 B read + 16 B written per grain; + 4 B per cell of the grid
 # DRAM bytes (read + write) of one k_brick<kVote> launch per view of the launch, from the committed ncu --set full
-# capture profiles/r2_k_brick_full.txt (33 views: 50.48 GB read + 28.71 GB written)
-VOTE_DRAM_BYTES_PER_VIEW = (50.480965e9 + 28.710393e9) / 33
+# capture profiles/r2_k_brick_full.txt (33 views: 50.48 GB read + 28.86 GB written)
+VOTE_DRAM_BYTES_PER_VIEW = (50.478269e9 + 28.861403e9) / 33
 # DRAM bytes of the two binning kernels per grain, from profiles/r1e_k_bin_full.txt (65 792 077 grains:
 # k_bin_split 1.053 + 1.006 GB, k_bin_chunk 1.055 + 1.457 GB)
 BIN_DRAM_BYTES_PER_GRAIN = (1.053481e9 + 1.005627e9 + 1.055078e9 + 1.456763e9) / 65792077
