@@ -535,7 +535,7 @@ SplitPlan split_plan(const EmuDev& P, int frame, int64_t n_grains, int32_t n_vie
 // group; with groups that fit the L2 the round trip through the scratch could stay on chip.  Measured on the bench
 // (1 024 views): one group 1.14 ms; groups of 128 / 96 / 64 / 48 / 32 / 16 MB: 1.34 / 1.40 / 1.50 / 1.56 / 1.71 / 2.31 ms -
 // the tail of every small launch costs more than the traffic saves, so the default is ONE group (the hook stays for
-// the record; gpurun_out/r2b_bin_sweep.txt).
+// the record).
 #ifndef EMU_BIN_GROUP_MB
 #define EMU_BIN_GROUP_MB (1 << 20)
 #endif
