@@ -42,9 +42,9 @@ BIN_BYTES_PER_GRAIN = 32.0       # 16 B read + 16 B written per grain; + 4 B per
 # DRAM bytes (read + write) of one k_brick<kVote> launch per view of the launch, from the committed ncu --set full
 # capture profiles/r2_k_brick_full.txt (33 views: 50.48 GB read + 28.86 GB written)
 VOTE_DRAM_BYTES_PER_VIEW = (50.478269e9 + 28.861403e9) / 33
-# DRAM bytes of the two binning kernels per grain, from profiles/r1e_k_bin_full.txt (65 792 077 grains:
-# k_bin_split 1.053 + 1.006 GB, k_bin_chunk 1.055 + 1.457 GB)
-BIN_DRAM_BYTES_PER_GRAIN = (1.053481e9 + 1.005627e9 + 1.055078e9 + 1.456763e9) / 65792077
+# DRAM bytes of the two binning kernels per grain, from profiles/r2_k_bin_full.txt (65 792 077 grains:
+# k_bin_split 1.055 + 1.004 GB, k_bin_chunk 1.061 + 1.467 GB)
+BIN_DRAM_BYTES_PER_GRAIN = (1.054695e9 + 1.003755e9 + 1.060990e9 + 1.466883e9) / 65792077
 
 
 def _gen_view(v):
@@ -406,7 +406,7 @@ def main():
     bin_gbs = bin_bytes / (bin_ms * 1e-3) / 1e9 if bin_ms > 0 else 0.0
     roofline_bin = {"kernel": "emu_bin_grains: k_bin_split + k_bin_chunk (two passes: chunks of cells through a scratch array, then one chunk per block in shared memory)", "bound": "hbm",
                     "achieved": bin_gbs, "peak": hbm, "unit": "GB/s", "frac": bin_gbs / hbm,
-                    "traffic": BIN_DRAM_BYTES_PER_GRAIN * n if tuple(CELL_UM) == (3.0, 4.0, 4.0) else None, "traffic_source": "profiles/r1e_k_bin_full.txt, both passes, per grain x grains",
+                    "traffic": BIN_DRAM_BYTES_PER_GRAIN * n if tuple(CELL_UM) == (3.0, 4.0, 4.0) else None, "traffic_source": "profiles/r2_k_bin_full.txt, both passes, per grain x grains",
                     "algorithmic_bytes": bin_bytes, "ms": bin_ms,
                     "algorithmic_bytes_per_grain": bin_bytes / max(1, n),
                     "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peaks['_source']})"}
