@@ -1218,9 +1218,16 @@ k_assoc_hits(int v0, const FindCtl* __restrict__ ctl, const unsigned* __restrict
       const int slot = (int)((w[k >> 1] >> (16 * (k & 1))) & 0xffffu);
       rows[k] = k < cnt ? slot_row[base + slot] : -1;
     }
+    // A grain is hit by hundreds of candidates and only the few that raise its maximum matter: look first (a plain
+    // load that may be stale - the keys only grow, so an old value can cause a needless atomic, never a missing one) and
+    // join the maximum only if this candidate's (n_tube, D2) is not already beaten.  Equal (n_tube, D2) must go on:
+    // that is the tie the two keys exist to detect.
+    unsigned long long seen[kRecSlots];
+#pragma unroll
+    for (int k = 0; k < kRecSlots; ++k) seen[k] = rows[k] >= 0 ? __ldcg(keyA + rows[k]) : ~0ull;
 #pragma unroll
     for (int k = 0; k < kRecSlots; ++k) {
-      if (rows[k] >= 0) { atomicMax(keyA + rows[k], ka); atomicMax(keyB + rows[k], kb); }
+      if (rows[k] >= 0 && (seen[k] >> kCiBits) <= k1) { atomicMax(keyA + rows[k], ka); atomicMax(keyB + rows[k], kb); }
     }
   }
 }
