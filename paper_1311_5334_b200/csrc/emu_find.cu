@@ -443,7 +443,8 @@ k_clear_seed_cnt(const FindCtl* __restrict__ ctl, unsigned long long* __restrict
   const size_t n = ctl->seed_count;
   ulonglong2* p2 = reinterpret_cast<ulonglong2*>(seed_cnt);
   const size_t stride = (size_t)gridDim.x * blockDim.x;
-  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; 2 * i < n; i += stride) p2[i] = make_ulonglong2(0ull, 0ull);
+  for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; 2 * i + 1 < n; i += stride) p2[i] = make_ulonglong2(0ull, 0ull);
+  if ((n & 1) && blockIdx.x == 0 && threadIdx.x == 0) seed_cnt[n - 1] = 0ull;
 }
 
 // ---------------------------------------------------------------------------------------------

@@ -126,9 +126,11 @@ k_recog(Recog R, const unsigned char* __restrict__ vox, int n_views, int* __rest
   };
 
   for (long long row = warp0; row < n_rows; row += n_warps) {
-    const int view = (int)(row / rows_per_view);
-    const int zy = (int)(row - (long long)view * rows_per_view);
-    const int z = zy / R.ny, y = zy - z * R.ny;
+    // (n_rows < 2^31 is checked by the C ABI: 32-bit divisions)
+    const unsigned urow = (unsigned)row, rpv = (unsigned)rows_per_view;
+    const int view = (int)(urow / rpv);
+    const unsigned zy = urow - (unsigned)view * rpv;
+    const int z = (int)(zy / (unsigned)R.ny), y = (int)(zy - (unsigned)z * (unsigned)R.ny);
     const unsigned char* line = vox + (size_t)view * rows_per_view * R.nx + ((size_t)z * R.ny + y) * R.nx;
     const unsigned long long tag = ((unsigned long long)(unsigned)y << 16) | ((unsigned long long)(unsigned)z << 32) | ((unsigned long long)(unsigned)view << 48);
 
@@ -160,15 +162,16 @@ k_recog(Recog R, const unsigned char* __restrict__ vox, int n_views, int* __rest
       if (lane == 31) right_in = next_first;
       prev_last = __shfl_sync(EMU_FULL, cur.w >> 24, 31);
       // per byte: above the threshold, higher than the left neighbour, at least as high as the right one
-      unsigned mk[4];
-      int cnt = 0;
+      // (one bit per voxel of my 16: the 0x01 bytes of a word are gathered into four bits by a multiply)
+      unsigned m16 = 0u;
 #pragma unroll
       for (int w = 0; w < 4; ++w) {
         const unsigned lf = __funnelshift_l(w ? q[w - 1] : (left_in << 24), q[w], 8);
         const unsigned rt = __funnelshift_r(q[w], w < 3 ? q[w + 1] : right_in, 8);
-        mk[w] = __vcmpgtu4(q[w], thr4) & __vcmpgtu4(q[w], lf) & __vcmpgeu4(q[w], rt) & 0x01010101u;
-        cnt += __popc(mk[w]);
+        const unsigned mk = __vsetgtu4(q[w], thr4) & __vsetgtu4(q[w], lf) & __vsetgeu4(q[w], rt);   // 0x01 per byte that passes
+        m16 |= ((mk * 0x01020408u) >> 24) << (4 * w);
       }
+      const int cnt = __popc(m16);
       // x order: lanes in order, voxels of a lane in order.  A lane rarely holds more than one or two survivors, so the
       // exclusive prefix over the lanes is a sum of ballots ("at least k survivors") rather than a shuffle scan
       unsigned any = __ballot_sync(EMU_FULL, cnt > 0);
@@ -180,13 +183,9 @@ k_recog(Recog R, const unsigned char* __restrict__ vox, int n_views, int* __rest
         any = __ballot_sync(EMU_FULL, cnt > k);
       }
       int at = head + qn + excl;
-      if (cnt) {
-#pragma unroll
-        for (int w = 0; w < 4; ++w)
-          for (unsigned m = mk[w]; m; m &= m - 1u) {            // the set bits in ascending order = ascending x
-            ring[at & (kRing - 1)] = tag | (unsigned long long)(unsigned)(x + 4 * w + ((__ffs((int)m) - 1) >> 3));
-            ++at;
-          }
+      for (; m16; m16 &= m16 - 1u) {                            // the set bits in ascending order = ascending x
+        ring[at & (kRing - 1)] = tag | (unsigned long long)(unsigned)(x + __ffs((int)m16) - 1);
+        ++at;
       }
       qn += total;
       while (qn >= 32) flush(32);
