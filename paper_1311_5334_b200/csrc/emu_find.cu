@@ -297,8 +297,19 @@ k_seed_pairs(EmuDev P, const int4* __restrict__ sorted, const int* __restrict__ 
       const int lz = (int)(((float)r + 0.5f) * inv_ny);              // r / ny (small integers: exact)
       const int cz = czA + lz, cy = cya + (r - lz * ny);
       const int rb = vbase + (cz * P.n[1] + cy) * P.n[0];
-      int s = __ldg(cell_start + rb + cxa);
-      const int e = __ldg(cell_start + rb + cxb + 1);
+      // Only the chord of the separation sphere in this row: a grain of row (cy, cz) is at least dy_min, dz_min away
+      // from A in y and z (the outer side of a boundary row is open: grains outside the box are clamped into it), so a
+      // partner has dx^2 < sep_max^2 - dy_min^2 - dz_min^2.  The box of rows holds about twice the pairs the sphere does.
+      const int ylo = cy == 0 ? -0x40000000 : cy * P.cs[1], yhi = cy == P.n[1] - 1 ? 0x40000000 : (cy + 1) * P.cs[1] - 1;
+      const int zlo = cz == 0 ? -0x40000000 : cz * P.cs[2], zhi = cz == P.n[2] - 1 ? 0x40000000 : (cz + 1) * P.cs[2] - 1;
+      const float dym = (float)max(0, max(ylo - A.y, A.y - yhi)), dzm = (float)max(0, max(zlo - A.z, A.z - zhi));
+      const float rx2 = (float)P.sep_max2 - dym * dym - dzm * dzm;     // exact: every term below 2^24
+      if (rx2 <= 0.0f) continue;
+      const int rx = (int)sqrtf(rx2) + 2;                              // (sqrt within 1 of the truth, one more for the strict <)
+      const int cxa_r = emu_cell_axis(A.x - rx, P.cs[0], P.inv_cs[0], P.n[0]);
+      const int cxb_r = emu_cell_axis(A.x + rx, P.cs[0], P.inv_cs[0], P.n[0]);
+      int s = __ldg(cell_start + rb + cxa_r);
+      const int e = __ldg(cell_start + rb + cxb_r + 1);
       s = max(s, a + 1);
       for (int j0 = s; j0 < e; j0 += 4) {
        int4 Bq[4];
