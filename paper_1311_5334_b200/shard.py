@@ -35,16 +35,18 @@ def split_views(n_views: int, world: int, grains_per_view=None):
     w = np.asarray(grains_per_view, np.float64) ** 2
     if len(w) != n_views:
         raise ValueError("grains_per_view must have one entry per view")
-    cum = np.concatenate(([0.0], np.cumsum(w)))
+    cum = np.concatenate(([0.0], np.cumsum(w)))          # cum[k] = weight of views 0..k-1
     cuts = [0]
     for r in range(1, world):
-        lo = min(n_views, cuts[-1] + 1) if n_views - cuts[-1] > world - r else cuts[-1] + (1 if cuts[-1] < n_views else 0)
-        hi = max(lo, n_views - (world - r)) if n_views >= world else n_views
+        # the cut closest to r / world of the total weight ...
         target = cum[-1] * r / world
         k = int(np.searchsorted(cum, target))
-        if k > 0 and abs(cum[k - 1] - target) <= abs(cum[min(k, n_views)] - target):
+        if k > 0 and (k > n_views or target - cum[k - 1] <= cum[k] - target):
             k -= 1
-        cuts.append(int(min(max(k, lo), hi)))
+        # ... but at least one view for every rank before and after it while views are left
+        lo = min(cuts[-1] + 1, n_views)
+        hi = max(lo, n_views - (world - r))
+        cuts.append(min(max(k, lo), hi))
     cuts.append(n_views)
     return [(cuts[r], cuts[r + 1] - cuts[r]) for r in range(world)]
 
