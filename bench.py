@@ -413,123 +413,135 @@ def main():
 
     single = None
     if args.latency_views > 0:
-        # one view per host call (H2D + path + D2H inside), config 4 (the bench density) and config 1 (one microscope view)
-        from emu_synth import CONFIGS, default_params, make_view
-        single = {}
-        for cfg_i in (CFG, 1):
-            pp = default_params(cfg_i, cell_um=CELL_UM, max_tracks_per_view=4096)
-            pp["tube_ext_q"] = TUBE_EXT_Q
-            pr = E.make_params(**{k: pp[k] for k in ("view_size_q", "cell_size_q", "sep_min_q", "sep_max_q", "tube_r2_q",
-                                                      "min_grains", "max_tracks_per_view", "tube_ext_q")})
-            views = [make_view(CONFIGS[cfg_i], cfg_i, v)[0] for v in range(args.latency_views)]
-            nmax = max(len(g) for g in views)
-            H1 = E.HostPath(pr, nmax, 1)
-            ts = []
-            for rep_i in range(2):                                  # the first round warms up
-                for g in views:
-                    H1.n_grains = len(g)
-                    H1.h_grains[:len(g)].copy_(torch.from_numpy(g))
-                    H1.h_view_off.copy_(torch.tensor([0, len(g)], dtype=torch.int32))
-                    torch.cuda.synchronize()
-                    t0 = time.perf_counter()
-                    H1.call()
-                    if rep_i:
-                        ts.append((time.perf_counter() - t0) * 1e3)
-            single[f"config{cfg_i}"] = {"views": len(views), "grains_per_view": int(np.mean([len(g) for g in views])),
-                                        "ms_median": float(np.median(ts)), "ms_max": float(np.max(ts))}
-            del H1
+        try:
+            # one view per host call (H2D + path + D2H inside), config 4 (the bench density) and config 1 (one microscope view)
+            from emu_synth import CONFIGS, default_params, make_view
+            single = {}
+            for cfg_i in (CFG, 1):
+                pp = default_params(cfg_i, cell_um=CELL_UM, max_tracks_per_view=4096)
+                pp["tube_ext_q"] = TUBE_EXT_Q
+                pr = E.make_params(**{k: pp[k] for k in ("view_size_q", "cell_size_q", "sep_min_q", "sep_max_q", "tube_r2_q",
+                                                          "min_grains", "max_tracks_per_view", "tube_ext_q")})
+                views = [make_view(CONFIGS[cfg_i], cfg_i, v)[0] for v in range(args.latency_views)]
+                nmax = max(len(g) for g in views)
+                H1 = E.HostPath(pr, nmax, 1)
+                ts = []
+                for rep_i in range(2):                                  # the first round warms up
+                    for g in views:
+                        H1.n_grains = len(g)
+                        H1.h_grains[:len(g)].copy_(torch.from_numpy(g))
+                        H1.h_view_off.copy_(torch.tensor([0, len(g)], dtype=torch.int32))
+                        torch.cuda.synchronize()
+                        t0 = time.perf_counter()
+                        H1.call()
+                        if rep_i:
+                            ts.append((time.perf_counter() - t0) * 1e3)
+                single[f"config{cfg_i}"] = {"views": len(views), "grains_per_view": int(np.mean([len(g) for g in views])),
+                                            "ms_median": float(np.median(ts)), "ms_max": float(np.max(ts))}
+                del H1
+                torch.cuda.empty_cache()
+        except Exception as exc:                              # an extra leg may not take the headline down with it
+            single = {"error": f"{type(exc).__name__}: {exc}"}
             torch.cuda.empty_cache()
 
     stream = None
     if args.stream_views > 0 and world == 1:
-        # the same workload in batches through emu_stream_* (H2D of batch k+1 and D2H of batch k-1
-        # behind the kernels of batch k), and config-1 views one per batch as a microscope would deliver them
-        from emu_synth import CONFIGS, default_params, make_view
-        stream = {}
-        torch.cuda.empty_cache()
-        SV, BV = min(args.stream_views, V), args.stream_batch
-        nb = (SV + BV - 1) // BV
-        bounds = [(b * BV, min(SV, (b + 1) * BV)) for b in range(nb)]
-        S = E.StreamPath(prm, max(int(off[b1] - off[b0]) for b0, b1 in bounds), BV)
+        try:
+            # the same workload in batches through emu_stream_* (H2D of batch k+1 and D2H of batch k-1
+            # behind the kernels of batch k), and config-1 views one per batch as a microscope would deliver them
+            from emu_synth import CONFIGS, default_params, make_view
+            stream = {}
+            torch.cuda.empty_cache()
+            SV, BV = min(args.stream_views, V), args.stream_batch
+            nb = (SV + BV - 1) // BV
+            bounds = [(b * BV, min(SV, (b + 1) * BV)) for b in range(nb)]
+            S = E.StreamPath(prm, max(int(off[b1] - off[b0]) for b0, b1 in bounds), BV)
 
-        def batch(b):
-            b0, b1 = bounds[b]
-            return grains[off[b0]:off[b1]], (off[b0:b1 + 1] - off[b0]).astype(np.int32)
-        for rep_i in range(2):                                             # the first round warms up
-            torch.cuda.synchronize()
-            t0 = time.perf_counter()
-            nt_s = 0
-            S.submit(*batch(0))
-            for b in range(1, nb):
-                S.submit(*batch(b))
+            def batch(b):
+                b0, b1 = bounds[b]
+                return grains[off[b0]:off[b1]], (off[b0:b1 + 1] - off[b0]).astype(np.int32)
+            for rep_i in range(2):                                             # the first round warms up
+                torch.cuda.synchronize()
+                t0 = time.perf_counter()
+                nt_s = 0
+                S.submit(*batch(0))
+                for b in range(1, nb):
+                    S.submit(*batch(b))
+                    nt_s += S.collect(copy=False)["n_tracks"]
                 nt_s += S.collect(copy=False)["n_tracks"]
-            nt_s += S.collect(copy=False)["n_tracks"]
-            dt = time.perf_counter() - t0
-        assert SV < V or nt_s == int(counts[E.EMU_CNT["tracks"]]), "the streamed batches and the one-call path disagree"
-        stream["config4"] = {"views": SV, "views_per_batch": BV, "grains_per_s": float(off[SV]) / dt, "views_per_s": SV / dt,
-                             "ms_per_view": dt / SV * 1e3, "tracks": nt_s,
-                             "call": "emu_stream_submit / emu_stream_collect, two batches in flight, pinned host buffers"}
-        S.close(); del S
-        torch.cuda.empty_cache()
-        pp = default_params(1, cell_um=CELL_UM, max_tracks_per_view=4096)
-        pp["tube_ext_q"] = TUBE_EXT_Q
-        pr1 = E.make_params(**{k: pp[k] for k in ("view_size_q", "cell_size_q", "sep_min_q", "sep_max_q", "tube_r2_q",
-                                                   "min_grains", "max_tracks_per_view", "tube_ext_q")})
-        views = [make_view(CONFIGS[1], 1, v)[0] for v in range(32)]
-        offs = [np.asarray([0, len(g)], np.int32) for g in views]
-        S = E.StreamPath(pr1, max(len(g) for g in views), 1)
-        for rep_i in range(2):
-            torch.cuda.synchronize()
-            t0 = time.perf_counter()
-            S.submit(views[0], offs[0])
-            for b in range(1, len(views)):
-                S.submit(views[b], offs[b])
+                dt = time.perf_counter() - t0
+            assert SV < V or nt_s == int(counts[E.EMU_CNT["tracks"]]), "the streamed batches and the one-call path disagree"
+            stream["config4"] = {"views": SV, "views_per_batch": BV, "grains_per_s": float(off[SV]) / dt, "views_per_s": SV / dt,
+                                 "ms_per_view": dt / SV * 1e3, "tracks": nt_s,
+                                 "call": "emu_stream_submit / emu_stream_collect, two batches in flight, pinned host buffers"}
+            S.close(); del S
+            torch.cuda.empty_cache()
+            pp = default_params(1, cell_um=CELL_UM, max_tracks_per_view=4096)
+            pp["tube_ext_q"] = TUBE_EXT_Q
+            pr1 = E.make_params(**{k: pp[k] for k in ("view_size_q", "cell_size_q", "sep_min_q", "sep_max_q", "tube_r2_q",
+                                                       "min_grains", "max_tracks_per_view", "tube_ext_q")})
+            views = [make_view(CONFIGS[1], 1, v)[0] for v in range(32)]
+            offs = [np.asarray([0, len(g)], np.int32) for g in views]
+            S = E.StreamPath(pr1, max(len(g) for g in views), 1)
+            for rep_i in range(2):
+                torch.cuda.synchronize()
+                t0 = time.perf_counter()
+                S.submit(views[0], offs[0])
+                for b in range(1, len(views)):
+                    S.submit(views[b], offs[b])
+                    S.collect(copy=False)
                 S.collect(copy=False)
-            S.collect(copy=False)
-            dt = time.perf_counter() - t0
-        stream["config1"] = {"views": len(views), "views_per_batch": 1, "views_per_s": len(views) / dt,
-                             "ms_per_view": dt / len(views) * 1e3, "microscope_rate_hz": 5.0}
-        S.close(); del S
-        torch.cuda.empty_cache()
+                dt = time.perf_counter() - t0
+            stream["config1"] = {"views": len(views), "views_per_batch": 1, "views_per_s": len(views) / dt,
+                                 "ms_per_view": dt / len(views) * 1e3, "microscope_rate_hz": 5.0}
+            S.close(); del S
+            torch.cuda.empty_cache()
+        except Exception as exc:                              # an extra leg may not take the headline down with it
+            stream = {"error": f"{type(exc).__name__}: {exc}"}
+            torch.cuda.empty_cache()
 
     recog = None
     if args.recognize_views > 0:
-        from emu_synth import CONFIGS, make_view
-        from emu_synth.voxels import PITCH_Q, THRESHOLD, render_stack
-        shape = (40, 1024, 1280)                                   # the paper's view: 1280 x 1024 px x 40 frames
-        NV = args.recognize_views
-        stacks = []
-        for v in range(NV):
-            g = make_view(CONFIGS[1], 1, v)[0].astype(np.int64)
-            g = g[(g[:, 0] < shape[2] * PITCH_Q[0]) & (g[:, 1] < shape[1] * PITCH_Q[1])]      # the part of the view the stack covers
-            stacks.append(render_stack(shape, g, key=(8, v)))
-        vox = np.stack(stacks)
-        d_vox = torch.from_numpy(vox).cuda()
-        cap = 1 << 20
-        d_g = torch.empty((cap, 4), dtype=torch.int32, device="cuda"); d_o = torch.empty(NV + 1, dtype=torch.int32, device="cuda")
-        d_c = torch.zeros(1, dtype=torch.int64, device="cuda"); d_s = torch.zeros(1, dtype=torch.int64, device="cuda")
-        ws = torch.empty(E.emu_recognize_ws_bytes(NV, shape[1], shape[0], cap), dtype=torch.uint8, device="cuda")
-        for _ in range(3):
-            E.emu_recognize_grains(d_vox, THRESHOLD, PITCH_Q, d_g, d_o, d_c, d_s, ws)
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record()
-        for _ in range(5):
-            E.emu_recognize_grains(d_vox, THRESHOLD, PITCH_Q, d_g, d_o, d_c, d_s, ws)
-        e1.record(); torch.cuda.synchronize()
-        ms = e0.elapsed_time(e1) / 5
-        ng = int(d_c.cpu()[0])
-        from oracle.recognize import recognize_grains as oracle_recognize     # the reported CPU baseline of this stage
-        t0 = time.perf_counter(); ref = oracle_recognize(vox[0], THRESHOLD, PITCH_Q); t_or = time.perf_counter() - t0
-        n0 = int(d_o.cpu()[1])
-        same = bool(n0 == len(ref) and np.array_equal(d_g[:n0].cpu().numpy(), ref))
-        alg = vox.size + 16.0 * ng + 4.0 * NV * shape[0] * shape[1]
-        recog = {"views": NV, "voxels_per_view": int(vox[0].size), "grains": ng, "ms": ms, "views_per_s": NV / (ms * 1e-3),
-                 "roofline": {"bound": "hbm", "achieved": alg / (ms * 1e-3) / 1e9, "peak": float(peaks["hbm_gbs"]), "unit": "GB/s",
-                              "frac": alg / (ms * 1e-3) / 1e9 / float(peaks["hbm_gbs"]),
-                              "algorithmic": "1 B per voxel + 16 B per grain + 4 B per row of voxels"},
-                 "cpu_baseline": {"kind": "oracle (numpy)", "views_per_s": 1.0 / t_or, "cores": 1},
-                 "first_view_identical_to_oracle": same}
-        del d_vox
+        try:
+            from emu_synth import CONFIGS, make_view
+            from emu_synth.voxels import PITCH_Q, THRESHOLD, render_stack
+            shape = (40, 1024, 1280)                                   # the paper's view: 1280 x 1024 px x 40 frames
+            NV = args.recognize_views
+            stacks = []
+            for v in range(NV):
+                g = make_view(CONFIGS[1], 1, v)[0].astype(np.int64)
+                g = g[(g[:, 0] < shape[2] * PITCH_Q[0]) & (g[:, 1] < shape[1] * PITCH_Q[1])]      # the part of the view the stack covers
+                stacks.append(render_stack(shape, g, key=(8, v)))
+            vox = np.stack(stacks)
+            d_vox = torch.from_numpy(vox).cuda()
+            cap = 1 << 20
+            d_g = torch.empty((cap, 4), dtype=torch.int32, device="cuda"); d_o = torch.empty(NV + 1, dtype=torch.int32, device="cuda")
+            d_c = torch.zeros(1, dtype=torch.int64, device="cuda"); d_s = torch.zeros(1, dtype=torch.int64, device="cuda")
+            ws = torch.empty(E.emu_recognize_ws_bytes(NV, shape[1], shape[0], cap), dtype=torch.uint8, device="cuda")
+            for _ in range(3):
+                E.emu_recognize_grains(d_vox, THRESHOLD, PITCH_Q, d_g, d_o, d_c, d_s, ws)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(5):
+                E.emu_recognize_grains(d_vox, THRESHOLD, PITCH_Q, d_g, d_o, d_c, d_s, ws)
+            e1.record(); torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1) / 5
+            ng = int(d_c.cpu()[0])
+            from oracle.recognize import recognize_grains as oracle_recognize     # the reported CPU baseline of this stage
+            t0 = time.perf_counter(); ref = oracle_recognize(vox[0], THRESHOLD, PITCH_Q); t_or = time.perf_counter() - t0
+            n0 = int(d_o.cpu()[1])
+            same = bool(n0 == len(ref) and np.array_equal(d_g[:n0].cpu().numpy(), ref))
+            alg = vox.size + 16.0 * ng + 4.0 * NV * shape[0] * shape[1]
+            recog = {"views": NV, "voxels_per_view": int(vox[0].size), "grains": ng, "ms": ms, "views_per_s": NV / (ms * 1e-3),
+                     "roofline": {"bound": "hbm", "achieved": alg / (ms * 1e-3) / 1e9, "peak": float(peaks["hbm_gbs"]), "unit": "GB/s",
+                                  "frac": alg / (ms * 1e-3) / 1e9 / float(peaks["hbm_gbs"]),
+                                  "algorithmic": "1 B per voxel + 16 B per grain + 4 B per row of voxels"},
+                     "cpu_baseline": {"kind": "oracle (numpy)", "views_per_s": 1.0 / t_or, "cores": 1},
+                     "first_view_identical_to_oracle": same}
+            del d_vox
+        except Exception as exc:                              # an extra leg may not take the headline down with it
+            recog = {"error": f"{type(exc).__name__}: {exc}"}
+            torch.cuda.empty_cache()
 
     val = n_total / (ms_step * 1e-3)
     line = {
