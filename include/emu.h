@@ -122,6 +122,31 @@ int emu_bin_grains(const emu_params* params, const int32_t* d_grains, const int3
                    int64_t n_grains, int32_t n_views, int32_t* d_sorted, int32_t* d_cell_start,
                    int64_t* d_status, void* d_ws, size_t ws_bytes, void* stream);
 
+/* A1 again, for callers that cannot hand over a workspace because they cannot allocate device memory at the point
+ * where a view has to be binned.  Who that is: the thread that follows the microscope (a view every 0.2 s),
+ * where a cudaMalloc or cudaFree would wait for every stream of the device and stall the camera copies running beside
+ * it; a plug-in inside a process whose own memory pool already holds the whole HBM, so a further allocation fails; a
+ * caller that was given input and output buffers by a framework and has no allocator of its own to ask for more.
+ * Same inputs, outputs, ordering and status as emu_bin_grains (the kernels are the same ones); only d_ws / ws_bytes are
+ * gone.  The scratch is a fixed block of EMU_BIN_NOALLOC_BYTES inside the library image: every GPU that loads the
+ * library holds it from load until the process exits, whether or not this call is ever made.
+ *  - Limit: emu_workspace_bytes(...)'s bin_bytes for the batch must be <= EMU_BIN_NOALLOC_BYTES (8 MiB: e.g. four
+ *    views of 64 k grains in 114 k cells each).  A larger batch gets EMU_ERR_CAPACITY before anything is
+ *    enqueued - split it into smaller calls, or use emu_bin_grains with a workspace.  emu_bin_noalloc_max_bytes() returns the limit.
+ *  - The call makes no cudaMalloc / cudaFree and calls nothing that does (kernel launches and cudaMemsetAsync on
+ *    `stream` only, with no emu_profile active).  The first call on each device looks up the device address of the
+ *    block (one cudaGetSymbolAddress, with the caller's current device); make that first call at set-up time, on the
+ *    device it will be used on and before any stream capture is begun; later calls on that device only read a table.
+ *  - All calls on one device share the one block.  Nothing in it has to be cleared by the caller: whatever must start at
+ *    zero is cleared on `stream` ahead of the kernels.  But two calls whose GPU work overlaps in time (different
+ *    streams, or two host threads) write the same scratch and corrupt each other: keep them on one stream or order
+ *    them with events.  emu_bin_grains with separate workspaces has no such restriction. */
+#define EMU_BIN_NOALLOC_BYTES (8u << 20)
+size_t emu_bin_noalloc_max_bytes(void);
+int emu_bin_grains_noalloc(const emu_params* params, const int32_t* d_grains, const int32_t* d_view_off,
+                           int64_t n_grains, int32_t n_views, int32_t* d_sorted, int32_t* d_cell_start,
+                           int64_t* d_status, void* stream);
+
 /* A2..A5 + A7: seeds -> tube count -> threshold -> exclusive association -> threshold -> order
  * (Fig. 4).
  *  in : d_sorted, d_cell_start as written by emu_bin_grains with the SAME params; d_view_off.

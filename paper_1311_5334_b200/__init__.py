@@ -7,9 +7,9 @@ built library, or without a CUDA device for the compute calls, everything here r
 """
 from .binding import (EMU_CNT, EMU_ST, EMU_STAGE, HostPath, StreamPath, Profile, emu_host_arena_bytes, FIT_DTYPE, TRACK_DTYPE, EmuError, PathBuffers, PathResult, emu_bin_grains,
                       emu_count_seeds, emu_find_tracks, emu_fit_tracks, emu_grid_cells, emu_workspace_bytes,
-                      emu_recognize_grains, emu_recognize_ws_bytes,
+                      emu_recognize_grains, emu_recognize_ws_bytes, emu_bin_grains_noalloc, emu_bin_noalloc_max_bytes,
                       exported_symbols, library_path, make_params, run_path)
 
 __all__ = ["EMU_CNT", "EMU_ST", "EMU_STAGE", "HostPath", "StreamPath", "Profile", "emu_host_arena_bytes", "FIT_DTYPE", "TRACK_DTYPE", "EmuError", "PathBuffers", "PathResult",
            "emu_bin_grains", "emu_count_seeds", "emu_find_tracks", "emu_fit_tracks", "emu_grid_cells",
-           "emu_workspace_bytes", "emu_recognize_grains", "emu_recognize_ws_bytes", "exported_symbols", "library_path", "make_params", "run_path"]
+           "emu_workspace_bytes", "emu_bin_grains_noalloc", "emu_bin_noalloc_max_bytes", "emu_recognize_grains", "emu_recognize_ws_bytes", "exported_symbols", "library_path", "make_params", "run_path"]

@@ -39,7 +39,8 @@ class emu_params(C.Structure):
 _SYMBOLS = ["emu_workspace_bytes", "emu_grid_cells", "emu_bin_grains", "emu_find_tracks", "emu_count_seeds",
             "emu_fit_tracks", "emu_host_arena_bytes", "emu_track_views_host", "emu_profile_create", "emu_profile_destroy", "emu_profile_begin", "emu_profile_end",
             "emu_profile_read", "emu_recognize_ws_bytes", "emu_recognize_grains", "emu_stream_arena_bytes", "emu_stream_create",
-            "emu_stream_destroy", "emu_stream_submit", "emu_stream_collect"]
+            "emu_stream_destroy", "emu_stream_submit", "emu_stream_collect", "emu_bin_noalloc_max_bytes",
+            "emu_bin_grains_noalloc"]
 EMU_STAGE = dict(bin_count=0, bin_scan=1, bin_scatter=2, bin_place=3, prep=4, vote=5, assoc=6, select=7, emit=8, fit=9,
                  seeds=10, cands=11, recog=12, generic=13)
 EMU_STAGE_COUNT = 16
@@ -64,6 +65,10 @@ def _load():
         L.emu_grid_cells.argtypes = [vp, C.POINTER(i32 * 3)]
         L.emu_bin_grains.restype = C.c_int
         L.emu_bin_grains.argtypes = [vp, vp, vp, i64, i32, vp, vp, vp, vp, sz, vp]
+        L.emu_bin_noalloc_max_bytes.restype = sz
+        L.emu_bin_noalloc_max_bytes.argtypes = []
+        L.emu_bin_grains_noalloc.restype = C.c_int
+        L.emu_bin_grains_noalloc.argtypes = [vp, vp, vp, i64, i32, vp, vp, vp, vp]
         L.emu_find_tracks.restype = C.c_int
         L.emu_find_tracks.argtypes = [vp, vp, vp, vp, i64, i32, vp, vp, vp, i64, vp, vp, sz, vp]
         L.emu_count_seeds.restype = C.c_int
@@ -172,6 +177,31 @@ def emu_bin_grains(params, d_grains, d_view_off, n_grains, n_views, d_sorted, d_
     _check(_load().emu_bin_grains(C.byref(params), _ptr(d_grains), _ptr(d_view_off), n_grains, n_views,
                                   _ptr(d_sorted), _ptr(d_cell_start), _ptr(d_status), _ptr(d_ws), _nbytes(d_ws),
                                   _stream()), "emu_bin_grains")
+
+
+def emu_bin_noalloc_max_bytes() -> int:
+    """Size of the scratch block built into the library (bytes): the largest `bin_bytes` emu_bin_grains_noalloc takes."""
+    return int(_load().emu_bin_noalloc_max_bytes())
+
+
+def emu_bin_grains_noalloc(params, d_grains, d_view_off, n_grains, n_views, d_sorted, d_cell_start, d_status):
+    """emu_bin_grains without the workspace argument, for code that must not (or cannot) allocate device memory where
+    it bins a view: an acquisition loop that may not stall the device with a cudaMalloc, a plug-in next to a memory
+    pool that already owns the GPU, a callee that only receives input and output tensors.  The scratch is a fixed
+    8 MiB block inside libemu4pi.so (held by every GPU that loads the library); batches whose `bin_bytes`
+    (emu_workspace_bytes) exceed it are refused.  Calls on one device share the block, so do not let two of them
+    overlap on the GPU; call it once at set-up on each device (the first call resolves the block's device address).
+    Results are those of emu_bin_grains, bit for bit."""
+    import torch
+    _dev(d_grains, torch.int32); _dev(d_view_off, torch.int32); _dev(d_sorted, torch.int32)
+    _dev(d_cell_start, torch.int32); _dev(d_status, torch.int64)
+    rc = _load().emu_bin_grains_noalloc(C.byref(params), _ptr(d_grains), _ptr(d_view_off), n_grains, n_views,
+                                        _ptr(d_sorted), _ptr(d_cell_start), _ptr(d_status), _stream())
+    if rc == -2:
+        raise EmuError(f"emu_bin_grains_noalloc: this batch ({n_grains} grains, {n_views} views) needs more scratch than the "
+                       f"{emu_bin_noalloc_max_bytes()} bytes built into the library (EMU_ERR_CAPACITY): bin fewer views per "
+                       "call or use emu_bin_grains with a workspace")
+    _check(rc, "emu_bin_grains_noalloc")
 
 
 def emu_find_tracks(params, d_sorted, d_cell_start, d_view_off, n_grains, n_views, d_tracks, d_track_off, d_members,

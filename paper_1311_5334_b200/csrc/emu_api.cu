@@ -2,6 +2,7 @@
 // the path runs in the kernels of emu_bin.cu / emu_find.cu / emu_fit.cu.
 #include <math.h>
 
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -440,6 +441,64 @@ int emu_fit_tracks(const emu_params* params, const int32_t* d_grains, const emu_
   if (!d_tracks || !d_track_off || !d_members || !d_fits) return EMU_ERR_INVALID;   // d_grains may be NULL when there are no grains
   if (!aligned16(d_grains) || !aligned16(d_tracks) || ((uintptr_t)d_fits & 7)) return EMU_ERR_INVALID;
   return emu_fit_launch(d_grains, d_tracks, d_track_off, d_members, n_views, d_fits, (cudaStream_t)stream);
+}
+
+}  // extern "C"
+
+// ---- emu_bin_grains_noalloc: A1 for callers that have no device memory to give as a workspace --------------------
+// (include/emu.h has the contract.)  The binning kernels need scratch next to their inputs and outputs: the per-cell
+// counters, the staging copy of the grains between the two passes, the per-view redo flags and chunk cursors.  The
+// normal entry point takes it from the caller; this one keeps a fixed block of it inside the library image, so every
+// device that loads libemu4pi.so carries EMU_BIN_NOALLOC_BYTES of it until the process exits, used or not.
+//
+// g_bin_scratch below is a DEVICE array.  On the host its name is only a handle for the runtime - not an address a
+// kernel may be given - so the device address is asked for once per device with cudaGetSymbolAddress, with that device
+// current, and it is this address that goes to the launcher.
+static __device__ __align__(256) unsigned char g_bin_scratch[EMU_BIN_NOALLOC_BYTES];
+
+namespace {
+constexpr int kNoallocMaxDevices = 64;
+std::mutex g_noalloc_mu;
+void* g_noalloc_ptr[kNoallocMaxDevices];          // device address of g_bin_scratch on device i, NULL = not asked yet
+
+// the scratch of the CURRENT device (first call on a device: one cudaGetSymbolAddress; afterwards a table look-up)
+int noalloc_scratch(void** out) {
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess) return EMU_ERR_CUDA;
+  if (dev < 0 || dev >= kNoallocMaxDevices) return EMU_ERR_INVALID;
+  std::lock_guard<std::mutex> lock(g_noalloc_mu);
+  if (!g_noalloc_ptr[dev]) {
+    void* p = nullptr;
+    if (cudaGetSymbolAddress(&p, g_bin_scratch) != cudaSuccess || !p) return EMU_ERR_CUDA;
+    g_noalloc_ptr[dev] = p;
+  }
+  *out = g_noalloc_ptr[dev];
+  return EMU_OK;
+}
+}  // namespace
+
+extern "C" {
+
+size_t emu_bin_noalloc_max_bytes(void) { return (size_t)EMU_BIN_NOALLOC_BYTES; }
+
+int emu_bin_grains_noalloc(const emu_params* params, const int32_t* d_grains, const int32_t* d_view_off, int64_t n_grains,
+                           int32_t n_views, int32_t* d_sorted, int32_t* d_cell_start, int64_t* d_status, void* stream) {
+  if (!params_ok(params)) return EMU_ERR_INVALID;
+  EmuDev d = make_dev(params);
+  if (!shape_ok(d, n_grains, n_views)) return EMU_ERR_INVALID;
+  if (!d_view_off || !d_cell_start || !d_status) return EMU_ERR_INVALID;
+  if (n_grains > 0 && (!d_grains || !d_sorted)) return EMU_ERR_INVALID;
+  if (!aligned16(d_grains) || !aligned16(d_sorted)) return EMU_ERR_INVALID;
+  // the size check comes first and runs on the host alone: a batch beyond the fixed block is refused before any CUDA call
+  if (emu_bin_ws_bytes(d, n_grains, n_views) > (size_t)EMU_BIN_NOALLOC_BYTES) return EMU_ERR_CAPACITY;
+  void* scratch = nullptr;
+  const int rc = noalloc_scratch(&scratch);
+  if (rc != EMU_OK) return rc;
+  // the block still holds whatever the previous call left in it.  The launcher does not rely on its contents: what has
+  // to start at zero (redo flags, chunk cursors, the global counters of the counting-sort path) it clears itself with
+  // cudaMemsetAsync on `stream`, ahead of the kernels, exactly as it does for a caller's uninitialised workspace.
+  return emu_bin_launch(d, 0, d_grains, d_view_off, n_grains, n_views, d_sorted, d_cell_start, d_status, scratch,
+                        (size_t)EMU_BIN_NOALLOC_BYTES, (cudaStream_t)stream);
 }
 
 }  // extern "C"
