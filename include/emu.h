@@ -53,8 +53,9 @@ typedef struct emu_params {
   int32_t max_tracks_per_view; /* capacity of the track list per view, 1..65536                            */
   int32_t reserved[4];         /* sizing hints for the internal chunks of emu_find_tracks:                 */
                                /* [0] = expected candidates per grain (0 = default 48; 48 B each),         */
-                               /* [1] = expected seeds per grain (0 = default 192; 160 B each: geometry,   */
-                               /*       counter and the hit record of the voting pass); [2], [3] must be 0 */
+                               /* [1] = expected seeds per grain (0 = default 192; 240 B each: geometry,   */
+                               /*       counter, the hit record of the voting pass and 2.5 per-brick list  */
+                               /*       records of 32 B); [2], [3] must be 0                               */
   int32_t angle_min_grains[8]; /* angle-dependent cut on the number of grains (Fig. 8(c): "a cut on */
                                /* the number of grains is applied according to the line drawn in the       */
                                /* figure"; the line is not given, hence a table - reading Q17): entry k    */
@@ -90,7 +91,10 @@ typedef struct emu_fit {       /* 48 B */
 #define EMU_CNT_MEMBERS 4
 #define EMU_CNT_STATUS 5       /* 0 = fine, else OR of the EMU_ST_* bits                                   */
 #define EMU_CNT_PAIR_TESTS 6   /* pair-distance tests executed (implementation figure)                     */
-#define EMU_CNT_NEED 7         /* largest seed count one internal chunk needed                             */
+#define EMU_CNT_NEED 7         /* largest seed CAPACITY one internal chunk needed: its seeds, or - when a   */
+                               /* seed's line crosses many bricks (fine cells, whole-line tube) - its      */
+                               /* per-brick list records / 2.5, whichever is larger.  After                */
+                               /* EMU_ST_SEED_OVERFLOW: raise reserved[1] to NEED / (grains of the chunk)  */
 #define EMU_ST_CAND_OVERFLOW 1    /* candidate workspace too small: give more workspace / raise reserved[0] */
 #define EMU_ST_TRACK_OVERFLOW 2   /* a view has more than max_tracks_per_view tracks                       */
 #define EMU_ST_MEMBER_OVERFLOW 4  /* members_capacity too small                                            */

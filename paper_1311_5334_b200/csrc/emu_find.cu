@@ -405,7 +405,7 @@ k_view_scan(const int* __restrict__ view_off, int v0, int v1, unsigned* __restri
 __global__ void __launch_bounds__(1024)
 k_chunk_offsets(int nv, const unsigned* __restrict__ tot, unsigned* __restrict__ off, unsigned* __restrict__ total_out,
                 unsigned cap, unsigned status_bit, FindCtl* __restrict__ ctl, unsigned long long* __restrict__ counts,
-                int count_slot, int need_slot) {
+                int count_slot, int need_slot, unsigned need_num, unsigned need_den) {
   __shared__ unsigned long long warp_sum[32];
   __shared__ unsigned long long carry_s;
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
@@ -437,7 +437,9 @@ k_chunk_offsets(int nv, const unsigned* __restrict__ tot, unsigned* __restrict__
     const unsigned long long total = carry_s;
     off[nv] = (unsigned)min(total, 0xffffffffull);
     if (count_slot >= 0) atomicAdd(counts + count_slot, total);
-    if (need_slot >= 0) atomicMax(counts + need_slot, total);
+    // what the chunk needed, in units of the seed capacity (a list that is sized as need_den / need_num entries per seed
+    // reports the seed capacity that would have held it)
+    if (need_slot >= 0) atomicMax(counts + need_slot, (total * need_num + need_den - 1) / need_den);
     if (total > cap) {
       atomicOr(counts + EMU_CNT_STATUS, (unsigned long long)status_bit);
       ctl->skip = 1;
@@ -2048,7 +2050,7 @@ static int vote_chunk(const EmuDev& P, const Tilings& TT, FindWs& W, const Frame
       d_view_off, v0, v1, W.seed_off, plane, W.view_seed_tot, counts));
   EMU_LAUNCH(EMU_STAGE_SEEDS, st, k_chunk_offsets<<<1, 1024, 0, st>>>(
       3 * nv, W.view_seed_tot, W.view_seed_off, &W.ctl->seed_count, (unsigned)W.seed_cap, (unsigned)EMU_ST_SEED_OVERFLOW,
-      W.ctl, counts, EMU_CNT_SEEDS, EMU_CNT_NEED));
+      W.ctl, counts, EMU_CNT_SEEDS, EMU_CNT_NEED, 1u, 1u));
   EMU_LAUNCH(EMU_STAGE_SEEDS, st, k_seed_pairs<1><<<kSM * 16, kVoteThreads, 0, st>>>(
       P, sorted, d_cell_start, d_view_off, v0, v1, W.seed_off, plane, W.view_seed_off, W.ctl, W.geo, W.ab, counts));
   // only the counters of the seeds this chunk has are cleared (the count is on the device)
@@ -2063,7 +2065,7 @@ static int vote_chunk(const EmuDev& P, const Tilings& TT, FindWs& W, const Frame
   else EMU_LAUNCH(EMU_STAGE_SEEDS, st, k_prep<0, false><<<gp, 256, 0, st>>>(P, W.ctl, W.view_seed_off, W.geo, W.bricks, W.vf_bricks, W.brick_cnt, nullptr, nullptr));
   EMU_LAUNCH(EMU_STAGE_SEEDS, st, k_chunk_offsets<<<1, 1024, 0, st>>>(
       (int)(W.brick_cap * W.prep_sub), W.brick_cnt, W.brick_off, &W.ctl->prep_count, (unsigned)W.prep_cap, (unsigned)EMU_ST_SEED_OVERFLOW,
-      W.ctl, counts, -1, -1));
+      W.ctl, counts, -1, EMU_CNT_NEED, 8u, (unsigned)kPrepPerSeed8));      // prep_cap = seed_cap * kPrepPerSeed8 / 8: NEED is in seeds
   EMU_CK(cudaMemsetAsync(W.brick_cnt, 0, (W.brick_cap * W.prep_sub + 1) * sizeof(unsigned), st));
   if (P.ext >= 0) EMU_LAUNCH(EMU_STAGE_SEEDS, st, k_prep<1, true><<<gp, 256, 0, st>>>(P, W.ctl, W.view_seed_off, W.geo, W.bricks, W.vf_bricks, W.brick_cnt, W.brick_off, W.prec));
   else EMU_LAUNCH(EMU_STAGE_SEEDS, st, k_prep<1, false><<<gp, 256, 0, st>>>(P, W.ctl, W.view_seed_off, W.geo, W.bricks, W.vf_bricks, W.brick_cnt, W.brick_off, W.prec));
@@ -2115,10 +2117,10 @@ int emu_find_launch(const EmuDev& P, int seeds_per_grain, int cand_per_grain, co
         nullptr, nullptr, nullptr, nullptr, counts));
     EMU_LAUNCH(EMU_STAGE_CANDS, st, k_chunk_offsets<<<1, 1024, 0, st>>>(
         3 * nv, W.view_cand_cnt, W.view_cand_off, &W.ctl->cand_count, (unsigned)W.cand_cap, (unsigned)EMU_ST_CAND_OVERFLOW,
-        W.ctl, counts, EMU_CNT_CANDIDATES, -1));
+        W.ctl, counts, EMU_CNT_CANDIDATES, -1, 1u, 1u));
     EMU_LAUNCH(EMU_STAGE_CANDS, st, k_chunk_offsets<<<1, 1024, 0, st>>>(
         3 * nv, W.view_ovf_cnt, W.view_ovf_off, &W.ctl->ovf_count, (unsigned)W.cand_cap, (unsigned)EMU_ST_CAND_OVERFLOW,
-        W.ctl, counts, -1, -1));
+        W.ctl, counts, -1, -1, 1u, 1u));
     EMU_CK(cudaMemsetAsync(W.view_cand_cnt, 0, (3 * (size_t)nv + 1) * sizeof(unsigned), st));
     EMU_CK(cudaMemsetAsync(W.view_ovf_cnt, 0, (3 * (size_t)nv + 1) * sizeof(unsigned), st));
     EMU_LAUNCH(EMU_STAGE_CANDS, st, k_cands<1><<<dim3(gx, 3 * nv), 256, 0, st>>>(

@@ -113,8 +113,9 @@ def test_batch_of_views_in_several_chunks(E, oracle_mod):
     ref = oracle_mod.track_views(p, b.grains, b.view_off, "cells", 0)
     prm = E.make_params(**{k: p[k] for k in ("view_size_q", "cell_size_q", "sep_min_q", "sep_max_q", "tube_r2_q", "min_grains")})
     _, rec = E.emu_workspace_bytes(prm, b.n_grains, b.n_views)
-    # the recommendation holds all 7 views at once; the minimum seed / candidate capacity (1 Mi seeds of 160 B:
-    # geometry, counter and hit records) holds about 3 views of this shape at the default hint of 192 seeds per grain
+    # the recommendation holds all 7 views at once; the minimum seed / candidate capacity (1 Mi seeds of 240 B:
+    # geometry, counter, hit records and per-brick list records) holds about 3 views of this shape at the default
+    # hint of 192 seeds per grain
     for ws in (None, 300 << 20):
         got = run_gpu(E, p, b.grains, b.view_off, find_ws_bytes=ws)
         assert_same_tracks(E, got, ref)
@@ -391,6 +392,36 @@ def test_device_side_overflows_are_reported_and_harmless(E, oracle_mod):
     out = status_of(prm, find_ws_bytes=E.emu_workspace_bytes(prm, b.n_grains, b.n_views)[1])
     assert int(out["counts"][E.EMU_CNT["status"]]) & E.EMU_ST["cand_overflow"]
     assert_same_tracks(E, run_gpu(E, p, b.grains, b.view_off), ref)
+
+
+def test_per_brick_list_overflow_reports_what_it_needs(E, config_oracle):
+    """The per-brick lists of prepared seeds hold 2.5 records per place of the seed list.  With 0.5 um cells along u a
+    (view, frame) of config 1 has more than four bricks and a whole line crosses most of them: the seeds themselves fit
+    a workspace sized for 70 seeds per grain (63 are found), their (seed, brick) records do not.  The call must say so
+    (EMU_ST_SEED_OVERFLOW) AND report in EMU_CNT_NEED a seed capacity that is enough - a caller who resizes from it
+    succeeds at the next attempt - not the seed count, which already fitted."""
+    import torch
+    from gpu_helpers import gpu_params
+    b, p, ref = config_oracle(1)
+    p = dict(p, cell_size_q=default_params(1, cell_um=(0.5, 4.0, 4.0))["cell_size_q"])
+    d_grains = torch.from_numpy(b.grains).cuda(); d_off = torch.from_numpy(b.view_off).cuda()
+
+    def run(spg):
+        prm = gpu_params(E, p, seeds_per_grain=spg)
+        B = E.PathBuffers(prm, b.n_grains, b.n_views, find_ws_bytes=E.emu_workspace_bytes(prm, b.n_grains, b.n_views)[1])
+        res = E.run_path(prm, d_grains, d_off, b.n_views, B)
+        torch.cuda.synchronize()
+        return res.host()
+    spg = 70
+    assert ref.counters["seeds"] <= spg * b.n_grains                       # the seed list itself is large enough
+    out = run(spg)
+    assert int(out["counts"][E.EMU_CNT["status"]]) == E.EMU_ST["seed_overflow"]
+    assert int(out["counts"][E.EMU_CNT["seeds"]]) == ref.counters["seeds"]
+    need = int(out["counts"][E.EMU_CNT["need"]])
+    assert need > spg * b.n_grains, "NEED must exceed the capacity that failed"
+    out = run((need + b.n_grains - 1) // b.n_grains)                        # resize from NEED, as emu.h says
+    assert_same_tracks(E, out, ref)
+    assert int(out["counts"][E.EMU_CNT["need"]]) == need                   # the same records, now held
 
 
 @pytest.mark.parametrize("cell_um", [(8.0, 8.0, 8.0), (4.0, 4.0, 4.0), (3.0, 4.0, 2.5)])
