@@ -540,8 +540,7 @@ SplitPlan split_plan(const EmuDev& P, int frame, int64_t n_grains, int32_t n_vie
 #define EMU_BIN_GROUP_MB (1 << 20)
 #endif
 int split_group_views(const SplitPlan& S, int32_t n_views) {
-  static int mb = 0;
-  if (!mb) { const char* e = getenv("EMU_BIN_GROUP_MB"); mb = e ? atoi(e) : EMU_BIN_GROUP_MB; if (mb < 1) mb = EMU_BIN_GROUP_MB; }   // (tuning hook)
+  const int mb = EMU_BIN_GROUP_MB;                   // compile-time only: the library reads no environment
   const int64_t per_view = (int64_t)S.K * S.cap * 16;
   const int64_t g = emu_max64(1, ((int64_t)mb << 20) / emu_max64(1, per_view));
   return (int)emu_min64(emu_min64(g, 65535), emu_max64(1, n_views));
