@@ -37,7 +37,9 @@ VIEW_AREA_CM2 = 350e-4 * 300e-4  # 350 x 300 um = 1.05e-3 cm^2 per view
 # them live; the constants serve the runs that have no such leg (N > 1).
 ALG_PER_SEED = {(8.0, 8.0, 8.0): (317.7, 2.88), (3.0, 4.0, 4.0): (102.1, 2.26)}
 INSTR_PER_TEST, INSTR_PER_PAIR = 18, 10    # read off the SASS: profiles/r2_sass_counts.md
-MIX_PEAK_SHARE = 99.3 / 128.0    # measured issue rate of the tube-test instruction mix / nominal issue rate (mb_pipes.cu)
+MIX_PEAK_SHARE = 99.3 / 128.0    # measured issue rate of the tube-test instruction mix / nominal issue rate: the committed
+                                 # round-2 run (profiles/r2_mb_pipes.md).  Used only when the live leg below is off or fails.
+MIX_SASS_PER_PAIR = 52           # SASS instructions of one pair-iteration of k_mix (profiles/r2_mb_pipes.md: 104 per two)
 BIN_BYTES_PER_GRAIN = 32.0       # 16 B read + 16 B written per grain; + 4 B per cell of the grid
 # DRAM bytes (read + write) of one k_brick<kVote> launch per view of the launch, from the committed ncu --set full
 # capture profiles/r2_k_brick_full.txt (33 views: 50.48 GB read + 28.86 GB written)
@@ -75,6 +77,23 @@ def params_dict():
     p = default_params(CFG, cell_um=CELL_UM, max_tracks_per_view=4096)
     p["tube_ext_q"] = TUBE_EXT_Q
     return p
+
+
+def measure_mix_peak():
+    """The measured issue peak of the voting kernel's own instruction mix, from THIS run: compile
+    microbench/mb_pipes.cu to a temporary directory, run it on the current GPU and read its k_mix line."""
+    import re
+    import tempfile
+    from paper_1311_5334_b200 import build as lib_build
+    with tempfile.TemporaryDirectory() as tmp:
+        exe = lib_build.build_microbench(tmp)
+        out = subprocess.run([exe], check=True, capture_output=True, text=True, timeout=120).stdout      # device 0, as the N = 1 run
+    pairs = float(re.search(r"=\s*([0-9.]+) lane-pairs / clk / SM", out).group(1))
+    ffma = re.search(r"^FFMA\s+[0-9.]+\s+([0-9.]+)", out, flags=re.M)
+    per_clk = pairs * MIX_SASS_PER_PAIR
+    return {"lane_instr_per_clk_sm": per_clk, "share_of_nominal": per_clk / 128.0, "lane_pairs_per_clk_sm": pairs,
+            "sass_instr_per_pair": MIX_SASS_PER_PAIR, "ffma_lane_ops_per_clk_sm": float(ffma.group(1)) if ffma else None,
+            "source": "microbench/mb_pipes.cu (k_mix) compiled and run inside this bench run"}
 
 
 class ClockSampler:
@@ -228,6 +247,9 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cell-um", type=float, nargs=3, default=None, help="override the cell size of the 3D hash (um)")
+    ap.add_argument("--mix-peak", type=int, default=1,
+                    help="1: compile and run microbench/mb_pipes.cu and report the measured issue peak of the voting kernel's "
+                         "instruction mix as roofline.mix_peak_measured (N = 1 only); 0: the committed round-2 figure")
     ap.add_argument("--latency-views", type=int, default=8,
                     help="also time single views one at a time through the host call (SURVEY 8(f) NEXT-3: the microscope "
                          "delivers one view every 0.2 s, P:102); adds the key single_view to the JSON line")
@@ -358,8 +380,10 @@ def main():
     cpu = None
     alg = ALG_PER_SEED.get(tuple(CELL_UM))
     parity = None
+    ref_tracks = None                                         # the oracle's result for views 0..nv_s-1 (kept for the streamed leg)
     if world == 1 and not args.no_cpu_baseline:
         dt, ng, cnt, ref = oracle_sample(nv_s, cores)
+        ref_tracks = ref
         # parity of what was TIMED: views 0..nv_s-1 of the last timed device step and of the last timed host call
         # against the oracle, element by element (SURVEY 8(c) comparison rule)
         parity = {"views_checked": nv_s, "tracks_checked": int(len(ref.tracks)), "members_checked": int(len(ref.members)),
@@ -375,6 +399,13 @@ def main():
 
     sm_max = float(peaks.get("sm_max_mhz") or 1965.0)
     alu_peak = 148 * 4 * 32 * sm_max * 1e6 / 1e12            # Tlane-instr/s
+    mix_peak = None
+    if args.mix_peak and world == 1:
+        try:
+            mix_peak = measure_mix_peak()
+        except Exception as exc:                              # an extra leg may not take the headline down with it
+            mix_peak = {"error": f"{type(exc).__name__}: {exc}"}
+    mix_share = mix_peak["share_of_nominal"] if mix_peak and "share_of_nominal" in mix_peak else MIX_PEAK_SHARE
     vote_ms = stage_ms["vote"] / max(1, stage_launches["vote"])
     roofline = None
     if alg is not None and stage_launches["vote"]:
@@ -386,9 +417,11 @@ def main():
         roofline = {"kernel": "k_brick<kVote> (A3 tube count + hit records on shared-memory bricks, three frames; the seeds of "
                               "A2 arrive as per-brick lists of prepared records)", "bound": "alu", "achieved": achieved, "peak": alu_peak,
                     "unit": "Tlane-instr/s", "frac": achieved / alu_peak,
-                    "frac_of_mix_peak": achieved / (alu_peak * MIX_PEAK_SHARE),
-                    "mix_peak_source": "profiles/r2_mb_pipes.md: the tube-test instruction mix sustains 99.3 of 128 "
-                                       "lane-instr per clock and SM",
+                    "frac_of_mix_peak": achieved / (alu_peak * mix_share),
+                    "mix_peak_measured": mix_peak,
+                    "mix_peak_source": ("measured in this run (mix_peak_measured)" if mix_share is not MIX_PEAK_SHARE else
+                                        "profiles/r2_mb_pipes.md (round-2 capture): the tube-test instruction mix sustains 99.3 of "
+                                        "128 lane-instr per clock and SM"),
                     "frac_on_kernel_tests": achieved / alu_peak * (gpu_tests * INSTR_PER_TEST + alg[1] * INSTR_PER_PAIR)
                                             / (alg[0] * INSTR_PER_TEST + alg[1] * INSTR_PER_PAIR),
                     "traffic": VOTE_DRAM_BYTES_PER_VIEW * views_per_launch if captured else None,
@@ -471,6 +504,12 @@ def main():
                 nt_s += S.collect(copy=False)["n_tracks"]
                 dt = time.perf_counter() - t0
             assert SV < V or nt_s == int(counts[E.EMU_CNT["tracks"]]), "the streamed batches and the one-call path disagree"
+            # parity of the streamed path itself, element by element: views 0..nv_s-1 as ONE batch through the same
+            # emu_stream object (the timed rounds above read only the counts back), against the oracle's result
+            if parity is not None and ref_tracks is not None and nv_s <= min(BV, SV):
+                S.submit(grains[:off[nv_s]], off[:nv_s + 1].astype(np.int32))
+                parity["stream"] = same_as_oracle(S.collect(copy=True), ref_tracks)
+                parity["identical"] = bool(parity["identical"] and parity["stream"])
             stream["config4"] = {"views": SV, "views_per_batch": BV, "grains_per_s": float(off[SV]) / dt, "views_per_s": SV / dt,
                                  "ms_per_view": dt / SV * 1e3, "tracks": nt_s,
                                  "call": "emu_stream_submit / emu_stream_collect, two batches in flight, pinned host buffers"}

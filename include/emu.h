@@ -235,7 +235,13 @@ int emu_track_views_host(const emu_params* params, const int32_t* h_grains, cons
  *               copy-out stream (while the next batch computes) and returns when they have arrived.  Outputs and
  *               return codes as emu_track_views_host.
  * With submit(k+1) called before collect(k), the input copy of k+1 and the output copy of k-1 hide behind the
- * kernels of k.  Every batch must satisfy n_grains <= max_grains, n_views <= max_views. */
+ * kernels of k.  Every batch must satisfy n_grains <= max_grains, n_views <= max_views.
+ * The three streams are the object's own (non-blocking) and are not ordered against any stream of the caller: d_arena
+ * must be IDLE when emu_stream_create is called (no work still queued anywhere that reads or writes it - with a caching
+ * allocator, synchronise the stream it was last used on) and must not be touched by the caller until destroy.
+ * If submit fails after part of the batch was queued (a launcher's error code, EMU_ERR_CUDA), it drains its copy-in and
+ * compute streams before returning: the batch does not count as in flight, nothing is left running, and the next
+ * submit may follow. */
 typedef struct emu_stream emu_stream;
 int emu_stream_arena_bytes(const emu_params* params, int64_t max_grains, int32_t max_views, size_t* arena_bytes);
 emu_stream* emu_stream_create(const emu_params* params, int64_t max_grains, int32_t max_views, void* d_arena,

@@ -322,6 +322,9 @@ class StreamPath:
         b = C.c_size_t(0)
         _check(_load().emu_stream_arena_bytes(C.byref(params), max_grains, max_views, C.byref(b)), "emu_stream_arena_bytes")
         self.arena = torch.empty(int(b.value), dtype=torch.uint8, device="cuda")
+        # the library works on three streams of its own, which know nothing of torch's: the block the caching allocator
+        # has just handed out may still be in use by work queued on the current stream, so let that finish first
+        torch.cuda.current_stream().synchronize()
         self._h = _load().emu_stream_create(C.byref(params), max_grains, max_views, _ptr(self.arena), _nbytes(self.arena))
         if not self._h:
             raise EmuError("emu_stream_create failed")

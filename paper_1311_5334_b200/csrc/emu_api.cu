@@ -374,22 +374,35 @@ int emu_stream_submit(emu_stream* S, const int32_t* h_grains, const int32_t* h_v
   auto& L = S->slot[S->submitted & 1];
   const EmuDev& d = S->dev;
   // the slot's buffers are free: its previous batch was collected (collect waits for the kernels and the output copy)
-  if (n_grains > 0 && cudaMemcpyAsync(L.grains, h_grains, (size_t)n_grains * 16, cudaMemcpyHostToDevice, S->s_in) != cudaSuccess) return EMU_ERR_CUDA;
-  if (cudaMemcpyAsync(L.view_off, h_view_off, ((size_t)n_views + 1) * 4, cudaMemcpyHostToDevice, S->s_in) != cudaSuccess) return EMU_ERR_CUDA;
-  if (cudaEventRecord(L.in_done, S->s_in) != cudaSuccess) return EMU_ERR_CUDA;
-  if (cudaStreamWaitEvent(S->s_run, L.in_done, 0) != cudaSuccess) return EMU_ERR_CUDA;
-  cudaStream_t st = S->s_run;
-  if (cudaMemsetAsync(L.status, 0, 8, st) != cudaSuccess) return EMU_ERR_CUDA;
-  int rc = emu_bin_launch(d, 0, L.grains, L.view_off, n_grains, n_views, S->sorted, S->cell_start, L.status, S->ws, S->ws_bytes, st);
-  if (rc != EMU_OK) return rc;
-  rc = emu_find_launch(d, seeds_per_grain(&S->params), cand_per_grain(&S->params), S->sorted, S->cell_start, L.view_off, n_grains, n_views,
-                       L.tracks, L.track_off, L.members, n_grains, L.counts, S->ws, S->ws_bytes, st);
-  if (rc != EMU_OK) return rc;
-  rc = emu_fit_launch(L.grains, L.tracks, L.track_off, L.members, n_views, L.fits, st);
-  if (rc != EMU_OK) return rc;
-  if (cudaMemcpyAsync(L.h_small, L.counts, 64, cudaMemcpyDeviceToHost, st) != cudaSuccess) return EMU_ERR_CUDA;
-  if (cudaMemcpyAsync(L.h_small + 8, L.status, 8, cudaMemcpyDeviceToHost, st) != cudaSuccess) return EMU_ERR_CUDA;
-  if (cudaEventRecord(L.run_done, st) != cudaSuccess) return EMU_ERR_CUDA;
+  auto enqueue = [&]() -> int {
+    if (n_grains > 0 && cudaMemcpyAsync(L.grains, h_grains, (size_t)n_grains * 16, cudaMemcpyHostToDevice, S->s_in) != cudaSuccess) return EMU_ERR_CUDA;
+    if (cudaMemcpyAsync(L.view_off, h_view_off, ((size_t)n_views + 1) * 4, cudaMemcpyHostToDevice, S->s_in) != cudaSuccess) return EMU_ERR_CUDA;
+    if (cudaEventRecord(L.in_done, S->s_in) != cudaSuccess) return EMU_ERR_CUDA;
+    if (cudaStreamWaitEvent(S->s_run, L.in_done, 0) != cudaSuccess) return EMU_ERR_CUDA;
+    cudaStream_t st = S->s_run;
+    if (cudaMemsetAsync(L.status, 0, 8, st) != cudaSuccess) return EMU_ERR_CUDA;
+    int rc = emu_bin_launch(d, 0, L.grains, L.view_off, n_grains, n_views, S->sorted, S->cell_start, L.status, S->ws, S->ws_bytes, st);
+    if (rc != EMU_OK) return rc;
+    rc = emu_find_launch(d, seeds_per_grain(&S->params), cand_per_grain(&S->params), S->sorted, S->cell_start, L.view_off, n_grains, n_views,
+                         L.tracks, L.track_off, L.members, n_grains, L.counts, S->ws, S->ws_bytes, st);
+    if (rc != EMU_OK) return rc;
+    rc = emu_fit_launch(L.grains, L.tracks, L.track_off, L.members, n_views, L.fits, st);
+    if (rc != EMU_OK) return rc;
+    if (cudaMemcpyAsync(L.h_small, L.counts, 64, cudaMemcpyDeviceToHost, st) != cudaSuccess) return EMU_ERR_CUDA;
+    if (cudaMemcpyAsync(L.h_small + 8, L.status, 8, cudaMemcpyDeviceToHost, st) != cudaSuccess) return EMU_ERR_CUDA;
+    if (cudaEventRecord(L.run_done, st) != cudaSuccess) return EMU_ERR_CUDA;
+    return EMU_OK;
+  };
+  const int erc = enqueue();
+  if (erc != EMU_OK) {
+    // part of the batch may already be queued (copies, kernels).  Nothing of it will be collected - `submitted` does
+    // not advance - so drain both streams before handing the error back: the slot and the shared work buffers are
+    // idle again and the next submit may reuse them.  (A sticky CUDA error makes these calls fail too; the caller
+    // then sees EMU_ERR_CUDA from every later call and has to destroy the stream object.)
+    cudaStreamSynchronize(S->s_in);
+    cudaStreamSynchronize(S->s_run);
+    return erc;
+  }
   L.n_grains = n_grains; L.n_views = n_views;
   return (int)(S->submitted++ & 0x3fffffff);
 }

@@ -41,7 +41,7 @@ __global__ void __launch_bounds__(1024, 2) k_pipe(unsigned* out, unsigned a, uns
   if (acc == 0x12345678u) out[0] = acc;
 }
 
-// the instruction mix of one pair of tube tests as k_brick<kVote> issues it (profiles/r2_k_brick_sass_counts.md):
+// the instruction mix of one pair of tube tests as k_brick<kVote> issues it (profiles/r2_sass_counts.md):
 // 2 LDS stand-ins (shared loads), 6 PRMT, 8 FADD, 6 FMUL, 12 FFMA, 1 FMNMX, 3 FSETP / ISETP, 6 integer (IADD3 / LEA /
 // VIMNMX) - run here without the branches and the stores, on register operands and one shared-memory table
 __global__ void __launch_bounds__(1024, 2) k_mix(unsigned* out, unsigned a, float fa, float fb, float fc) {

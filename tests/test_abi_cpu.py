@@ -63,3 +63,10 @@ def test_compute_calls_refuse_host_tensors(E):
     t = torch.zeros((4, 4), dtype=torch.int32)
     with pytest.raises(E.EmuError):          # no CPU fallback: a host tensor is an error, not a slow path
         E.emu_bin_grains(prm, t, t, 4, 1, t, t, t, t)
+
+
+def test_microbenchmark_compiles_for_sm100a(tmp_path):
+    """microbench/mb_pipes.cu (the measured issue peak bench.py reports) is not part of build(); it must still compile"""
+    from paper_1311_5334_b200 import build as lib_build
+    exe = lib_build.build_microbench(str(tmp_path))
+    assert os.path.exists(exe) and os.path.getsize(exe) > 0
