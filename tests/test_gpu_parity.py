@@ -444,3 +444,26 @@ def test_bounded_tube_bit_exact(E, oracle_mod, cfg, ext_q, cell_um):
     assert_same_tracks(E, got, ref)
     whole = oracle_mod.track_views(default_params(cfg), b.grains, b.view_off, "cells", 1)
     assert ref.counters["candidates"] < whole.counters["candidates"]
+
+
+@pytest.mark.parametrize("variant", ["bounded_tube", "angle_cut"])
+def test_bounded_tube_and_angle_cut_on_config4_views(E, oracle_mod, variant):
+    """The two extensions at the density and geometry bench.py times (config 4 in 3 x 4 x 4 um cells: three bricks per
+    (view, frame), so the clip of a bounded seed against SEVERAL bricks and the angle cut's per-view compaction at 1 400
+    tracks per view are exercised): four views, once with the bounded tube of 20 um as `bench.py --tube-ext-um 20`
+    runs it and once with the sloping angle table, against the oracle element by element."""
+    import bench
+    V = 4
+    grains, off = bench.make_workload(0, V)
+    p = dict(bench.params_dict())
+    if variant == "bounded_tube":
+        p["tube_ext_q"] = 1280
+    else:
+        p["angle_min_grains"] = [14, 13, 12, 11, 10, 9, 9, 8]
+    ref = oracle_mod.track_views(p, grains, off, "cells", 0)
+    # the extension does change the list: fewer tracks than the contract gives on the same views (the oracle's stored
+    # per-view counts, tests/golden/config4_view_digests.json)
+    with open(os.path.join(HERE, "golden", "config4_view_digests.json")) as f:
+        whole = sum(x["n_tracks"] for x in json.load(f)["views"][:V])
+    assert 0 < len(ref.tracks) < whole
+    assert_same_tracks(E, run_gpu(E, p, grains, off), ref)
