@@ -2,7 +2,7 @@
 // pure IADD3, pure IMAD, pure IMAD.WIDE and the kernel's own mix; the roofline for the reported fraction is the
 // measured peak of that mix").  A standalone measurement program, not part of libemu4pi.so:
 //
-//   nvcc -gencode arch=compute_100a,code=sm_100a -O3 -o mb_pipes paper_1311_5334_b200/csrc/mb_pipes.cu && ./mb_pipes
+//   nvcc -gencode arch=compute_100a,code=sm_100a -O3 -o mb_pipes paper_1311_5334_b200/microbench/mb_pipes.cu && ./mb_pipes
 //
 // Every kernel runs one instruction (or the instruction mix of the tube test) on 8 independent registers per
 // thread in a long unrolled loop, 2 blocks of 1 024 threads per SM (all 64 warps resident), and reports
@@ -26,18 +26,20 @@ __global__ void __launch_bounds__(1024, 2) k_pipe(unsigned* out, unsigned a, uns
 #pragma unroll
     for (int i = 0; i < 8; ++i) {
       if (kOp == 0) asm volatile("fma.rn.f32 %0, %0, %1, %2;" : "+f"(f[i]) : "f"(fa), "f"(fb));
-      if (kOp == 1) asm volatile("add.s32 %0, %0, %1;" : "+r"(r[i]) : "r"(a));
+      // (the second operand of the next three is the NEIGHBOURING register, which changes every iteration: with a loop
+      //  constant there ptxas folds two adds into one IADD3, drops the idempotent max and shortens the mad.wide chain)
+      if (kOp == 1) asm volatile("add.s32 %0, %0, %1;" : "+r"(r[i]) : "r"(r[(i + 1) & 7]));
       if (kOp == 2) asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(r[i]) : "r"(a), "r"(b));
       if (kOp == 3) asm volatile("prmt.b32 %0, %0, %1, %2;" : "+r"(r[i]) : "r"(a), "r"(b));
       if (kOp == 4) asm volatile("mad.lo.s32 %0, %0, %1, %2;" : "+r"(r[i]) : "r"(a), "r"(b));
-      if (kOp == 5) asm volatile("mad.wide.u32 %0, %1, %2, %0;" : "+l"(w[i]) : "r"(a), "r"(r[i]));
-      if (kOp == 6) asm volatile("max.f32 %0, %0, %1;" : "+f"(f[i]) : "f"(fa));
+      if (kOp == 5) asm volatile("mad.wide.u32 %0, %1, %2, %0;" : "+l"(w[i]) : "r"(a), "r"((unsigned)(w[(i + 1) & 7] >> 32)));   // the HIGH half: all 64 bits of the chain stay live
+      if (kOp == 6) asm volatile("max.f32 %0, %0, %1;" : "+f"(f[i]) : "f"(f[(i + 1) & 7]));
       if (kOp == 7) asm volatile("{ .reg .pred p; setp.gt.f32 p, %0, %1; selp.f32 %0, %0, %2, p; }" : "+f"(f[i]) : "f"(fa), "f"(fb));
     }
   }
   unsigned acc = 0;
 #pragma unroll
-  for (int i = 0; i < 8; ++i) acc += r[i] + __float_as_uint(f[i]) + (unsigned)w[i];
+  for (int i = 0; i < 8; ++i) acc += r[i] + __float_as_uint(f[i]) + (unsigned)w[i] + (unsigned)(w[i] >> 32);
   if (acc == 0x12345678u) out[0] = acc;
 }
 
@@ -97,10 +99,10 @@ int main() {
   cudaMalloc(&out, 256);
   const int blocks = sm * 2, threads = 1024;
   const double clk = (double)khz * 1e3;
-  const char* names[8] = {"FFMA", "IADD3 (add.s32)", "LOP3", "PRMT", "IMAD (mad.lo)", "IMAD.WIDE", "FMNMX", "FSETP+FSEL"};
+  const char* names[8] = {"FFMA", "add.s32 (IADD3|IMAD.IADD)", "LOP3", "PRMT", "IMAD (mad.lo)", "mad.wide.u32 + 64-bit acc", "FMNMX", "FSETP+FSEL"};
   const double per_iter[8] = {8, 8, 8, 8, 8, 8, 8, 16};
   printf("device: %d SMs, %.0f MHz\n", sm, clk / 1e6);
-  printf("%-18s %12s %22s\n", "instruction", "ms", "lane-ops / clk / SM");
+  printf("%-28s %12s %22s\n", "instruction", "ms", "lane-ops / clk / SM");
   double ms[8];
   ms[0] = time_ms([&] { k_pipe<0><<<blocks, threads>>>(out, 3u, 5u, 1.0001f, 0.5f); });
   ms[1] = time_ms([&] { k_pipe<1><<<blocks, threads>>>(out, 3u, 5u, 1.0001f, 0.5f); });
@@ -111,11 +113,11 @@ int main() {
   ms[6] = time_ms([&] { k_pipe<6><<<blocks, threads>>>(out, 3u, 5u, 1.0001f, 0.5f); });
   ms[7] = time_ms([&] { k_pipe<7><<<blocks, threads>>>(out, 3u, 5u, 1.0001f, 0.5f); });
   for (int k = 0; k < 8; ++k)
-    printf("%-18s %12.4f %22.1f\n", names[k], ms[k], per_iter[k] * kIters * (double)blocks * threads / (ms[k] * 1e-3 * clk * sm));
+    printf("%-28s %12.4f %22.1f\n", names[k], ms[k], per_iter[k] * kIters * (double)blocks * threads / (ms[k] * 1e-3 * clk * sm));
   const double mix_ms = time_ms([&] { k_mix<<<blocks, threads>>>(out, 1664525u, 3.f, 5.f, 7.f); });
   // instructions of one iteration of k_mix are counted from its SASS (cuobjdump -sass mb_pipes | the loop of k_mix):
   // the figure printed is per SOURCE iteration; multiply by the SASS count to get lane-instructions per clock
-  printf("%-18s %12.4f %22s\n", "tube-test mix", mix_ms, "(see iterations/clk)");
+  printf("%-28s %12.4f %22s\n", "tube-test mix", mix_ms, "(see iterations/clk)");
   printf("tube-test mix: %.3f pair-iterations / clk / SM per lane-group of 32 = %.2f lane-pairs / clk / SM\n",
          (double)kIters * blocks * threads / 32.0 / (mix_ms * 1e-3 * clk * sm), (double)kIters * blocks * threads / (mix_ms * 1e-3 * clk * sm));
   cudaFree(out);
